@@ -1,0 +1,308 @@
+"""Pins for the oracle's equilibrium, equations of motion, weight equation and RK4 (no GPU).
+
+SURVEY.md section 8(c) pins P5-P11, P15.  Each is a property fixed by the paper's equations
+(Eq.(2)-(8), L45-65, L314) or by vector calculus; none re-types the oracle's formulas.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+from scipy.integrate import quad
+
+from oracle import Oracle
+from paper_2606_24327_b200 import synth
+
+
+def _eq(o, R, Z):
+    return o.equil(R, Z)
+
+
+@pytest.fixture(scope="module", params=["cfg0", "cfg1-equilibrium"])
+def eq_case(request, cfg0_oracle):
+    """(cfg, oracle): config 0 (R0 = B0 = 1) and config 1's equilibrium (R0 = 1.67, B0 = 2, q1 != 0), so that a
+    dropped factor of R0, B0 or a cannot hide behind a unit value."""
+    if request.param == "cfg0":
+        cfg, RZ, tri, o, _ = cfg0_oracle
+        return cfg, o
+    cfg = dataclasses.replace(synth.CONFIGS[1], nr=4, ntheta=12, n_planes=8, em=True)
+    RZ, tri = synth.make_mesh(cfg)
+    o = Oracle()
+    o.equilibrium_set(**synth.equilibrium_args(cfg))
+    o.species_set(**synth.species_args(cfg))
+    o.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+    return cfg, o
+
+
+# P5 ---------------------------------------------------------------------------------------
+def test_P5_field_line_pitch_averages_to_q(eq_case):
+    """(1/2pi) oint (B_phi/R)/(B_theta/r) dtheta = q(r): the sqrt(1-eps^2) in qbar (reading R10) is exactly
+    what makes the prescribed q(r) the field-line safety factor.  Golden values: q(r) from BASELINE
+    config 0, q = 1.4 + 0.5 (r/a)^2."""
+    cfg, o = eq_case
+    q0, q1, q2 = cfg.q  # BASELINE.json configs[0] / configs[1]
+    gold = [(x, q0 + q1 * x + q2 * x * x) for x in (0.25, 0.5, 0.75, 0.9)]
+    for r_over_a, q_expected in gold:
+        r = r_over_a * cfg.a
+
+        def pitch(th):
+            R, Z = cfg.R0 + r * np.cos(th), r * np.sin(th)
+            e = _eq(o, R, Z)
+            bth = -np.sin(th) * e["B_R"] + np.cos(th) * e["B_Z"]
+            return (e["B_phi"] / R) / (bth / r)
+
+        val, _ = quad(pitch, 0, 2 * np.pi, epsabs=1e-13, epsrel=1e-13)
+        assert abs(val / (2 * np.pi) - q_expected) < 1e-11, (r_over_a, val / (2 * np.pi), q_expected)
+        assert abs(_eq(o, cfg.R0 + r, 0.0)["q"] - q_expected) < 1e-14
+        assert pitch(0.3) > 0  # B_theta, B_phi > 0: cos(m theta - n phi) with m ~ nq is field aligned (R11)
+
+
+# P6 ---------------------------------------------------------------------------------------
+def test_P6_divB_gradB_curlb_by_finite_differences(eq_case):
+    cfg, o = eq_case
+    rng = np.random.default_rng(0)
+    h = 1e-5
+    for _ in range(10):
+        r, th = cfg.a * rng.uniform(0.1, 0.95), rng.uniform(0, 2 * np.pi)
+        R, Z = cfg.R0 + r * np.cos(th), r * np.sin(th)
+        e = _eq(o, R, Z)
+        eRp, eRm, eZp, eZm = _eq(o, R + h, Z), _eq(o, R - h, Z), _eq(o, R, Z + h), _eq(o, R, Z - h)
+        d = lambda k, p, m_: (p[k] - m_[k]) / (2 * h)
+        # div B = (1/R) d_R (R B_R) + d_Z B_Z  (axisymmetric)
+        divB = ((R + h) * eRp["B_R"] - (R - h) * eRm["B_R"]) / (2 * h) / R + d("B_Z", eZp, eZm)
+        assert abs(divB) < 1e-8 * e["B"] / cfg.a
+        assert abs(d("B", eRp, eRm) - e["gradB_R"]) < 1e-8 * e["B"] / cfg.a
+        assert abs(d("B", eZp, eZm) - e["gradB_Z"]) < 1e-8 * e["B"] / cfg.a
+        assert e["gradB_phi"] == 0.0
+        assert abs(e["b_R"] ** 2 + e["b_phi"] ** 2 + e["b_Z"] ** 2 - 1) < 1e-15
+        curl = np.array([-d("b_phi", eZp, eZm),
+                         d("b_R", eZp, eZm) - d("b_Z", eRp, eRm),
+                         ((R + h) * eRp["b_phi"] - (R - h) * eRm["b_phi"]) / (2 * h) / R])
+        got = np.array([e["curlb_R"], e["curlb_phi"], e["curlb_Z"]])
+        assert np.abs(curl - got).max() < 1e-8 / cfg.a
+        # independent route: curl b = (curl B + b x grad B)/B with curl B = (0, d_Z B_R - d_R B_Z, 0)
+        cB = np.array([0.0, d("B_R", eZp, eZm) - d("B_Z", eRp, eRm), 0.0])
+        b = np.array([e["b_R"], e["b_phi"], e["b_Z"]])
+        gB = np.array([e["gradB_R"], 0.0, e["gradB_Z"]])
+        bxg = np.array([b[1] * gB[2] - b[2] * gB[1], b[2] * gB[0] - b[0] * gB[2], b[0] * gB[1] - b[1] * gB[0]])
+        assert np.abs((cB + bxg) / e["B"] - got).max() < 1e-8 / cfg.a
+        # psi'' is the derivative of psi'
+        p1p, p1m = _eq(o, cfg.R0 + r + h, 0.0)["psi1"], _eq(o, cfg.R0 + r - h, 0.0)["psi1"]
+        assert abs((p1p - p1m) / (2 * h) - _eq(o, cfg.R0 + r, 0.0)["psi2"]) < 1e-7
+
+
+# helpers -----------------------------------------------------------------------------------
+def _energy(o, cfg, R, Z, phi, u, mu):
+    g, _ = o.gather(R, Z, phi)
+    B = np.array([o.equil(r, z)["B"] for r, z in zip(R, Z)])
+    return 0.5 * u * u + mu * B + cfg.qom * (g[0] - u * g[4])
+
+
+def _psi_of_r(o, cfg, r):
+    return quad(lambda t: o.equil(cfg.R0 + t, 0.0)["psi1"], 0.0, r, epsabs=1e-15, epsrel=1e-14)[0]
+
+
+def _pphi(o, cfg, R, Z, u):
+    out = np.zeros(R.shape[0])
+    for i, (r_, z_, u_) in enumerate(zip(R, Z, u)):
+        e = o.equil(r_, z_)
+        out[i] = cfg.qom * _psi_of_r(o, cfg, e["r"]) + u_ * e["F"] / e["B"]
+    return out
+
+
+def _smooth_case(P=8, n=400, seed=21, zero=False):
+    """Small unstructured mesh carrying GLOBAL QUARTIC fields on all planes (inside the element space, n = 0):
+    the interpolated field is then a C-infinity function, so RK4 shows its full order."""
+    cfg = dataclasses.replace(synth.CONFIGS[0], structured=False, nr=5, ntheta=14, n_planes=P, seed=seed, n_markers=n,
+                              R0=1.3, B0=1.7, a=0.4, q=(1.4, 0.1, 0.5))  # no unit-valued parameter
+    RZ, tri = synth.make_mesh(cfg)
+    o = Oracle()
+    o.equilibrium_set(**synth.equilibrium_args(cfg))
+    o.species_set(**synth.species_args(cfg))
+    o.mesh_load(RZ, tri, P, cfg.phi_period)
+    rng = np.random.default_rng(seed)
+    nod = np.zeros((2, RZ.shape[0], 6))
+    if not zero:
+        for f in range(2):
+            co = {(i, j): rng.normal() * 2e-3 for i in range(5) for j in range(5 - i)}
+            X, Y = (RZ[:, 0] - cfg.R0) / cfg.a, RZ[:, 1] / cfg.a
+            for q, (dx, dy) in enumerate([(0, 0), (1, 0), (0, 1), (2, 0), (1, 1), (0, 2)]):
+                s = 0.0
+                for (i, j), c in co.items():
+                    if i < dx or j < dy:
+                        continue
+                    k = c * np.prod([i - t for t in range(dx)]) * np.prod([j - t for t in range(dy)])
+                    s = s + k * X ** (i - dx) * Y ** (j - dy)
+                nod[f, :, q] = s / cfg.a ** (dx + dy)
+    for f in range(2):
+        o.fields_set(f, np.broadcast_to(nod[f], (P,) + nod[f].shape).copy())
+    m = synth.make_markers(cfg, n)
+    keep = np.hypot(m["R"] - cfg.R0, m["Z"]) < 0.75 * cfg.a  # stay clear of the outer boundary
+    m = {k: v[keep] for k, v in m.items()}
+    return cfg, o, m
+
+
+# P7 + P9 -----------------------------------------------------------------------------------
+def test_P7_P9_rk4_fourth_order_and_energy_with_smooth_fields():
+    """Static fields: E = u^2/2 + mu B + qom (Phi - u A) is an invariant of Eq.(2)-(6) (p_par form, R6), so RK4's
+    drift falls 16x per halving of dt; so does the self-convergence error of every state component."""
+    cfg, o, m = _smooth_case()
+    T = 0.4
+    E0 = _energy(o, cfg, m["R"], m["Z"], m["phi"], m["u"], m["mu"])
+    res = {}
+    for n in (4, 8, 16, 32):
+        res[n] = o.push_rk4(m["R"], m["Z"], m["phi"], m["u"], m["w"], m["mu"], m["p"], T / n, n)
+        assert (res[n][5] == 0).all()
+    drift = {n: np.abs(_energy(o, cfg, *res[n][:4], m["mu"]) - E0).max() for n in res}
+    assert drift[4] / drift[8] > 11 and drift[8] / drift[16] > 11, drift
+    assert drift[32] < 1e-7 * np.abs(E0).max(), drift
+    err = {n: max(np.abs(res[n][q] - res[32][q]).max() for q in (0, 1, 3, 4)) for n in (4, 8, 16)}
+    # Richardson: e(4)-ish ratios; (e4-e32)/(e8-e32) -> (16^3-1)/(16^2-1)*... ~ 16.06, (e8-e32)/(e16-e32) ~ 17
+    assert 12 < err[4] / err[8] < 20 and 13 < err[8] / err[16] < 21, err
+
+
+def test_P7_energy_drift_with_genuine_FE_fields(cfg0_oracle):
+    """Config 0's helical FE fields (non-axisymmetric, only C1): energy is still an invariant of the flow because
+    the gather returns the exact gradient of the interpolant; the drift is tiny and falls with dt (order is
+    reduced by the C0 gradient kinks at element edges - not a bug)."""
+    cfg, RZ, tri, o, _ = cfg0_oracle
+    m = synth.make_markers(cfg, 1500)
+    E0 = _energy(o, cfg, m["R"], m["Z"], m["phi"], m["u"], m["mu"])
+    d = {}
+    for n in (5, 10, 20):
+        r = o.push_rk4(m["R"], m["Z"], m["phi"], m["u"], m["w"], m["mu"], m["p"], 0.25 / n, n)
+        ok = r[5] == 0
+        d[n] = np.median(np.abs(_energy(o, cfg, r[0][ok], r[1][ok], r[2][ok], r[3][ok], m["mu"][ok]) - E0[ok]) / np.abs(E0[ok]))
+    assert d[5] < 1e-6 and d[5] / d[10] > 2.5 and d[10] / d[20] > 2.5, d
+
+
+# P8 ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("charge_sign", [1.0, -1.0])
+def test_P8_canonical_toroidal_momentum(charge_sign):
+    """Axisymmetric case (zero perturbation): P_phi = qom psi(r) + u F/B is conserved at 4th order with
+    b* = B*/B*_par (reading R7).  The literal L53 expression b + (m/q) u curl b / B*_par drifts at a dt-independent
+    level - that is how the reading was chosen.  Run for both charge signs (R8)."""
+    cfg, o, m = _smooth_case(zero=True, n=120)
+    sp = synth.species_args(cfg)
+    sp["qom"] *= charge_sign
+    cfg = dataclasses.replace(cfg)
+    T = 0.4
+
+    def run(bstar_exact, n):
+        o.species_set(**{**sp, "bstar_exact": bstar_exact})
+        r = o.push_rk4(m["R"], m["Z"], m["phi"], m["u"], m["w"], m["mu"], m["p"], T / n, n)
+        qom = sp["qom"]
+        P1 = np.array([qom * _psi_of_r(o, cfg, o.equil(a, b)["r"]) + c * o.equil(a, b)["F"] / o.equil(a, b)["B"] for a, b, c in zip(r[0], r[1], r[3])])
+        P0 = np.array([qom * _psi_of_r(o, cfg, o.equil(a, b)["r"]) + c * o.equil(a, b)["F"] / o.equil(a, b)["B"] for a, b, c in zip(m["R"], m["Z"], m["u"])])
+        return np.abs(P1 - P0) / np.abs(P0).max()
+
+    d4, d8, d16 = run(1, 4), run(1, 8), run(1, 16)
+    # order from the median over markers (a few fast, strongly drifting markers are still pre-asymptotic at dt = 0.1)
+    assert np.median(d4) / np.median(d8) > 12 and np.median(d8) / np.median(d16) > 12, (np.median(d4), np.median(d8), np.median(d16))
+    assert d16.max() < 5e-9, d16.max()
+    l4, l16 = run(0, 4), run(0, 16)
+    assert np.median(l16) > 1000 * np.median(d16) and 0.5 < np.median(l4) / np.median(l16) < 2.0  # dt-independent drift
+    o.species_set(**synth.species_args(cfg))
+
+
+# P10 --------------------------------------------------------------------------------------
+def test_P10_flat_profile_weight_closed_form():
+    """kappa_n = kappa_T = 0 (flat n, T = 1) and static fields: Eq.(7) integrates exactly to
+    w(t) - w(0) = -(p qom/T) [ (Phi - u A)(t) - (Phi - u A)(0) ]  (dE/dt = 0 and f0 = f0(E))."""
+    cfg, o, m = _smooth_case(n=300)
+    sp = synth.species_args(cfg)
+    sp.update(kappa_n=0.0, kappa_T=0.0)
+    o.species_set(**sp)
+    p = 0.5 + np.arange(m["R"].shape[0]) % 3  # not all ones
+    g0, _ = o.gather(m["R"], m["Z"], m["phi"])
+    diffs = []
+    for n in (8, 16):
+        r = o.push_rk4(m["R"], m["Z"], m["phi"], m["u"], m["w"], m["mu"], p, 0.4 / n, n)
+        g1, _ = o.gather(r[0], r[1], r[2])
+        pred = -(p * cfg.qom) * ((g1[0] - r[3] * g1[4]) - (g0[0] - m["u"] * g0[4]))
+        got = r[4] - m["w"]
+        diffs.append(np.abs(got - pred).max() / np.abs(pred).max())
+    assert diffs[1] < 1e-6 and diffs[0] / diffs[1] > 10, diffs
+    # nonlinear weight mode (p - w): dw/dt = (p - w) * L  =>  ln((p - w)/(p - w0)) = -int L = linear-result/p
+    sp2 = dict(sp, weight_mode=1)
+    o.species_set(**sp2)
+    r2 = o.push_rk4(m["R"], m["Z"], m["phi"], m["u"], m["w"], m["mu"], p, 0.4 / 16, 16)
+    o.species_set(**sp)
+    r1 = o.push_rk4(m["R"], m["Z"], m["phi"], m["u"], m["w"], m["mu"], p, 0.4 / 16, 16)
+    lin = (r1[4] - m["w"]) / p
+    assert np.abs(np.log((p - r2[4]) / (p - m["w"])) + lin).max() < 1e-5 * max(np.abs(lin).max(), 1e-3)  # RK4 truncation at dt = 0.025
+
+
+# P11 --------------------------------------------------------------------------------------
+def test_P11_grad_ln_f0_by_finite_differences(eq_case):
+    """Eq.(8) profiles (L314) inside a Maxwellian (L63): the analytic gradients used in Eq.(7) equal central
+    differences of ln f0; and ln f0(u=0, mu=0) = ln n - 1.5 ln T with n, T from Eq.(8) as printed (L314),
+    evaluated here in 30-digit arithmetic with r0 = a/2 (L316)."""
+    cfg, o = eq_case
+    rng = np.random.default_rng(1)
+    h = 1e-6
+    for _ in range(12):
+        r, th = cfg.a * rng.uniform(0.15, 0.9), rng.uniform(0, 2 * np.pi)
+        R, Z, u, mu = cfg.R0 + r * np.cos(th), r * np.sin(th), rng.normal(), rng.exponential()
+        g = o.grad_ln_f0(R, Z, u, mu)
+        fd = np.array([(o.ln_f0(R + h, Z, u, mu) - o.ln_f0(R - h, Z, u, mu)) / (2 * h),
+                       (o.ln_f0(R, Z + h, u, mu) - o.ln_f0(R, Z - h, u, mu)) / (2 * h),
+                       (o.ln_f0(R, Z, u + h, mu) - o.ln_f0(R, Z, u - h, mu)) / (2 * h)])
+        assert np.abs(g - fd).max() < 2e-8 * max(1.0, np.abs(fd).max()), (g, fd)
+    import mpmath as mp
+    mp.mp.dps = 30
+    for r_over_a in (0.2, 0.5, 0.8):
+        H = lambda kap, w: mp.exp(-kap * w * (mp.mpf(cfg.a) / cfg.R0) * mp.tanh((r_over_a * mp.mpf(cfg.a) - mp.mpf(cfg.a) / 2) / (w * mp.mpf(cfg.a))))
+        expect = mp.log(H(cfg.kappa_n, cfg.w_n)) - mp.mpf(3) / 2 * mp.log(H(cfg.kappa_T, cfg.w_T))
+        val = o.ln_f0(cfg.R0 + r_over_a * cfg.a, 0.0, 0.0, 0.0)
+        assert abs(val - float(expect)) < 1e-13
+
+
+# P15 --------------------------------------------------------------------------------------
+def test_P15_infinite_charge_limit_follows_field_lines():
+    """qom -> infinity (kappa = m/q -> 0), zero fields, mu = 0: Eq.(2) reduces to dX/dt = u b, so r is constant and
+    the toroidal angle advances by int (B_phi/R)/(B_theta/r) dtheta along the orbit (with P5: q(r) per turn)."""
+    cfg, o, m = _smooth_case(zero=True, n=60)
+    sp = synth.species_args(cfg)
+    sp.update(qom=1e13, kappa_n=0.0, kappa_T=0.0)
+    o.species_set(**sp)
+    mu0 = np.zeros_like(m["mu"])
+    u = np.where(np.abs(m["u"]) < 0.3, 0.7, m["u"])
+    T, n = 0.6, 24
+    r = o.push_rk4(m["R"], m["Z"], m["phi"], u, m["w"], mu0, m["p"], T / n, n)
+    r0 = np.hypot(m["R"] - cfg.R0, m["Z"])
+    r1 = np.hypot(r[0] - cfg.R0, r[1])
+    assert np.abs(r1 - r0).max() < 1e-9 * cfg.a
+    assert np.abs(r[3] - u).max() < 1e-12  # no mirror force, no field: u constant
+    for i in range(0, r0.shape[0], 7):
+        th0, th1 = np.arctan2(m["Z"][i], m["R"][i] - cfg.R0), np.arctan2(r[1][i], r[0][i] - cfg.R0)
+        th1 = th0 + np.angle(np.exp(1j * (th1 - th0)))  # short orbit: |dtheta| < pi
+
+        def pitch(th, rr=r0[i]):
+            R, Z = cfg.R0 + rr * np.cos(th), rr * np.sin(th)
+            e = o.equil(R, Z)
+            return (e["B_phi"] / R) / ((-np.sin(th) * e["B_R"] + np.cos(th) * e["B_Z"]) / rr)
+
+        dphi_pred = quad(pitch, th0, th1, epsabs=1e-13, epsrel=1e-13)[0]
+        dphi = np.angle(np.exp(1j * (r[2][i] - m["phi"][i])))
+        assert abs(dphi - dphi_pred) < 1e-8, (i, dphi, dphi_pred)
+    o.species_set(**synth.species_args(cfg))
+
+
+def test_lost_marker_status_and_zero_field_outside(cfg0_oracle):
+    """O9 / reading R15: a marker evaluated outside the mesh keeps moving in the equilibrium with zero perturbed
+    field and carries a sticky status flag; markers that stay inside are never flagged."""
+    cfg, RZ, tri, o, _ = cfg0_oracle
+    R = np.array([cfg.R0 + 0.999 * cfg.a, cfg.R0 + 0.5 * cfg.a])
+    Z = np.array([0.0, 0.0])
+    phi = np.array([0.1, 0.1])
+    u = np.array([0.5, 0.5])
+    mu = np.array([3.0, 0.1])  # large mu: grad-B drift pushes the first marker across the outer boundary
+    w = np.zeros(2)
+    p = np.ones(2)
+    out = o.push_rk4(R, Z, phi, u, w, mu, p, 0.05, 40)
+    assert out[5][1] == 0
+    r_end = np.hypot(out[0][0] - cfg.R0, out[1][0])
+    if r_end > cfg.a:
+        assert out[5][0] != 0
+    d, outside = o.rhs(np.array([cfg.R0 + 1.5 * cfg.a]), np.array([0.0]), phi[:1], u[:1], w[:1], mu[:1], p[:1])
+    assert outside[0] == 1 and np.isfinite(d).all() and d[4, 0] == 0.0
