@@ -1,0 +1,271 @@
+#!/usr/bin/env python
+"""Benchmark of the fused gather + RK4 marker push (BASELINE.json metric) on N B200s of one node.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--markers M] [--dt 0.05] [--impl reference]
+
+One step = one RK4 step of the whole hot path over all markers of the config (store, periodic sort by cell,
+locate, gather, equilibrium, equations of motion, weight, RK4 combine).  Prints ONE JSON line on rank 0.
+`value` = marker RK4 pushes/s with the markers resident in HBM; `e2e` = the same through the C-ABI with HOST
+buffers (H2D of the marker arrays and D2H of the result inside the timed region).
+--impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_24327_b200 import shard, synth  # noqa: E402
+
+METRIC = "marker RK4 pushes/sec incl. field gather (fp64, 1 B200), % of roofline"
+UNIT = "marker-pushes/s"
+FLOP_PER_PUSH = 3772.0          # 943 flop per RK stage x 4
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
+KEYS = ("R", "Z", "phi", "u", "w", "mu", "p")
+SORT_EVERY = 10                 # BASELINE configs[2]: "re-sorted by triangle every 10 steps"
+
+
+def make_inputs(cfg, n, start, pinned):
+    """Markers [start, start+n) in chunks; returns dict of numpy arrays (views of pinned torch tensors if pinned)."""
+    import torch
+    host = {k: (torch.empty(n, dtype=torch.float64, pin_memory=True) if pinned else torch.empty(n, dtype=torch.float64)) for k in KEYS}
+    views = {k: v.numpy() for k, v in host.items()}
+    chunk = 5_000_000
+    for s in range(0, n, chunk):
+        e = min(n, s + chunk)
+        m = synth.make_markers(cfg, e - s, start + s)
+        for k in KEYS:
+            views[k][s:e] = m[k]
+    return host, views
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=lambda: [self.lines.append(l) for l in self.proc.stdout], daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def setup_case(cfg, backend):
+    RZ, tri = synth.make_mesh(cfg)
+    dphi, dap = synth.make_fields(cfg, RZ)
+    backend.equilibrium_set(**synth.equilibrium_args(cfg))
+    backend.species_set(**synth.species_args(cfg))
+    backend.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+    backend.fields_set(0, dphi)
+    backend.fields_set(1, dap)
+    return RZ, tri, (dphi, dap)
+
+
+def time_oracle(cfg, n_sample, steps, start=0):
+    """The oracle as it stands on the host cores: pushes/s on n_sample markers x steps RK4 steps."""
+    from oracle import Oracle, oracle_threads
+    o = Oracle()
+    setup_case(cfg, o)
+    m = synth.make_markers(cfg, n_sample, start)
+    args = [m[k] for k in KEYS]
+    t0 = time.perf_counter()
+    o.push_rk4(*args, cfg.dt, steps)
+    dt = time.perf_counter() - t0
+    return n_sample * steps / dt, oracle_threads(), dt
+
+
+def run_reference(args, cfg, rank, world):
+    if rank != 0:
+        return
+    n_sample = args.ref_markers
+    from oracle import Oracle, oracle_threads
+    o = Oracle()
+    setup_case(cfg, o)
+    m = synth.make_markers(cfg, n_sample, 0)
+    st = [m[k] for k in KEYS]
+    for _ in range(args.warmup):
+        o.push_rk4(*[a[: max(1, n_sample // 10)] for a in st], cfg.dt, 1)
+    t0 = time.perf_counter()
+    cur = st
+    for _ in range(args.steps):
+        r = o.push_rk4(*cur, cfg.dt, 1)
+        cur = [r[0], r[1], r[2], r[3], r[4], st[5], st[6]]
+    el = time.perf_counter() - t0
+    val = n_sample * args.steps / el
+    sample = f"{n_sample} markers of {cfg.name} (of {cfg.n_markers}) per step"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(cfg, n_sample, args),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, n, args):
+    return {"workload": f"{cfg.name}: {2 * cfg.nr * cfg.ntheta} triangles x {cfg.n_planes} planes, {n} markers/GPU, EM={cfg.em}, dt={cfg.dt}, RK4, sort every {SORT_EVERY} steps",
+            "markers_per_gpu": n, "triangles": 2 * cfg.nr * cfg.ntheta, "planes": cfg.n_planes, "dt": cfg.dt, "push_variant": args.variant,
+            "l2": "inputs_exceed_l2" if n * 104 > 126e6 else "l2_flushed_between_steps"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--markers", type=int, default=None, help="markers per GPU (default: the config's)")
+    ap.add_argument("--dt", type=float, default=None)
+    ap.add_argument("--variant", type=int, default=0, help="0 tiled push kernel, 1 simple")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-sample", type=int, default=400_000, help="markers of the oracle cpu_baseline leg (x 4 steps)")
+    ap.add_argument("--ref-markers", type=int, default=200_000, help="markers per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    import dataclasses
+    cfg = synth.CONFIGS[args.config]
+    if args.dt is not None:
+        cfg = dataclasses.replace(cfg, dt=args.dt)
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, cfg, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2606_24327_b200.binding import Trimeg
+
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    n = args.markers if args.markers is not None else cfg.n_markers
+    start, _ = shard.marker_slice(n, rank, world)
+
+    g = Trimeg(local)
+    setup_case(cfg, g)
+    host, views = make_inputs(cfg, n, start, pinned=True)
+    dev = {k: v.cuda(non_blocking=True) for k, v in host.items()}
+    torch.cuda.synchronize()
+    g.set_push_variant(args.variant)
+    g.set_sort_interval(SORT_EVERY)
+    g.markers_bind(*[dev[k] for k in KEYS])
+    dfma = g.bench_dfma()
+
+    # ---- device-resident timing
+    for _ in range(args.warmup):
+        g.push_rk4(cfg.dt, 1)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    launches, sorted_steps, slow = 0, [], 0
+    ev[0].record()
+    for s in range(args.steps):
+        g.push_rk4(cfg.dt, 1)
+        ev[s + 1].record()
+        st = g.push_stats()
+        launches += st["launches"]
+        slow += st["slow_path"]
+        sorted_steps.append(st["sorts"] > 0)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if rank == 0 else None
+    step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
+    total_s = shard.reduce_max_seconds(sum(step_ms) * 1e-3, dist if world > 1 else None)
+    value = shard.job_rate(n * args.steps, world, total_s)
+    kern_ms = [t for t, srt in zip(step_ms, sorted_steps) if not srt] or step_ms
+    kern_s = statistics.mean(kern_ms) * 1e-3
+    achieved = FLOP_PER_PUSH * n / kern_s / 1e12
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned): H2D marker arrays, push, D2H result
+    pinned_out = {k: torch.empty(n, dtype=torch.float64, pin_memory=True).numpy() for k in ("R", "Z", "phi", "u", "w")}
+    pinned_out["status"] = torch.empty(n, dtype=torch.int32, pin_memory=True).numpy()
+    e2e_steps = max(1, min(args.e2e_steps, args.steps))
+
+    def e2e_step():
+        g.markers_bind(*[views[k] for k in KEYS])
+        g.push_rk4(cfg.dt, 1)
+        g.markers_get(host=True, pinned=pinned_out)
+
+    e2e_step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(e2e_steps):
+        e2e_step()
+    b.record()
+    torch.cuda.synchronize()
+    e2e_s = shard.reduce_max_seconds(a.elapsed_time(b) * 1e-3, dist if world > 1 else None)
+    e2e_val = shard.job_rate(n * e2e_steps, world, e2e_s)
+    checksum = float(pinned_out["w"][: min(n, 1000)].sum())
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, n, args), "clocks": clocks,
+                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 7 * 8 * n, "d2h_bytes_per_step": (5 * 8 + 4) * n, "steps": e2e_steps,
+                        "note": "bind(HOST) includes the first sort by cell; PCIe-bound"},
+                "gpu_launches": launches,
+                "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
+                             "traffic": None, "kernel": "k_push_tiled" if args.variant == 0 else "k_push_simple", "kernel_ms": 1e3 * kern_s,
+                             "flop_per_push": FLOP_PER_PUSH, "peak_kind": "nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (derived, DESIGN.md)",
+                             "measured_dfma_tflops": dfma, "frac_of_measured_dfma": achieved / dfma,
+                             "hbm_algorithmic_GBps": 121.0 * n / kern_s / 1e9},
+                "slow_path_evals": slow, "e2e_checksum": checksum}
+        if not args.no_cpu_baseline:
+            cpu_n = min(n, args.cpu_sample)
+            v, cores, secs = time_oracle(cfg, cpu_n, 4)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
+                                    "sample": f"first {cpu_n} markers of the same workload x 4 RK4 steps"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,145 @@
+/*
+ * trimeg.h -- C-ABI of the B200-native TRIMEG-C1 marker push (arxiv/paper_2606_24327).
+ *
+ * The library computes, for every marker of a gyrokinetic particle-in-cell run, the paper's
+ * "particle push" (section 3.2): locate the marker in the unstructured poloidal
+ * triangle mesh and its toroidal interval, interpolate the perturbed fields dPhi, dA_par and their
+ * gradients with the C1 finite element x toroidal cubic B-spline representation (L35), evaluate the
+ * equilibrium field, and advance the gyrocentre equations Eq.(2)-(6) (L45-55) and the delta-f weight
+ * equation Eq.(7) (L65) -- here fused into a 4-stage Runge-Kutta step on the device.
+ *
+ * Conventions
+ *   - plain C, no exceptions cross this boundary; every call returns 0 or a negative trimeg_status.
+ *   - all floating point is IEEE double; indices are int32; sizes int64.
+ *   - "memspace" says where a caller buffer lives: TRIMEG_HOST (pageable or pinned host memory) or
+ *     TRIMEG_DEVICE (memory of the context's CUDA device).  The caller owns every buffer it passes;
+ *     the library copies what it keeps, except the marker scratch (see trimeg_markers_bind).
+ *   - all work is enqueued on the CUDA stream given at trimeg_create and is asynchronous with
+ *     respect to the host unless the call returns data into HOST memory (then it synchronises).
+ *   - coordinates are right-handed cylindrical (R, phi, Z); marker state is stored (R, Z, phi, u, w).
+ *   - there is no CPU fallback: without a CUDA device trimeg_create fails with TRIMEG_ERR_CUDA.
+ */
+#ifndef TRIMEG_H
+#define TRIMEG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TRIMEG_OK = 0,
+    TRIMEG_ERR_BAD_ARG = -1,   /* null pointer, non-positive size, dt <= 0 or not finite, n_planes < 4 ... */
+    TRIMEG_ERR_BAD_STATE = -2, /* call order: e.g. fields_set before mesh_load, push before markers_bind */
+    TRIMEG_ERR_BAD_MESH = -3,  /* vertex index out of range, clockwise or degenerate triangle */
+    TRIMEG_ERR_CUDA = -4,      /* a CUDA runtime call failed; see trimeg_last_error */
+    TRIMEG_ERR_OOM = -5        /* device allocation failed or the bound scratch is too small */
+} trimeg_status;
+
+enum { TRIMEG_HOST = 0, TRIMEG_DEVICE = 1 };
+enum { TRIMEG_FIELD_PHI = 0, TRIMEG_FIELD_APAR = 1 };
+
+typedef struct trimeg_ctx trimeg_ctx;
+
+/* Create a context on CUDA device `device`; `cuda_stream` is a cudaStream_t (0/NULL = legacy default
+ * stream), typically torch.cuda.current_stream().cuda_stream.  *out is set only on success. */
+int trimeg_create(trimeg_ctx** out, int device, void* cuda_stream);
+int trimeg_destroy(trimeg_ctx* ctx);
+/* Block the host until everything enqueued on the context's stream has finished. */
+int trimeg_sync(trimeg_ctx* ctx);
+/* Human-readable text of the last error on this context ("" if none); valid until the next call. */
+const char* trimeg_last_error(const trimeg_ctx* ctx);
+
+/* Analytic concentric-circular tokamak equilibrium ("computes the equilibrium configuration of
+ * the magnetic field"; the paper's numeric B-spline equilibrium L87/L121 is replaced by the closed form the
+ * BASELINE configs give):  B = grad(psi) x grad(phi) + B0 R0 grad(phi),  psi'(r) = B0 r / qbar(r),
+ * q(r) = q0 + q1 r/a + q2 (r/a)^2,  qbar = q sqrt(1 - r^2/R0^2) if qbar_sqrt else q,  r^2 = (R-R0)^2 + Z^2. */
+typedef struct {
+    double R0, a, B0, q0, q1, q2;
+    int32_t qbar_sqrt;
+} trimeg_equil;
+int trimeg_equilibrium_set(trimeg_ctx* ctx, const trimeg_equil* eq);
+
+/* Species and equilibrium profiles.  qom = q_s/m_s in the normalised units of Eq.(2)-(6) (sign = charge sign);
+ * Eq.(8) (L314): H(r)/H(r0) = exp[-kappa_H w_H (a/R0) tanh((r - r0)/(w_H a))] for H = n, T.
+ * bstar_exact = 1: bstar = Bstar / Bstar_par with Bstar = B + (m/q) u curl b (default); 0: the literal expression printed at L53.
+ * weight_mode = 0: dw/dt = -p [...] (linear delta-f, default); 1: dw/dt = -(p - w) [...]. */
+typedef struct {
+    double qom;
+    double kappa_n, kappa_T, w_n, w_T, r0;
+    int32_t bstar_exact;
+    int32_t weight_mode;
+} trimeg_species;
+int trimeg_species_set(trimeg_ctx* ctx, const trimeg_species* sp);
+
+/* Poloidal mesh + toroidal grid (L35; positioning tables L89, L125-140 are built here, once).
+ * RZ: HOST [n_nodes][2] node coordinates; tri: HOST [n_tri][3] vertex indices, counter-clockwise.
+ * n_planes >= 4 uniform planes over [0, phi_period) (periodic).  Replaces any previous mesh and drops fields.
+ * Errors: BAD_ARG, BAD_MESH (index out of range, non-CCW/degenerate triangle), OOM, CUDA. */
+int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t n_tri, const int32_t* tri,
+                     int32_t n_planes, double phi_period);
+
+/* Nodal degrees of freedom of one perturbed field (L35 "field variables on the grid"):
+ * dof [n_planes][n_nodes][6] = (f, f_R, f_Z, f_RR, f_RZ, f_ZZ) per node, physical derivatives; per-plane
+ * values are toroidal B-spline coefficients.  Converted on the device to per-triangle polynomial
+ * coefficients.  A field never set is zero.  Errors: BAD_ARG, BAD_STATE (no mesh), OOM, CUDA. */
+int trimeg_fields_set(trimeg_ctx* ctx, int which, const double* dof, int memspace);
+
+/* Grid-to-particle interpolation at arbitrary points (the paper's G2P function, L35, L103):
+ * out [8][n] = Phi, dPhi/dR, dPhi/dZ, dPhi/dphi, Apar, dApar/dR, dApar/dZ, dApar/dphi (d/dphi is the raw
+ * angle derivative, not divided by R).  tri_out (nullable) [n]: index of the containing triangle in the
+ * caller's numbering, -1 = outside the mesh (outputs are then zero).  R, Z, phi, out, tri_out all live in
+ * `memspace`.  Errors: BAD_ARG, BAD_STATE (no mesh), CUDA. */
+int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi, double* out,
+                  int32_t* tri_out, int memspace);
+
+/* Bytes of DEVICE scratch trimeg_markers_bind needs for n markers (0 on error). */
+size_t trimeg_scratch_bytes(const trimeg_ctx* ctx, int64_t n);
+
+/* Hand n markers to the library (L89: R, Z, phi, v_par, w per marker; mu and p are constants of the motion).
+ * The seven arrays [n] live in `memspace` and are read once (copied into the library's structure-of-arrays
+ * store, which lives in `scratch`: DEVICE memory owned by the caller that must stay valid until the next
+ * bind/destroy; with TRIMEG_HOST inputs the call returns after the copies are enqueued from the caller's
+ * buffers, so those must stay valid until trimeg_sync).  Marker status is reset to 0.
+ * Errors: BAD_ARG, BAD_STATE (no mesh), OOM (scratch too small), CUDA. */
+int trimeg_markers_bind(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi,
+                        const double* u, const double* w, const double* mu, const double* p, int memspace,
+                        void* scratch, size_t scratch_bytes);
+
+/* Current marker state in the caller's original order.  Any pointer may be null (skipped).
+ * status bit 0: some RK stage was evaluated outside the mesh (zero perturbed field was used). */
+int trimeg_markers_get(trimeg_ctx* ctx, double* R, double* Z, double* phi, double* u, double* w, int32_t* status,
+                       int memspace);
+
+/* Re-sort the marker store by cell (triangle x toroidal interval) now / every n-th RK4 step (0 = never again;
+ * a sort is always done once after bind before the first push). */
+int trimeg_sort(trimeg_ctx* ctx);
+int trimeg_set_sort_interval(trimeg_ctx* ctx, int32_t every_n_steps);
+
+/* Advance all bound markers by nsteps classical RK4 steps of size dt with the fields frozen (north_star;
+ * the paper returns the five time derivatives to the host instead, L89).  phi is wrapped into
+ * [0, phi_period) after every step.  Errors: BAD_ARG (dt <= 0 or not finite, nsteps < 0), BAD_STATE
+ * (mesh, equilibrium, species or markers missing), CUDA. */
+int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps);
+
+/* One evaluation of the right-hand side for the bound markers in the caller's order -- the paper's own kernel
+ * boundary (L89: "time derivatives of R, Z, phi, v_par and the marker weights w").  out [5][n] in `memspace`. */
+int trimeg_rhs(trimeg_ctx* ctx, double* out, int memspace);
+
+/* Select the push kernel: 0 = tiled (cell-coherent gather through shared memory, default),
+ * 1 = simple (one thread per marker, coefficients through L1/L2).  Both compute the same thing. */
+int trimeg_set_push_variant(trimeg_ctx* ctx, int32_t variant);
+
+/* Diagnostics used by the benchmark: achieved FP64 FMA throughput of this device in TFLOP/s
+ * (a register-only DFMA loop; the roofline's measured "alu" peak). */
+int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops);
+/* Counters of the last trimeg_push_rk4 call: [0] kernel launches, [1] marker-stage evaluations that took the
+ * slow (out-of-tile) gather path, [2] markers flagged lost, [3] sorts done. */
+int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRIMEG_H */
