@@ -32,7 +32,7 @@ UNIT = "marker-pushes/s"
 FLOP_PER_PUSH = 3772.0          # 943 flop per RK stage x 4
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
 KEYS = ("R", "Z", "phi", "u", "w", "mu", "p")
-SORT_EVERY = 10                 # BASELINE configs[2]: "re-sorted by triangle every 10 steps"
+SORT_EVERY = 1                  # tiled kernel: re-bin every step (BASELINE configs[2] uses 10)
 
 
 def make_inputs(cfg, n, start, pinned):
@@ -137,8 +137,8 @@ def run_reference(args, cfg, rank, world):
 
 
 def workload_config(cfg, n, args):
-    return {"workload": f"{cfg.name}: {2 * cfg.nr * cfg.ntheta} triangles x {cfg.n_planes} planes, {n} markers/GPU, EM={cfg.em}, dt={cfg.dt}, RK4, sort every {SORT_EVERY} steps",
-            "markers_per_gpu": n, "triangles": 2 * cfg.nr * cfg.ntheta, "planes": cfg.n_planes, "dt": cfg.dt, "push_variant": args.variant,
+    return {"workload": f"{cfg.name}: {2 * cfg.nr * cfg.ntheta} triangles x {cfg.n_planes} planes, {n} markers/GPU, EM={cfg.em}, dt={cfg.dt}, RK4, sort every {args.sort_every} steps",
+            "markers_per_gpu": n, "triangles": 2 * cfg.nr * cfg.ntheta, "planes": cfg.n_planes, "dt": cfg.dt, "push_variant": args.variant, "sort_every": args.sort_every,
             "l2": "inputs_exceed_l2" if n * 104 > 126e6 else "l2_flushed_between_steps"}
 
 
@@ -152,6 +152,7 @@ def main():
     ap.add_argument("--markers", type=int, default=None, help="markers per GPU (default: the config's)")
     ap.add_argument("--dt", type=float, default=None)
     ap.add_argument("--variant", type=int, default=0, help="0 tiled push kernel, 1 simple")
+    ap.add_argument("--sort-every", type=int, default=SORT_EVERY, help="re-sort the marker store every n RK4 steps (inside the timed region)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample", type=int, default=400_000, help="markers of the oracle cpu_baseline leg (x 4 steps)")
     ap.add_argument("--ref-markers", type=int, default=200_000, help="markers per step of --impl reference")
@@ -184,7 +185,7 @@ def main():
     dev = {k: v.cuda(non_blocking=True) for k, v in host.items()}
     torch.cuda.synchronize()
     g.set_push_variant(args.variant)
-    g.set_sort_interval(SORT_EVERY)
+    g.set_sort_interval(args.sort_every)
     g.markers_bind(*[dev[k] for k in KEYS])
     dfma = g.bench_dfma()
 

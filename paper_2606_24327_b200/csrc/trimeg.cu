@@ -14,6 +14,7 @@
 
 #include "trimeg_host_setup.hpp"
 #include "trimeg_math.cuh"
+#include "trimeg_tile.cuh"
 
 using namespace trimeg;
 
@@ -24,11 +25,23 @@ struct MarkerSoA {           // one of two buffers living in the caller's scratc
 };
 struct DevTables {
     const TriGeom* geom;     // [T]
-    const double* coef;      // [T][P+3][21][2]; padded plane pp holds toroidal plane (pp-1) mod P
+    const double* coef;      // [T][P+3+2*PLANE_PAD][21][2]; see PLANE_PAD in trimeg_math.cuh
     BoxGrid bg;
     TorP tor;
     int T;
-    long long tri_stride;    // doubles per triangle = (P+3)*42
+    long long tri_stride;    // doubles per triangle = (P+3+2*PLANE_PAD)*42
+};
+
+// tiled push configuration: patches of 16 triangles + halo (56 slots), windows of 4 toroidal intervals (+1 each side),
+// 4 groups of 128 threads per CTA, one CTA per SM
+using Tile = TileCfg<16, 56, 4, 128, 4>;
+// cell numbering used by the sort: super-cell (patch, window) major, then triangle within the patch, then interval
+struct CellMap {
+    int P, nwin;
+    __host__ __device__ __forceinline__ int cell(int t, int k) const {
+        int patch = t / Tile::TP, tl = t - patch * Tile::TP, wdw = k / Tile::WK, kl = k - wdw * Tile::WK;
+        return ((patch * nwin + wdw) * Tile::TP + tl) * Tile::WK + kl;
+    }
 };
 
 __constant__ double c_Aplus[21 * 18];
@@ -79,12 +92,12 @@ __global__ void k_fields_set(int T, int P, int which, const int* __restrict__ tr
         for (int m = 0; m < 6; ++m) s = fma(K[r * 6 + m], c[qi[m]], s);
         z[r] = s;
     }
-    long long tri_stride = (long long)(P + 3) * PLANE_STRIDE;
+    const int NPP = P + 3 + 2 * PLANE_PAD;
+    long long tri_stride = (long long)NPP * PLANE_STRIDE;
     double* base = coef + (long long)t * tri_stride;
-    int slots[3] = {k + 1, -1, -1};
-    if (k == P - 1) slots[1] = 0;
-    if (k == 0) slots[1] = P + 1;
-    if (k == 1) slots[2] = P + 2;
+    int slots[3];
+#pragma unroll
+    for (int s = 0; s < 3; ++s) { int pp = k + 1 + PLANE_PAD + (s - 1) * P; slots[s] = (pp >= 0 && pp < NPP) ? pp : -1; }
 #pragma unroll
     for (int i = 0; i < 21; ++i) {
         double v = c[i] - (c_Nul[i * 3] * z[0] + c_Nul[i * 3 + 1] * z[1] + c_Nul[i * 3 + 2] * z[2]);
@@ -109,7 +122,7 @@ __device__ __forceinline__ void gather_at(const DevTables& tb, int t, double R, 
     ref_coords(g, R, Z, xi, eta);
     double w[4], dw[4];
     int kk = bspline_weights(tb.tor, phi, w, dw);
-    LdGlobal ld{reinterpret_cast<const double2*>(tb.coef + (long long)t * tb.tri_stride + (long long)kk * PLANE_STRIDE)};
+    LdGlobal ld{reinterpret_cast<const double2*>(tb.coef + (long long)t * tb.tri_stride + (long long)(kk + PLANE_PAD) * PLANE_STRIDE)};
     double acc[8];
     gather_cell(ld, xi, eta, w, dw, acc);
     to_fields(g, acc, f);
@@ -167,6 +180,37 @@ __global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, Sp
     s.status[m] = st;
 }
 
+
+// markers outside the mesh (sorted behind the last cell): same arithmetic through the simple path
+__global__ void __launch_bounds__(128) k_push_lost(DevTables tb, EquilP ep, SpeciesP sp, MarkerSoA s, const int* __restrict__ first, long long n, double dt) {
+    long long m0 = *first;
+    for (long long m = m0 + (long long)blockIdx.x * blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
+        double y0[5] = {s.R[m], s.Z[m], s.phi[m], s.u[m], s.w[m]};
+        double mu = s.mu[m], p = s.p[m];
+        int t = s.tri[m], st = s.status[m];
+        double k[5], acc[5], y[5];
+        st |= stage_simple(tb, ep, sp, t, y0[0], y0[1], y0[2], y0[3], y0[4], mu, p, k);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { acc[q] = k[q]; y[q] = fma(0.5 * dt, k[q], y0[q]); }
+        st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { acc[q] = fma(2.0, k[q], acc[q]); y[q] = fma(0.5 * dt, k[q], y0[q]); }
+        st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { acc[q] = fma(2.0, k[q], acc[q]); y[q] = fma(dt, k[q], y0[q]); }
+        st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k);
+        const double h6 = dt / 6.0;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) y[q] = fma(h6, acc[q] + k[q], y0[q]);
+        double ph = fma(-tb.tor.period, floor(y[2] * tb.tor.inv_period), y[2]);
+        if (ph < 0.0) ph += tb.tor.period;
+        if (ph >= tb.tor.period) ph -= tb.tor.period;
+        s.R[m] = y[0]; s.Z[m] = y[1]; s.phi[m] = ph; s.u[m] = y[3]; s.w[m] = y[4];
+        s.tri[m] = t;
+        s.status[m] = st;
+    }
+}
+
 __global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP sp, MarkerSoA s, long long n, double* __restrict__ out) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= n) return;
@@ -176,6 +220,213 @@ __global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP s
     long long o = s.id[m];
 #pragma unroll
     for (int q = 0; q < 5; ++q) out[(long long)q * n + o] = d[q];
+}
+
+
+// ============================================================================================ tiled push (variant 0)
+struct TileGroupSmem {   // pointers into one group's slice of shared memory
+    double *ia, *ib, *ic, *res;
+    int *meta, *lost, *hist, *wsum;
+};
+
+template <class C>
+__global__ void __launch_bounds__(C::NT* C::NG, 1)
+k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, double dt, int* __restrict__ work_counter,
+             unsigned long long* __restrict__ stats) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    double* coef = reinterpret_cast<double*>(smem + C::OFF_COEF);
+    SlotGeom* sgeom = reinterpret_cast<SlotGeom*>(smem + C::OFF_GEOM);
+    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + C::OFF_MISC);
+    int* sh_sc = reinterpret_cast<int*>(smem + C::OFF_MISC + 16);
+    int* sh_slow = reinterpret_cast<int*>(smem + C::OFF_MISC + 20);
+
+    const int tid = threadIdx.x, grp = tid / C::NT, gtid = tid - grp * C::NT, bar_id = 1 + grp;
+    TileGroupSmem gs;
+    {
+        unsigned char* g0 = smem + C::OFF_GRP + C::GRP_BYTES * grp;
+        gs.ia = reinterpret_cast<double*>(g0);
+        gs.ib = gs.ia + C::NT;
+        gs.ic = gs.ib + C::NT;
+        gs.res = gs.ic + C::NT;
+        gs.meta = reinterpret_cast<int*>(gs.res + 8 * C::NT);
+        gs.lost = gs.meta + C::NT;
+        gs.hist = gs.lost + C::NT;
+        gs.wsum = gs.hist + C::HIST;
+    }
+    if (tid == 0) { mbar_init(mbar, 1); *sh_slow = 0; asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+    for (int i = gtid; i < C::HIST; i += C::NT) gs.hist[i] = 0;
+    unsigned phase = 0;
+    const int P = tb.tor.P;
+    const double h2 = 0.5 * dt, h6 = dt / 6.0;
+
+    for (;;) {
+        __syncthreads();   // previous super-cell fully consumed (coefficients, geometry, sh_sc)
+        if (tid == 0) *sh_sc = atomicAdd(work_counter, 1);
+        __syncthreads();
+        const int sc = *sh_sc;
+        if (sc >= tt.nsc) break;
+        const int begin = tt.offs[(long long)sc * C::CPS], end = tt.offs[(long long)(sc + 1) * C::CPS];
+        if (begin == end) continue;
+        const int patch = sc / tt.nwin, k0 = (sc - patch * tt.nwin) * C::WK;
+        const int ns = tt.nslots[patch];
+        const int* pslots = tt.slots + (long long)patch * C::SMAX;
+        // ---- stage geometry (generic stores) and coefficient blocks (TMA bulk copies)
+        if (tid < ns) {
+            int t = pslots[tid];
+            SlotGeom g;
+            if (t >= 0) {
+                const TriGeom tg = tb.geom[t];
+                g.v0x = tg.v0x; g.v0y = tg.v0y; g.a11 = tg.a11; g.a12 = tg.a12; g.a21 = tg.a21; g.a22 = tg.a22;
+                const short* nb = tt.nbr + ((long long)patch * C::SMAX + tid) * 4;
+                g.nbr[0] = nb[0]; g.nbr[1] = nb[1]; g.nbr[2] = nb[2]; g.nbr[3] = -1;
+            } else {
+                g.v0x = g.v0y = 1e300; g.a11 = g.a12 = g.a21 = g.a22 = 0.0; g.nbr[0] = g.nbr[1] = g.nbr[2] = g.nbr[3] = -1;
+            }
+            g.tri = t; g.pad = 0;
+            sgeom[tid] = g;
+        }
+        if (tid < 32) {
+            int cnt = 0;
+            for (int sl = tid; sl < ns; sl += 32) cnt += pslots[sl] >= 0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the block vs. the async writes
+            if (tid == 0) mbar_expect_tx(mbar, (unsigned)(cnt * C::SLOT_DOUBLES * sizeof(double)));
+            __syncwarp();
+            for (int sl = tid; sl < ns; sl += 32) {
+                int t = pslots[sl];
+                if (t >= 0)
+                    tma_bulk_g2s(coef + (size_t)sl * C::SLOT_DOUBLES, tb.coef + (long long)t * tb.tri_stride + (long long)k0 * PLANE_STRIDE,
+                                 (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
+            }
+        }
+        mbar_wait(mbar, phase);
+        phase ^= 1;
+        __syncthreads();
+
+        // ---- chunks of NT markers, one group each
+        for (int chunk = begin + grp * C::NT; chunk < end; chunk += C::NT * C::NG) {
+            const int m = chunk + gtid;
+            const bool active = m < end;
+            const int n_items = min(C::NT, end - chunk);
+            double y0[5], y[5], acc[5], mu = 0.0, pw = 0.0;
+            int st = 0, home = -1, cur = -1, tri_last = -1;
+            if (active) {
+                y0[0] = s.R[m]; y0[1] = s.Z[m]; y0[2] = s.phi[m]; y0[3] = s.u[m]; y0[4] = s.w[m];
+                mu = s.mu[m]; pw = s.p[m]; st = s.status[m];
+                tri_last = s.tri[m];
+                int sl = tri_last - patch * C::TP;
+                if (sl >= 0 && sl < C::TP) home = sl;
+                else {   // drifted since the last sort: look for the triangle in the halo
+                    for (int q = C::TP; q < ns; ++q) if (sgeom[q].tri == tri_last) { home = q; break; }
+                }
+                cur = home;
+            } else {
+#pragma unroll
+                for (int q = 0; q < 5; ++q) y0[q] = 0.0;
+            }
+#pragma unroll
+            for (int q = 0; q < 5; ++q) { y[q] = y0[q]; acc[q] = 0.0; }
+
+#pragma unroll 1
+            for (int stage = 0; stage < 4; ++stage) {
+                // -- owner: locate in slot space, toroidal cell, counting-sort rank
+                int bin = C::NBINS - 1, rank = 0;
+                double ia = y[0], ib = y[1], ic = y[2];
+                if (active) {
+                    int sl = cur >= 0 ? cur : home;
+                    double xi = 0.0, eta = 0.0;
+                    if (sl >= 0) {
+                        int hop = 0;
+                        for (; hop < 16; ++hop) {
+                            const SlotGeom& g = sgeom[sl];
+                            double dx = y[0] - g.v0x, dy = y[1] - g.v0y;
+                            xi = fma(g.a11, dx, g.a12 * dy);
+                            eta = fma(g.a21, dx, g.a22 * dy);
+                            double l0 = 1.0 - xi - eta;
+                            if (fmin(fmin(xi, eta), l0) >= INSIDE_TOL) break;
+                            int e = (eta <= xi && eta <= l0) ? 0 : ((l0 <= xi) ? 1 : 2);
+                            sl = g.nbr[e];
+                            if (sl < 0) break;
+                        }
+                        if (hop == 16) sl = -1;
+                    }
+                    double sf;
+                    int k = toroidal_interval(tb.tor, y[2], sf);
+                    int dk = k - k0;
+                    if (dk > P / 2) dk -= P; else if (dk < -(P / 2)) dk += P;
+                    int lk = dk + C::HK;
+                    cur = sl;
+                    if (sl >= 0 && lk >= 0 && lk < C::NW) {
+                        bin = sl * C::NW + lk;
+                        ia = xi; ib = eta; ic = sf;
+                        tri_last = sgeom[sl].tri;
+                    }
+                    rank = atomicAdd(gs.hist + bin, 1);
+                }
+                group_sync(bar_id, C::NT);
+                group_scan<C::NT, C::HIST>(gs.hist, gs.wsum, gtid, bar_id);
+                if (active) {
+                    int pos = gs.hist[bin] + rank;
+                    gs.ia[pos] = ia; gs.ib[pos] = ib; gs.ic[pos] = ic;
+                    gs.meta[pos] = gtid | (bin << 12);
+                }
+                group_sync(bar_id, C::NT);
+                for (int i = gtid; i < C::HIST; i += C::NT) gs.hist[i] = 0;   // next stage's histogram
+                // -- gather thread: item gtid in cell order
+                if (gtid < n_items) {
+                    const int meta = gs.meta[gtid], owner = meta & 0xfff, b = meta >> 12;
+                    const double a_ = gs.ia[gtid], b_ = gs.ib[gtid], c_ = gs.ic[gtid];
+                    Fields f;
+                    int lost = 0;
+                    if (b != C::NBINS - 1) {
+                        const int sl = b / C::NW, lk = b - sl * C::NW;
+                        double w[4], dw[4], g8[8];
+                        bspline_from_s(tb.tor, c_, w, dw);
+                        LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
+                        gather_cell(ld, a_, b_, w, dw, g8);
+                        const SlotGeom& g = sgeom[sl];
+                        f.P = g8[0]; f.PR = fma(g.a11, g8[1], g.a21 * g8[2]); f.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); f.Pp = g8[3];
+                        f.A = g8[4]; f.AR = fma(g.a11, g8[5], g.a21 * g8[6]); f.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); f.Ap = g8[7];
+                    } else {   // slow path: global tables
+                        int t = locate_box(tb.bg, tb.geom, a_, b_);
+                        gather_at(tb, t, a_, b_, c_, f);
+                        lost = t < 0;
+                        atomicAdd(sh_slow, 1);
+                    }
+                    double* r = gs.res + owner;
+                    r[0] = f.P; r[C::NT] = f.PR; r[2 * C::NT] = f.PZ; r[3 * C::NT] = f.Pp;
+                    r[4 * C::NT] = f.A; r[5 * C::NT] = f.AR; r[6 * C::NT] = f.AZ; r[7 * C::NT] = f.Ap;
+                    gs.lost[owner] = lost;
+                }
+                group_sync(bar_id, C::NT);
+                // -- owner: equilibrium, equations of motion, RK4 bookkeeping
+                if (active) {
+                    const double* r = gs.res + gtid;
+                    Fields f{r[0], r[C::NT], r[2 * C::NT], r[3 * C::NT], r[4 * C::NT], r[5 * C::NT], r[6 * C::NT], r[7 * C::NT]};
+                    st |= gs.lost[gtid];
+                    double d[5];
+                    rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, f, d);
+                    const double wgt = (stage == 0 || stage == 3) ? 1.0 : 2.0;
+                    const double hs = stage == 2 ? dt : h2;
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) { acc[q] = fma(wgt, d[q], acc[q]); y[q] = fma(hs, d[q], y0[q]); }
+                }
+            }
+            if (active) {
+#pragma unroll
+                for (int q = 0; q < 5; ++q) y[q] = fma(h6, acc[q], y0[q]);
+                double ph = fma(-tb.tor.period, floor(y[2] * tb.tor.inv_period), y[2]);
+                if (ph < 0.0) ph += tb.tor.period;
+                if (ph >= tb.tor.period) ph -= tb.tor.period;
+                s.R[m] = y[0]; s.Z[m] = y[1]; s.phi[m] = ph; s.u[m] = y[3]; s.w[m] = y[4];
+                s.tri[m] = tri_last;
+                s.status[m] = st;
+            }
+        }
+    }
+    __syncthreads();
+    if (tid == 0 && *sh_slow) atomicAdd(stats + 1, (unsigned long long)*sh_slow);
 }
 
 // ============================================================================================ marker store / sort
@@ -198,13 +449,13 @@ __global__ void k_unsort(MarkerSoA s, long long n, double* R, double* Z, double*
     if (status) status[o] = s.status[m];
 }
 // cell key = tri * P + toroidal interval; markers outside the mesh go to the last cell (T*P)
-__global__ void __launch_bounds__(256) k_sort_keys(DevTables tb, MarkerSoA s, long long n, int* __restrict__ keys, int* __restrict__ hist) {
+__global__ void __launch_bounds__(256) k_sort_keys(DevTables tb, CellMap cm, int ncell, MarkerSoA s, long long n, int* __restrict__ keys, int* __restrict__ hist) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= n) return;
     int t = locate_walk(tb.bg, tb.geom, s.tri[m], s.R[m], s.Z[m]);
-    double w[4], dw[4];
-    int k = bspline_weights(tb.tor, s.phi[m], w, dw);
-    int key = t < 0 ? tb.T * tb.tor.P : t * tb.tor.P + k;
+    double sf;
+    int k = toroidal_interval(tb.tor, s.phi[m], sf);
+    int key = t < 0 ? ncell : cm.cell(t, k);
     s.tri[m] = t;
     keys[m] = key;
     atomicAdd(hist + key, 1);
@@ -314,6 +565,13 @@ struct trimeg_ctx {
     long long steps_since_sort = 0;
     int variant = 0;
     long long stats[4] = {0, 0, 0, 0};
+    // tiled kernel tables
+    int *d_pslots = nullptr, *d_pnslots = nullptr, *d_work = nullptr;
+    short* d_pnbr = nullptr;
+    unsigned long long* d_stats = nullptr;
+    TileTables tt{};
+    CellMap cm{};
+    bool tiled_ok = false;
 };
 
 static int fail(trimeg_ctx* c, int code, const char* fmt, ...) {
@@ -344,6 +602,8 @@ static void free_mesh(trimeg_ctx* c) {
     cudaFree(c->d_geom); cudaFree(c->d_tri); cudaFree(c->d_head); cudaFree(c->d_list); cudaFree(c->d_new_of_orig);
     cudaFree(c->d_RZ); cudaFree(c->d_K); cudaFree(c->d_coef);
     cudaFree(c->d_hist); cudaFree(c->d_offs); cudaFree(c->d_fill); cudaFree(c->d_sums);
+    cudaFree(c->d_pslots); cudaFree(c->d_pnslots); cudaFree(c->d_pnbr); cudaFree(c->d_work); cudaFree(c->d_stats);
+    c->d_pslots = c->d_pnslots = c->d_work = nullptr; c->d_pnbr = nullptr; c->d_stats = nullptr;
     c->d_geom = nullptr; c->d_tri = c->d_head = c->d_list = c->d_new_of_orig = nullptr;
     c->d_RZ = c->d_K = c->d_coef = nullptr;
     c->d_hist = c->d_offs = c->d_fill = c->d_sums = nullptr;
@@ -447,9 +707,15 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
         if (!trimeg_host::triangle_K(ec, v, &K[(size_t)t * 18])) return fail(ctx, TRIMEG_ERR_BAD_MESH, "mesh_load: degenerate triangle %d", g.orig);
     }
     ctx->T = T; ctx->P = n_planes; ctx->n_nodes = n_nodes; ctx->period = phi_period;
-    const long long tri_stride = (long long)(n_planes + 3) * PLANE_STRIDE;
+    const long long tri_stride = (long long)(n_planes + 3 + 2 * PLANE_PAD) * PLANE_STRIDE;
     const size_t coef_bytes = (size_t)T * tri_stride * sizeof(double);
-    ctx->ncell = (long long)T * n_planes;
+    trimeg_host::HostPatches hp;
+    trimeg_host::build_patches(hm, RZ, n_nodes, T, Tile::TP, Tile::SMAX, hp);
+    const int nwin = (n_planes + Tile::WK - 1) / Tile::WK;
+    ctx->cm.P = n_planes; ctx->cm.nwin = nwin;
+    ctx->ncell = (long long)hp.npatch * nwin * Tile::CPS;
+    if ((double)hp.npatch * nwin * Tile::CPS + 2 > 2.0e9) return fail(ctx, TRIMEG_ERR_BAD_ARG, "mesh_load: too many cells for int32 ids");
+    ctx->tiled_ok = (n_planes % Tile::WK == 0) && (n_planes >= Tile::NW);
     CU(cudaMalloc(&ctx->d_geom, sizeof(TriGeom) * T));
     CU(cudaMalloc(&ctx->d_tri, sizeof(int) * 3 * T));
     CU(cudaMalloc(&ctx->d_head, sizeof(int) * hm.head.size()));
@@ -463,6 +729,19 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     CU(cudaMalloc(&ctx->d_offs, sizeof(int) * ncnt));
     CU(cudaMalloc(&ctx->d_fill, sizeof(int) * ncnt));
     CU(cudaMalloc(&ctx->d_sums, sizeof(int) * (ncnt / SCAN_CHUNK + 2)));
+    CU(cudaMalloc(&ctx->d_pslots, sizeof(int) * hp.slots.size()));
+    CU(cudaMalloc(&ctx->d_pnslots, sizeof(int) * hp.nslots.size()));
+    CU(cudaMalloc(&ctx->d_pnbr, sizeof(short) * hp.nbr.size()));
+    CU(cudaMalloc(&ctx->d_work, sizeof(int) * 4));
+    CU(cudaMalloc(&ctx->d_stats, sizeof(unsigned long long) * 4));
+    CU(cudaMemcpyAsync(ctx->d_pslots, hp.slots.data(), sizeof(int) * hp.slots.size(), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->d_pnslots, hp.nslots.data(), sizeof(int) * hp.nslots.size(), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->d_pnbr, hp.nbr.data(), sizeof(short) * hp.nbr.size(), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_stats, 0, sizeof(unsigned long long) * 4, ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_offs, 0, sizeof(int) * ncnt, ctx->stream));
+    ctx->tt.slots = ctx->d_pslots; ctx->tt.nbr = ctx->d_pnbr; ctx->tt.nslots = ctx->d_pnslots; ctx->tt.offs = ctx->d_offs;
+    ctx->tt.npatch = hp.npatch; ctx->tt.nwin = nwin; ctx->tt.nsc = hp.npatch * nwin;
+    CU(cudaFuncSetAttribute(k_push_tiled<Tile>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tile::BYTES));
     CU(cudaMemcpyAsync(ctx->d_geom, geom.data(), sizeof(TriGeom) * T, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_tri, hm.tri.data(), sizeof(int) * 3 * T, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_head, hm.head.data(), sizeof(int) * hm.head.size(), cudaMemcpyHostToDevice, ctx->stream));
@@ -548,12 +827,12 @@ static void carve(MarkerSoA& s, char*& p, long long n) {
 
 static int do_sort(trimeg_ctx* ctx) {
     const long long n = ctx->n;
-    const long long ncnt = ctx->ncell + 1;
+    const long long ncnt = ctx->ncell + 2;   // cells + lost bin + end sentinel
     MarkerSoA& a = ctx->buf[ctx->cur];
     MarkerSoA& b = ctx->buf[ctx->cur ^ 1];
     CU(cudaMemsetAsync(ctx->d_hist, 0, sizeof(int) * ncnt, ctx->stream));
     CU(cudaMemsetAsync(ctx->d_fill, 0, sizeof(int) * ncnt, ctx->stream));
-    k_sort_keys<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, a, n, ctx->d_keys, ctx->d_hist);
+    k_sort_keys<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, ctx->cm, (int)ctx->ncell, a, n, ctx->d_keys, ctx->d_hist);
     KCHECK();
     int nb = (int)((ncnt + SCAN_CHUNK - 1) / SCAN_CHUNK);
     k_scan_reduce<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_hist, ncnt, ctx->d_sums);
@@ -650,15 +929,28 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps) {
         return fail(ctx, TRIMEG_ERR_BAD_STATE, "push_rk4: mesh, equilibrium, species and markers must be set first");
     CU(cudaSetDevice(ctx->device));
     ctx->stats[0] = ctx->stats[1] = ctx->stats[2] = ctx->stats[3] = 0;
+    CU(cudaMemsetAsync(ctx->d_stats, 0, sizeof(unsigned long long) * 4, ctx->stream));
     const long long n = ctx->n;
     for (int s = 0; s < nsteps; ++s) {
         if (!ctx->sorted || (ctx->sort_every > 0 && ctx->steps_since_sort >= ctx->sort_every)) {
             int rc = do_sort(ctx);
             if (rc) return rc;
         }
-        k_push_simple<<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->buf[ctx->cur], n, dt);
-        KCHECK();
-        ctx->stats[0] += 1;
+        if (ctx->variant == 0 && ctx->tiled_ok) {
+            CU(cudaMemsetAsync(ctx->d_work, 0, sizeof(int), ctx->stream));
+            k_push_tiled<Tile><<<ctx->num_sms, Tile::NT * Tile::NG, Tile::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, ctx->buf[ctx->cur], dt,
+                                                                                           ctx->d_work, ctx->d_stats);
+            KCHECK();
+            // markers outside the mesh sit behind the last cell: push them with the simple kernel
+            // (their count is only known on the device; the launch is sized for the worst case of 0..n and exits early)
+            k_push_lost<<<148 * 4, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->buf[ctx->cur], ctx->d_offs + ctx->ncell, n, dt);
+            KCHECK();
+            ctx->stats[0] += 2;
+        } else {
+            k_push_simple<<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->buf[ctx->cur], n, dt);
+            KCHECK();
+            ctx->stats[0] += 1;
+        }
         ctx->steps_since_sort += 1;
     }
     return TRIMEG_OK;
@@ -713,6 +1005,13 @@ int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops) {
 int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]) {
     if (!ctx || !out) return TRIMEG_ERR_BAD_ARG;
     for (int i = 0; i < 4; ++i) out[i] = ctx->stats[i];
+    if (ctx->d_stats) {   // slow-path evaluations are counted on the device
+        unsigned long long h[4] = {0, 0, 0, 0};
+        CU(cudaSetDevice(ctx->device));
+        CU(cudaMemcpyAsync(h, ctx->d_stats, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        out[1] = (int64_t)h[1];
+    }
     return TRIMEG_OK;
 }
 

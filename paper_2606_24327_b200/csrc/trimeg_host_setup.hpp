@@ -194,3 +194,80 @@ inline int build_mesh(int64_t n_nodes, const double* RZ, int64_t T, const int32_
 }
 
 }  // namespace trimeg_host
+
+// ---------------------------------------------------------------------------------------------------------
+// Static patches for the tiled push kernel: a patch is a run of TP consecutive triangles in the spatial
+// (Morton) numbering; its slot list = own triangles (slots 0..TP-1) followed by a halo of nearby triangles
+// (first the ring of triangles sharing a vertex with the patch, edge-neighbours first, then further rings,
+// nearest to the patch centroid first) up to SMAX slots.  nbr gives, per slot and edge, the slot across that
+// edge or -1 when that triangle is not staged (or the edge is on the mesh boundary).
+namespace trimeg_host {
+struct HostPatches {
+    int TP = 0, SMAX = 0, npatch = 0;
+    std::vector<int32_t> slots;    // [npatch][SMAX], -1 = unused
+    std::vector<int16_t> nbr;      // [npatch][SMAX][4] (4th = pad)
+    std::vector<int32_t> nslots;   // [npatch]
+};
+inline void build_patches(const HostMesh& hm, const double* RZ, int64_t n_nodes, int64_t T, int TP, int SMAX, HostPatches& hp) {
+    hp.TP = TP; hp.SMAX = SMAX; hp.npatch = (int)((T + TP - 1) / TP);
+    hp.slots.assign((size_t)hp.npatch * SMAX, -1);
+    hp.nbr.assign((size_t)hp.npatch * SMAX * 4, -1);
+    hp.nslots.assign(hp.npatch, 0);
+    // node -> triangles CSR
+    std::vector<int32_t> nhead(n_nodes + 1, 0), nlist(3 * T);
+    for (int64_t t = 0; t < T; t++) for (int v = 0; v < 3; v++) nhead[hm.tri[3 * t + v] + 1]++;
+    for (int64_t n = 0; n < n_nodes; n++) nhead[n + 1] += nhead[n];
+    { std::vector<int32_t> f(nhead.begin(), nhead.end() - 1); for (int64_t t = 0; t < T; t++) for (int v = 0; v < 3; v++) nlist[f[hm.tri[3 * t + v]]++] = (int32_t)t; }
+    std::vector<double> cx(T), cy(T);
+    for (int64_t t = 0; t < T; t++) { cx[t] = (RZ[2 * hm.tri[3 * t]] + RZ[2 * hm.tri[3 * t + 1]] + RZ[2 * hm.tri[3 * t + 2]]) / 3; cy[t] = (RZ[2 * hm.tri[3 * t] + 1] + RZ[2 * hm.tri[3 * t + 1] + 1] + RZ[2 * hm.tri[3 * t + 2] + 1]) / 3; }
+    std::vector<int32_t> slot_of(T, -1), mark(T, -1);
+    std::vector<int32_t> cur, frontier, next;
+    struct Cand { double key; int32_t t; };
+    std::vector<Cand> cand;
+    for (int p = 0; p < hp.npatch; p++) {
+        int64_t t0 = (int64_t)p * TP, t1 = std::min<int64_t>(T, t0 + TP);
+        int32_t* sl = &hp.slots[(size_t)p * SMAX];
+        int ns = 0;
+        double pcx = 0, pcy = 0;
+        for (int64_t t = t0; t < t1; t++) { sl[ns] = (int32_t)t; slot_of[t] = ns; mark[t] = p; ns++; pcx += cx[t]; pcy += cy[t]; }
+        pcx /= (t1 - t0); pcy /= (t1 - t0);
+        int own = ns;
+        // pad unused own slots (last patch) so that own triangles always sit at slot = t - t0
+        for (; ns < TP && ns < SMAX; ns++) sl[ns] = -1;
+        frontier.assign(sl, sl + own);
+        for (int ring = 0; ring < 4 && ns < SMAX && !frontier.empty(); ring++) {
+            cand.clear();
+            for (int32_t t : frontier) for (int v = 0; v < 3; v++) {
+                int32_t node = hm.tri[3 * t + v];
+                for (int32_t q = nhead[node]; q < nhead[node + 1]; q++) {
+                    int32_t o = nlist[q];
+                    if (mark[o] == p) continue;
+                    mark[o] = p;
+                    bool edge_nb = false;
+                    for (int e = 0; e < 3; e++) { int32_t nb = hm.nbr[3 * o + e]; if (nb >= 0 && slot_of[nb] >= 0 && slot_of[nb] < own && nb >= t0 && nb < t1) edge_nb = true; }
+                    double d2 = (cx[o] - pcx) * (cx[o] - pcx) + (cy[o] - pcy) * (cy[o] - pcy);
+                    cand.push_back({(ring == 0 && edge_nb ? 0.0 : 1.0) + 1e-3 * d2 / (1e-300 + d2 + 1.0) + ring, o});
+                    cand.back().key = ring * 10.0 + (edge_nb && ring == 0 ? 0.0 : 1.0) + d2 / (d2 + 1.0);
+                }
+            }
+            std::sort(cand.begin(), cand.end(), [](const Cand& a, const Cand& b) { return a.key < b.key; });
+            next.clear();
+            for (const Cand& c : cand) {
+                if (ns >= SMAX) break;
+                sl[ns] = c.t; slot_of[c.t] = ns; ns++; next.push_back(c.t);
+            }
+            frontier.swap(next);
+        }
+        hp.nslots[p] = ns;
+        for (int s = 0; s < ns; s++) {
+            int32_t t = sl[s];
+            if (t < 0) continue;
+            for (int e = 0; e < 3; e++) {
+                int32_t nb = hm.nbr[3 * t + e];
+                hp.nbr[((size_t)p * SMAX + s) * 4 + e] = (nb >= 0 && slot_of[nb] >= 0) ? (int16_t)slot_of[nb] : (int16_t)-1;
+            }
+        }
+        for (int s = 0; s < ns; s++) if (sl[s] >= 0) slot_of[sl[s]] = -1;
+    }
+}
+}  // namespace trimeg_host

@@ -11,6 +11,9 @@ namespace trimeg {
 
 constexpr int NCOEF = 21;                 // quintic monomials xi^i eta^j, i + j <= 5
 constexpr int PLANE_STRIDE = NCOEF * 2;   // doubles per (triangle, plane): [21][field]
+constexpr int PLANE_PAD = 1;              // extra toroidal planes on each side of the padded coefficient table
+// padded table: plane index pp in [0, P + 3 + 2 PLANE_PAD) holds toroidal plane (pp - 1 - PLANE_PAD) mod P, so the four planes
+// k-1..k+2 of interval k are pp = k + PLANE_PAD .. k + PLANE_PAD + 3, contiguous for every k (no wrap in the kernels)
 constexpr double INSIDE_TOL = -1e-12;
 
 struct EquilP {
@@ -48,15 +51,19 @@ __device__ __forceinline__ double rcp_nr(double x) {   // 1/x: hardware seed + N
 }
 
 // ---- toroidal uniform periodic cubic B-spline (L35) -------------------------------------------------
-// returns padded plane base kk (planes kk..kk+3 of the padded table hold toroidal planes k-1..k+2)
-__device__ __forceinline__ int bspline_weights(const TorP& tp, double phi, double w[4], double dw[4]) {
+// interval index k in [0, P) and fraction s in [0, 1] of phi (any real)
+__device__ __forceinline__ int toroidal_interval(const TorP& tp, double phi, double& s) {
     double pm = fma(-tp.period, floor(phi * tp.inv_period), phi);
     if (pm < 0.0) pm += tp.period;
     if (pm >= tp.period) pm -= tp.period;
     double u = pm * tp.inv_dphi;
     int k = (int)u;
     if (k >= tp.P) k = tp.P - 1;
-    double s = u - (double)k, t = 1.0 - s;
+    s = u - (double)k;
+    return k;
+}
+__device__ __forceinline__ void bspline_from_s(const TorP& tp, double s, double w[4], double dw[4]) {
+    double t = 1.0 - s;
     const double sixth = 1.0 / 6.0;
     double s2 = s * s, t2 = t * t;
     w[0] = t2 * t * sixth;
@@ -67,6 +74,12 @@ __device__ __forceinline__ int bspline_weights(const TorP& tp, double phi, doubl
     dw[3] = s2 * tp.half_inv_dphi;
     dw[1] = s * fma(3.0, s, -4.0) * tp.half_inv_dphi;
     dw[2] = -t * fma(3.0, t, -4.0) * tp.half_inv_dphi;
+}
+// returns the interval k; the four planes are padded-table planes k + PLANE_PAD .. k + PLANE_PAD + 3
+__device__ __forceinline__ int bspline_weights(const TorP& tp, double phi, double w[4], double dw[4]) {
+    double s;
+    int k = toroidal_interval(tp, phi, s);
+    bspline_from_s(tp, s, w, dw);
     return k;
 }
 
@@ -91,26 +104,24 @@ __device__ __forceinline__ void horner2(Ld ld, int off, double x, double& v0, do
     }
 }
 
-// acc[0..3] += (w p, w p_xi, w p_eta, dw p) for field 0, acc[4..7] likewise for field 1
+// acc[0..3] += (w p, w p_xi, w p_eta, dw p) for field 0, acc[4..7] likewise for field 1.
+// Outer Horner in eta runs j = 5 -> 0 and consumes each a_j(xi), a_j'(xi) as soon as the inner Horner produced it,
+// so only the three running sums per field stay live.
 template <typename Ld>
 __device__ __forceinline__ void quintic_pair_accum(Ld ld, double xi, double eta, double w, double dw, double acc[8]) {
-    double a0[6], a1[6], b0[5], b1[5];
-    double dz0, dz1;
-    horner2<5>(ld, 0, xi, a0[0], b0[0], a1[0], b1[0]);
-    horner2<4>(ld, 6, xi, a0[1], b0[1], a1[1], b1[1]);
-    horner2<3>(ld, 11, xi, a0[2], b0[2], a1[2], b1[2]);
-    horner2<2>(ld, 15, xi, a0[3], b0[3], a1[3], b1[3]);
-    horner2<1>(ld, 18, xi, a0[4], b0[4], a1[4], b1[4]);
-    horner2<0>(ld, 20, xi, a0[5], dz0, a1[5], dz1);
-    double p0 = fma(a0[5], eta, a0[4]), p1 = fma(a1[5], eta, a1[4]);
-    double py0 = a0[5], py1 = a1[5];
-    double px0 = b0[4], px1 = b1[4];
-#pragma unroll
-    for (int j = 3; j >= 0; --j) {
-        py0 = fma(py0, eta, p0); py1 = fma(py1, eta, p1);
-        p0 = fma(p0, eta, a0[j]); p1 = fma(p1, eta, a1[j]);
-        px0 = fma(px0, eta, b0[j]); px1 = fma(px1, eta, b1[j]);
-    }
+    double p0, p1, py0, py1, px0, px1, a0, a1, b0, b1;
+    horner2<0>(ld, 20, xi, p0, b0, p1, b1);          // a_5 (constant)
+    horner2<1>(ld, 18, xi, a0, px0, a1, px1);        // a_4, a_4'
+    py0 = p0; py1 = p1;
+    p0 = fma(p0, eta, a0); p1 = fma(p1, eta, a1);
+    horner2<2>(ld, 15, xi, a0, b0, a1, b1);
+    py0 = fma(py0, eta, p0); py1 = fma(py1, eta, p1); p0 = fma(p0, eta, a0); p1 = fma(p1, eta, a1); px0 = fma(px0, eta, b0); px1 = fma(px1, eta, b1);
+    horner2<3>(ld, 11, xi, a0, b0, a1, b1);
+    py0 = fma(py0, eta, p0); py1 = fma(py1, eta, p1); p0 = fma(p0, eta, a0); p1 = fma(p1, eta, a1); px0 = fma(px0, eta, b0); px1 = fma(px1, eta, b1);
+    horner2<4>(ld, 6, xi, a0, b0, a1, b1);
+    py0 = fma(py0, eta, p0); py1 = fma(py1, eta, p1); p0 = fma(p0, eta, a0); p1 = fma(p1, eta, a1); px0 = fma(px0, eta, b0); px1 = fma(px1, eta, b1);
+    horner2<5>(ld, 0, xi, a0, b0, a1, b1);
+    py0 = fma(py0, eta, p0); py1 = fma(py1, eta, p1); p0 = fma(p0, eta, a0); p1 = fma(p1, eta, a1); px0 = fma(px0, eta, b0); px1 = fma(px1, eta, b1);
     acc[0] = fma(w, p0, acc[0]); acc[1] = fma(w, px0, acc[1]); acc[2] = fma(w, py0, acc[2]); acc[3] = fma(dw, p0, acc[3]);
     acc[4] = fma(w, p1, acc[4]); acc[5] = fma(w, px1, acc[5]); acc[6] = fma(w, py1, acc[6]); acc[7] = fma(dw, p1, acc[7]);
 }

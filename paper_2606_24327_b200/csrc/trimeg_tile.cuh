@@ -1,0 +1,104 @@
+// Tiled RK4 push: cell-coherent gather through shared memory.
+//
+// Why: one field evaluation reads 8 x 21 coefficients = 1344 B per marker.  Through L1 with one address per lane
+// that costs >= 1344*32/128 = 336 L1 cycles per warp (measured: 16-32 B/clk/SM delivered when lanes diverge), against
+// 338 DFMA = 169 issue cycles per SM of FP64 work.  Shared memory delivers 256 B/clk/SM when consecutive lanes read
+// the same address (measured), i.e. 168 cycles per warp -- if the lanes of a warp sit in the same few cells.  RK
+// stages 2-4 are evaluated at displaced positions (at dt = 0.05 most markers leave their home triangle), so lanes
+// are re-grouped by cell before every gather:
+//   owner thread (holds the marker's RK state in registers)   gather thread (rank i in cell order)
+//     locate by edge walk in the staged patch, B-spline cell
+//     counting sort by (slot, plane) in shared memory  ---->   reads (xi, eta, s) of the i-th marker in cell order,
+//                                                              evaluates 2 fields x 4 planes with near-broadcast LDS.128,
+//     reads 8 field values back, equilibrium + RHS     <----   writes physical-gradient results to the owner's row
+// The coefficient blocks of a patch of TP triangles plus a halo (SMAX slots), for a window of WK toroidal intervals
+// plus HK on either side, are staged per super-cell with 1-D TMA bulk copies (cp.async.bulk + mbarrier).
+// Markers whose stage position leaves the staged set take the slow path (global table through L1/L2).
+#pragma once
+#include "trimeg_math.cuh"
+
+namespace trimeg {
+
+struct TileTables {
+    const int* slots;        // [npatch][SMAX] global triangle per slot, -1 unused
+    const short* nbr;        // [npatch][SMAX][4] slot across edge e, -1 = not staged / boundary
+    const int* nslots;       // [npatch]
+    const int* offs;         // [ncell + 1] exclusive offsets of the cell-sorted marker store
+    int npatch, nwin, nsc;   // super-cells = npatch * nwin
+};
+
+template <int TP_, int SMAX_, int WK_, int NT_, int NG_>
+struct TileCfg {
+    static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD, NT = NT_, NG = NG_;   // NG groups of NT threads
+    static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
+    static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
+    static constexpr int NBINS = SMAX * NW + 1;      // + slow bin
+    static constexpr int CPS = TP * WK;              // cells per super-cell
+    static constexpr int SLOT_DOUBLES = NPL * PLANE_STRIDE;
+    static constexpr int HIST = ((NBINS + 31) / 32) * 32;
+    // shared memory carve-up (bytes)
+    static constexpr size_t OFF_COEF = 0;
+    static constexpr size_t OFF_GEOM = OFF_COEF + sizeof(double) * SMAX * SLOT_DOUBLES;
+    static constexpr size_t OFF_GRP = OFF_GEOM + 64 * SMAX;
+    static constexpr size_t GRP_BYTES = sizeof(double) * NT * 3 + sizeof(int) * NT + sizeof(double) * 8 * NT + sizeof(int) * NT + sizeof(int) * (HIST + 32);
+    static constexpr size_t OFF_MISC = OFF_GRP + GRP_BYTES * NG;
+    static constexpr size_t BYTES = OFF_MISC + 64;
+};
+
+struct __align__(16) SlotGeom {   // 64 B
+    double v0x, v0y, a11, a12, a21, a22;
+    short nbr[4];
+    int tri, pad;
+};
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, int count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count)); }
+__device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigned bytes, void* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src), "r"(bytes),
+                 "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void group_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+
+struct LdShared {   // coefficient pair fetch from the staged block
+    unsigned base;  // shared-space byte address of the cell's first plane
+    __device__ __forceinline__ void operator()(int idx, double& a, double& b) const {
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "r"(base + 16u * (unsigned)idx));
+    }
+};
+
+// exclusive scan of h[0..n) in place by one group of NT threads (n <= NT * PER); warp-shuffle based
+template <int NT, int HIST>
+__device__ __forceinline__ void group_scan(int* h, int* wsum, int gtid, int bar_id) {
+    constexpr int PER = (HIST + NT - 1) / NT;
+    int v[PER], s = 0;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) { int idx = gtid * PER + i; v[i] = idx < HIST ? h[idx] : 0; s += v[i]; }
+    int lane = gtid & 31, wid = gtid >> 5, x = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) wsum[wid] = x;
+    group_sync(bar_id, NT);
+    if (wid == 0) {
+        int t = lane < NT / 32 ? wsum[lane] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, t, o); if (lane >= o) t += y; }
+        if (lane < NT / 32) wsum[lane] = t;
+    }
+    group_sync(bar_id, NT);
+    int ex = (wid ? wsum[wid - 1] : 0) + x - s;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) { int idx = gtid * PER + i; if (idx < HIST) h[idx] = ex; ex += v[i]; }
+    group_sync(bar_id, NT);
+}
+
+}  // namespace trimeg
