@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -33,8 +34,8 @@ struct DevTables {
 };
 
 // tiled push configuration: patches of 16 triangles + halo (56 slots), windows of 4 toroidal intervals (+1 each side),
-// 4 groups of 128 threads per CTA, one CTA per SM
-using Tile = TileCfg<16, 56, 4, 128, 4>;
+// 16 independent warps per CTA, one CTA per SM
+using Tile = TileCfg<16, 56, 4, 16>;
 // cell numbering used by the sort: super-cell (patch, window) major, then triangle within the patch, then interval
 struct CellMap {
     int P, nwin;
@@ -224,43 +225,36 @@ __global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP s
 
 
 // ============================================================================================ tiled push (variant 0)
-struct TileGroupSmem {   // pointers into one group's slice of shared memory
-    double *ia, *ib, *ic, *res;
-    int *meta, *lost, *hist, *wsum;
+// queue of retired markers (lives in the inactive marker buffer): SoA with capacity cap
+struct RetireQueue {
+    double* y;      // [5][cap] stage position
+    double* acc;    // [5][cap] weighted sum of the k's so far
+    int* m;         // [cap] marker index
+    int* info;      // [cap] stage | status << 8
+    int* count;     // device counter
+    int cap;
 };
 
 template <class C>
-__global__ void __launch_bounds__(C::NT* C::NG, 1)
-k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, double dt, int* __restrict__ work_counter,
-             unsigned long long* __restrict__ stats) {
+__global__ void __launch_bounds__(C::NTHREADS, 1)
+k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, RetireQueue rq, double dt, int* __restrict__ work_counter) {
     extern __shared__ __align__(128) unsigned char smem[];
     double* coef = reinterpret_cast<double*>(smem + C::OFF_COEF);
     SlotGeom* sgeom = reinterpret_cast<SlotGeom*>(smem + C::OFF_GEOM);
     unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + C::OFF_MISC);
     int* sh_sc = reinterpret_cast<int*>(smem + C::OFF_MISC + 16);
-    int* sh_slow = reinterpret_cast<int*>(smem + C::OFF_MISC + 20);
+    int* sh_next = reinterpret_cast<int*>(smem + C::OFF_MISC + 20);
 
-    const int tid = threadIdx.x, grp = tid / C::NT, gtid = tid - grp * C::NT, bar_id = 1 + grp;
-    TileGroupSmem gs;
-    {
-        unsigned char* g0 = smem + C::OFF_GRP + C::GRP_BYTES * grp;
-        gs.ia = reinterpret_cast<double*>(g0);
-        gs.ib = gs.ia + C::NT;
-        gs.ic = gs.ib + C::NT;
-        gs.res = gs.ic + C::NT;
-        gs.meta = reinterpret_cast<int*>(gs.res + 8 * C::NT);
-        gs.lost = gs.meta + C::NT;
-        gs.hist = gs.lost + C::NT;
-        gs.wsum = gs.hist + C::HIST;
-    }
-    if (tid == 0) { mbar_init(mbar, 1); *sh_slow = 0; asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-    for (int i = gtid; i < C::HIST; i += C::NT) gs.hist[i] = 0;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    double* xch = reinterpret_cast<double*>(smem + C::OFF_WARP + C::WARP_BYTES * wid);   // [8][32]
+    if (tid == 0) { mbar_init(mbar, 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
     unsigned phase = 0;
     const int P = tb.tor.P;
     const double h2 = 0.5 * dt, h6 = dt / 6.0;
+    constexpr unsigned FULL = 0xffffffffu;
 
     for (;;) {
-        __syncthreads();   // previous super-cell fully consumed (coefficients, geometry, sh_sc)
+        __syncthreads();   // previous super-cell fully consumed (coefficients, geometry, sh_sc, sh_next)
         if (tid == 0) *sh_sc = atomicAdd(work_counter, 1);
         __syncthreads();
         const int sc = *sh_sc;
@@ -271,6 +265,7 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, d
         const int ns = tt.nslots[patch];
         const int* pslots = tt.slots + (long long)patch * C::SMAX;
         // ---- stage geometry (generic stores) and coefficient blocks (TMA bulk copies)
+        if (tid == 0) *sh_next = begin;
         if (tid < ns) {
             int t = pslots[tid];
             SlotGeom g;
@@ -289,7 +284,7 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, d
             int cnt = 0;
             for (int sl = tid; sl < ns; sl += 32) cnt += pslots[sl] >= 0;
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+            for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(FULL, cnt, o);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the block vs. the async writes
             if (tid == 0) mbar_expect_tx(mbar, (unsigned)(cnt * C::SLOT_DOUBLES * sizeof(double)));
             __syncwarp();
@@ -304,14 +299,17 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, d
         phase ^= 1;
         __syncthreads();
 
-        // ---- chunks of NT markers, one group each
-        for (int chunk = begin + grp * C::NT; chunk < end; chunk += C::NT * C::NG) {
-            const int m = chunk + gtid;
-            const bool active = m < end;
-            const int n_items = min(C::NT, end - chunk);
+        // ---- each warp grabs chunks of 32 markers until the super-cell is drained
+        for (;;) {
+            int chunk = 0;
+            if (lane == 0) chunk = atomicAdd(sh_next, 32);
+            chunk = __shfl_sync(FULL, chunk, 0);
+            if (chunk >= end) break;
+            const int m = chunk + lane;
+            bool alive = m < end;   // owner role: this lane still integrates a marker
             double y0[5], y[5], acc[5], mu = 0.0, pw = 0.0;
             int st = 0, home = -1, cur = -1, tri_last = -1;
-            if (active) {
+            if (alive) {
                 y0[0] = s.R[m]; y0[1] = s.Z[m]; y0[2] = s.phi[m]; y0[3] = s.u[m]; y0[4] = s.w[m];
                 mu = s.mu[m]; pw = s.p[m]; st = s.status[m];
                 tri_last = s.tri[m];
@@ -330,10 +328,10 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, d
 
 #pragma unroll 1
             for (int stage = 0; stage < 4; ++stage) {
-                // -- owner: locate in slot space, toroidal cell, counting-sort rank
-                int bin = C::NBINS - 1, rank = 0;
-                double ia = y[0], ib = y[1], ic = y[2];
-                if (active) {
+                // -- owner: locate in slot space, toroidal cell
+                int key = 0x7fffffff;
+                double ia = 0.0, ib = 0.0, ic = 0.0;
+                if (alive) {
                     int sl = cur >= 0 ? cur : home;
                     double xi = 0.0, eta = 0.0;
                     if (sl >= 0) {
@@ -356,64 +354,81 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, d
                     int dk = k - k0;
                     if (dk > P / 2) dk -= P; else if (dk < -(P / 2)) dk += P;
                     int lk = dk + C::HK;
-                    cur = sl;
                     if (sl >= 0 && lk >= 0 && lk < C::NW) {
-                        bin = sl * C::NW + lk;
+                        cur = sl;
+                        key = ((sl * C::NW + lk) << 5) | lane;
                         ia = xi; ib = eta; ic = sf;
                         tri_last = sgeom[sl].tri;
+                    } else {
+                        // left the staged block: retire (the follow-up kernel finishes this step from here)
+                        int slot = atomicAdd(rq.count, 1);
+                        if (slot < rq.cap) {
+#pragma unroll
+                            for (int q = 0; q < 5; ++q) { rq.y[(size_t)q * rq.cap + slot] = y[q]; rq.acc[(size_t)q * rq.cap + slot] = acc[q]; }
+                            rq.m[slot] = m;
+                            rq.info[slot] = stage | (st << 8);
+                            alive = false;
+                        } else {   // queue full (pathological): evaluate in place through the global tables
+                            int t = tri_last;
+                            double d[5];
+                            st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, pw, d);
+                            if (t >= 0) tri_last = t;
+                            const double wgt = (stage == 0 || stage == 3) ? 1.0 : 2.0;
+                            const double hs = stage == 2 ? dt : h2;
+#pragma unroll
+                            for (int q = 0; q < 5; ++q) { acc[q] = fma(wgt, d[q], acc[q]); y[q] = fma(hs, d[q], y0[q]); }
+                            key = 0x7ffffffe;   // participates in the exchange as a no-op
+                        }
                     }
-                    rank = atomicAdd(gs.hist + bin, 1);
                 }
-                group_sync(bar_id, C::NT);
-                group_scan<C::NT, C::HIST>(gs.hist, gs.wsum, gtid, bar_id);
-                if (active) {
-                    int pos = gs.hist[bin] + rank;
-                    gs.ia[pos] = ia; gs.ib[pos] = ib; gs.ic[pos] = ic;
-                    gs.meta[pos] = gtid | (bin << 12);
-                }
-                group_sync(bar_id, C::NT);
-                for (int i = gtid; i < C::HIST; i += C::NT) gs.hist[i] = 0;   // next stage's histogram
-                // -- gather thread: item gtid in cell order
-                if (gtid < n_items) {
-                    const int meta = gs.meta[gtid], owner = meta & 0xfff, b = meta >> 12;
-                    const double a_ = gs.ia[gtid], b_ = gs.ib[gtid], c_ = gs.ic[gtid];
-                    Fields f;
-                    int lost = 0;
-                    if (b != C::NBINS - 1) {
-                        const int sl = b / C::NW, lk = b - sl * C::NW;
-                        double w[4], dw[4], g8[8];
-                        bspline_from_s(tb.tor, c_, w, dw);
-                        LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
-                        gather_cell(ld, a_, b_, w, dw, g8);
-                        const SlotGeom& g = sgeom[sl];
-                        f.P = g8[0]; f.PR = fma(g.a11, g8[1], g.a21 * g8[2]); f.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); f.Pp = g8[3];
-                        f.A = g8[4]; f.AR = fma(g.a11, g8[5], g.a21 * g8[6]); f.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); f.Ap = g8[7];
-                    } else {   // slow path: global tables
-                        int t = locate_box(tb.bg, tb.geom, a_, b_);
-                        gather_at(tb, t, a_, b_, c_, f);
-                        lost = t < 0;
-                        atomicAdd(sh_slow, 1);
+                // -- regroup the warp's lanes by cell: bitonic sort of (cell, lane) keys
+                xch[lane] = ia; xch[32 + lane] = ib; xch[64 + lane] = ic;
+                int skey = key;
+#pragma unroll
+                for (int kk = 2; kk <= 32; kk <<= 1) {
+#pragma unroll
+                    for (int j = kk >> 1; j > 0; j >>= 1) {
+                        int other = __shfl_xor_sync(FULL, skey, j);
+                        bool up = (lane & kk) == 0, lower = (lane & j) == 0;
+                        skey = (lower == up) ? min(skey, other) : max(skey, other);
                     }
-                    double* r = gs.res + owner;
-                    r[0] = f.P; r[C::NT] = f.PR; r[2 * C::NT] = f.PZ; r[3 * C::NT] = f.Pp;
-                    r[4 * C::NT] = f.A; r[5 * C::NT] = f.AR; r[6 * C::NT] = f.AZ; r[7 * C::NT] = f.Ap;
-                    gs.lost[owner] = lost;
                 }
-                group_sync(bar_id, C::NT);
+                __syncwarp();
+                // -- gather lane: the lane-th marker of the warp in cell order
+                const bool work = skey < 0x7ffffffe;
+                const int owner = skey & 31, bin = skey >> 5;
+                Fields f{0, 0, 0, 0, 0, 0, 0, 0};
+                if (work) {
+                    const double a_ = xch[owner], b_ = xch[32 + owner], c_ = xch[64 + owner];
+                    const int sl = bin / C::NW, lk = bin - sl * C::NW;
+                    double w[4], dw[4], g8[8];
+                    bspline_from_s(tb.tor, c_, w, dw);
+                    LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
+                    gather_cell(ld, a_, b_, w, dw, g8);
+                    const SlotGeom& g = sgeom[sl];
+                    f.P = g8[0]; f.PR = fma(g.a11, g8[1], g.a21 * g8[2]); f.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); f.Pp = g8[3];
+                    f.A = g8[4]; f.AR = fma(g.a11, g8[5], g.a21 * g8[6]); f.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); f.Ap = g8[7];
+                }
+                __syncwarp();   // all items read before the rows are reused for results
+                if (work) {
+                    double* r = xch + owner;
+                    r[0] = f.P; r[32] = f.PR; r[64] = f.PZ; r[96] = f.Pp; r[128] = f.A; r[160] = f.AR; r[192] = f.AZ; r[224] = f.Ap;
+                }
+                __syncwarp();
                 // -- owner: equilibrium, equations of motion, RK4 bookkeeping
-                if (active) {
-                    const double* r = gs.res + gtid;
-                    Fields f{r[0], r[C::NT], r[2 * C::NT], r[3 * C::NT], r[4 * C::NT], r[5 * C::NT], r[6 * C::NT], r[7 * C::NT]};
-                    st |= gs.lost[gtid];
+                if (alive && key < 0x7ffffffe) {
+                    const double* r = xch + lane;
+                    Fields fo{r[0], r[32], r[64], r[96], r[128], r[160], r[192], r[224]};
                     double d[5];
-                    rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, f, d);
+                    rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, fo, d);
                     const double wgt = (stage == 0 || stage == 3) ? 1.0 : 2.0;
                     const double hs = stage == 2 ? dt : h2;
 #pragma unroll
                     for (int q = 0; q < 5; ++q) { acc[q] = fma(wgt, d[q], acc[q]); y[q] = fma(hs, d[q], y0[q]); }
                 }
+                __syncwarp();   // results read before the next stage's items overwrite the rows
             }
-            if (active) {
+            if (alive) {
 #pragma unroll
                 for (int q = 0; q < 5; ++q) y[q] = fma(h6, acc[q], y0[q]);
                 double ph = fma(-tb.tor.period, floor(y[2] * tb.tor.inv_period), y[2]);
@@ -425,8 +440,36 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, d
             }
         }
     }
-    __syncthreads();
-    if (tid == 0 && *sh_slow) atomicAdd(stats + 1, (unsigned long long)*sh_slow);
+}
+
+// finish the step of the retired markers through the global tables (same arithmetic as the simple path)
+__global__ void __launch_bounds__(128) k_push_finish(DevTables tb, EquilP ep, SpeciesP sp, MarkerSoA s, RetireQueue rq, double dt) {
+    const int count = min(*rq.count, rq.cap);
+    const double h2 = 0.5 * dt, h6 = dt / 6.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < count; i += gridDim.x * blockDim.x) {
+        const int m = rq.m[i], info = rq.info[i];
+        int st = info >> 8, t = s.tri[m];
+        double y0[5] = {s.R[m], s.Z[m], s.phi[m], s.u[m], s.w[m]};
+        const double mu = s.mu[m], p = s.p[m];
+        double y[5], acc[5], d[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { y[q] = rq.y[(size_t)q * rq.cap + i]; acc[q] = rq.acc[(size_t)q * rq.cap + i]; }
+        for (int stage = info & 0xff; stage < 4; ++stage) {
+            st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, d);
+            const double wgt = (stage == 0 || stage == 3) ? 1.0 : 2.0;
+            const double hs = stage == 2 ? dt : h2;
+#pragma unroll
+            for (int q = 0; q < 5; ++q) { acc[q] = fma(wgt, d[q], acc[q]); y[q] = fma(hs, d[q], y0[q]); }
+        }
+#pragma unroll
+        for (int q = 0; q < 5; ++q) y[q] = fma(h6, acc[q], y0[q]);
+        double ph = fma(-tb.tor.period, floor(y[2] * tb.tor.inv_period), y[2]);
+        if (ph < 0.0) ph += tb.tor.period;
+        if (ph >= tb.tor.period) ph -= tb.tor.period;
+        s.R[m] = y[0]; s.Z[m] = y[1]; s.phi[m] = ph; s.u[m] = y[3]; s.w[m] = y[4];
+        if (t >= 0) s.tri[m] = t;
+        s.status[m] = st;
+    }
 }
 
 // ============================================================================================ marker store / sort
@@ -524,6 +567,8 @@ __global__ void __launch_bounds__(256) k_sort_scatter(MarkerSoA a, MarkerSoA b, 
     b.R[pos] = a.R[m]; b.Z[pos] = a.Z[m]; b.phi[pos] = a.phi[m]; b.u[pos] = a.u[m]; b.w[pos] = a.w[m];
     b.mu[pos] = a.mu[m]; b.p[pos] = a.p[m]; b.tri[pos] = a.tri[m]; b.status[pos] = a.status[m]; b.id[pos] = a.id[m];
 }
+
+__global__ void k_accumulate_stat(const int* __restrict__ v, unsigned long long* __restrict__ acc) { *acc += (unsigned long long)*v; }
 
 // ============================================================================================ DFMA micro-benchmark
 __global__ void __launch_bounds__(512) k_dfma(double* out, int iters, double a, double b) {
@@ -937,15 +982,25 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps) {
             if (rc) return rc;
         }
         if (ctx->variant == 0 && ctx->tiled_ok) {
-            CU(cudaMemsetAsync(ctx->d_work, 0, sizeof(int), ctx->stream));
-            k_push_tiled<Tile><<<ctx->num_sms, Tile::NT * Tile::NG, Tile::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, ctx->buf[ctx->cur], dt,
-                                                                                           ctx->d_work, ctx->d_stats);
+            // retire queue lives in the inactive marker buffer (free between sorts)
+            MarkerSoA& spare = ctx->buf[ctx->cur ^ 1];
+            RetireQueue rq;
+            const size_t pool = (size_t)((char*)spare.tri - (char*)spare.R);   // the seven double arrays are contiguous
+            rq.cap = (int)std::min<size_t>((size_t)n, pool / (10 * sizeof(double) + 2 * sizeof(int)));
+            rq.y = spare.R; rq.acc = rq.y + 5 * (size_t)rq.cap;
+            rq.m = (int*)(rq.acc + 5 * (size_t)rq.cap); rq.info = rq.m + rq.cap;
+            rq.count = ctx->d_work + 1;
+            CU(cudaMemsetAsync(ctx->d_work, 0, 2 * sizeof(int), ctx->stream));
+            k_push_tiled<Tile><<<ctx->num_sms, Tile::NTHREADS, Tile::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, ctx->buf[ctx->cur], rq, dt, ctx->d_work);
             KCHECK();
-            // markers outside the mesh sit behind the last cell: push them with the simple kernel
-            // (their count is only known on the device; the launch is sized for the worst case of 0..n and exits early)
+            k_push_finish<<<ctx->num_sms * 8, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->buf[ctx->cur], rq, dt);
+            KCHECK();
+            k_accumulate_stat<<<1, 1, 0, ctx->stream>>>(ctx->d_work + 1, ctx->d_stats + 1);
+            KCHECK();
+            // markers outside the mesh sit behind the last cell: push them through the simple path
             k_push_lost<<<148 * 4, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->buf[ctx->cur], ctx->d_offs + ctx->ncell, n, dt);
             KCHECK();
-            ctx->stats[0] += 2;
+            ctx->stats[0] += 4;
         } else {
             k_push_simple<<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->buf[ctx->cur], n, dt);
             KCHECK();

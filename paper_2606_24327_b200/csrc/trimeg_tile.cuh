@@ -6,14 +6,18 @@
 // the same address (measured), i.e. 168 cycles per warp -- if the lanes of a warp sit in the same few cells.  RK
 // stages 2-4 are evaluated at displaced positions (at dt = 0.05 most markers leave their home triangle), so lanes
 // are re-grouped by cell before every gather:
-//   owner thread (holds the marker's RK state in registers)   gather thread (rank i in cell order)
+//   owner lane (holds the marker's RK state in registers)      gather lane (rank i of the warp in cell order)
 //     locate by edge walk in the staged patch, B-spline cell
-//     counting sort by (slot, plane) in shared memory  ---->   reads (xi, eta, s) of the i-th marker in cell order,
+//     warp bitonic sort of (cell, lane) keys           ---->   reads (xi, eta, s) of the i-th marker in cell order,
 //                                                              evaluates 2 fields x 4 planes with near-broadcast LDS.128,
 //     reads 8 field values back, equilibrium + RHS     <----   writes physical-gradient results to the owner's row
+// Everything between two stagings is warp-synchronous (no block barrier): the 16 warps of the CTA run independently
+// and hide each other's latencies.
 // The coefficient blocks of a patch of TP triangles plus a halo (SMAX slots), for a window of WK toroidal intervals
 // plus HK on either side, are staged per super-cell with 1-D TMA bulk copies (cp.async.bulk + mbarrier).
-// Markers whose stage position leaves the staged set take the slow path (global table through L1/L2).
+// A marker whose stage position leaves the staged set RETIRES: it parks (marker index, stage, y_stage, k-sum) in a
+// global queue and a follow-up kernel finishes its step through the global tables, so that no warp ever waits on
+// a divergent slow lane.
 #pragma once
 #include "trimeg_math.cuh"
 
@@ -27,21 +31,20 @@ struct TileTables {
     int npatch, nwin, nsc;   // super-cells = npatch * nwin
 };
 
-template <int TP_, int SMAX_, int WK_, int NT_, int NG_>
+template <int TP_, int SMAX_, int WK_, int NWARPS_>
 struct TileCfg {
-    static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD, NT = NT_, NG = NG_;   // NG groups of NT threads
+    static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD, NWARPS = NWARPS_, NTHREADS = 32 * NWARPS_;
     static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
     static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
-    static constexpr int NBINS = SMAX * NW + 1;      // + slow bin
+    static constexpr int NBINS = SMAX * NW;          // (slot, local interval) cells of the staged block
     static constexpr int CPS = TP * WK;              // cells per super-cell
     static constexpr int SLOT_DOUBLES = NPL * PLANE_STRIDE;
-    static constexpr int HIST = ((NBINS + 31) / 32) * 32;
     // shared memory carve-up (bytes)
     static constexpr size_t OFF_COEF = 0;
     static constexpr size_t OFF_GEOM = OFF_COEF + sizeof(double) * SMAX * SLOT_DOUBLES;
-    static constexpr size_t OFF_GRP = OFF_GEOM + 64 * SMAX;
-    static constexpr size_t GRP_BYTES = sizeof(double) * NT * 3 + sizeof(int) * NT + sizeof(double) * 8 * NT + sizeof(int) * NT + sizeof(int) * (HIST + 32);
-    static constexpr size_t OFF_MISC = OFF_GRP + GRP_BYTES * NG;
+    static constexpr size_t OFF_WARP = OFF_GEOM + 64 * SMAX;
+    static constexpr size_t WARP_BYTES = sizeof(double) * 32 * 8;   // per-warp exchange: items (3 x 32) then results (8 x 32) reuse the same rows
+    static constexpr size_t OFF_MISC = OFF_WARP + WARP_BYTES * NWARPS;
     static constexpr size_t BYTES = OFF_MISC + 64;
 };
 
@@ -75,30 +78,5 @@ struct LdShared {   // coefficient pair fetch from the staged block
         asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "r"(base + 16u * (unsigned)idx));
     }
 };
-
-// exclusive scan of h[0..n) in place by one group of NT threads (n <= NT * PER); warp-shuffle based
-template <int NT, int HIST>
-__device__ __forceinline__ void group_scan(int* h, int* wsum, int gtid, int bar_id) {
-    constexpr int PER = (HIST + NT - 1) / NT;
-    int v[PER], s = 0;
-#pragma unroll
-    for (int i = 0; i < PER; ++i) { int idx = gtid * PER + i; v[i] = idx < HIST ? h[idx] : 0; s += v[i]; }
-    int lane = gtid & 31, wid = gtid >> 5, x = s;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
-    if (lane == 31) wsum[wid] = x;
-    group_sync(bar_id, NT);
-    if (wid == 0) {
-        int t = lane < NT / 32 ? wsum[lane] : 0;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, t, o); if (lane >= o) t += y; }
-        if (lane < NT / 32) wsum[lane] = t;
-    }
-    group_sync(bar_id, NT);
-    int ex = (wid ? wsum[wid - 1] : 0) + x - s;
-#pragma unroll
-    for (int i = 0; i < PER; ++i) { int idx = gtid * PER + i; if (idx < HIST) h[idx] = ex; ex += v[i]; }
-    group_sync(bar_id, NT);
-}
 
 }  // namespace trimeg
