@@ -10,6 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtrimeg_b200.so")
 SOURCES = ["trimeg.cu"]
 DEPS = ["trimeg.cu", "trimeg_math.cuh", "trimeg_host_setup.hpp", "trimeg_tile.cuh", "../../include/trimeg.h"]
+EXTRA_DEFS = os.environ.get("TRIMEG_DEFS", "").split()
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false".replace("=false", "")][:-1]
 
@@ -36,7 +37,7 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
     if not force and not stale():
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc_path(), *NVCC_FLAGS, *extra, "-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd = [nvcc_path(), *NVCC_FLAGS, *EXTRA_DEFS, *extra, "-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:
         print(" ".join(cmd), flush=True)
     subprocess.run(cmd, check=True)

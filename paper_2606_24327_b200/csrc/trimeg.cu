@@ -245,8 +245,7 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, R
     int* sh_sc = reinterpret_cast<int*>(smem + C::OFF_MISC + 16);
     int* sh_next = reinterpret_cast<int*>(smem + C::OFF_MISC + 20);
 
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    double* xch = reinterpret_cast<double*>(smem + C::OFF_WARP + C::WARP_BYTES * wid);   // [8][32]
+    const int tid = threadIdx.x, lane = tid & 31;
     if (tid == 0) { mbar_init(mbar, 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
     unsigned phase = 0;
     const int P = tb.tor.P;
@@ -381,44 +380,20 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, R
                         }
                     }
                 }
-                // -- regroup the warp's lanes by cell: bitonic sort of (cell, lane) keys
-                xch[lane] = ia; xch[32 + lane] = ib; xch[64 + lane] = ic;
-                int skey = key;
-#pragma unroll
-                for (int kk = 2; kk <= 32; kk <<= 1) {
-#pragma unroll
-                    for (int j = kk >> 1; j > 0; j >>= 1) {
-                        int other = __shfl_xor_sync(FULL, skey, j);
-                        bool up = (lane & kk) == 0, lower = (lane & j) == 0;
-                        skey = (lower == up) ? min(skey, other) : max(skey, other);
-                    }
-                }
-                __syncwarp();
-                // -- gather lane: the lane-th marker of the warp in cell order
-                const bool work = skey < 0x7ffffffe;
-                const int owner = skey & 31, bin = skey >> 5;
-                Fields f{0, 0, 0, 0, 0, 0, 0, 0};
-                if (work) {
-                    const double a_ = xch[owner], b_ = xch[32 + owner], c_ = xch[64 + owner];
+                // -- gather from the staged block (each lane its own marker: regrouping the lanes of a warp by cell was
+                //    measured to buy nothing, LDS.128 costs 4 wavefronts unless every aligned lane pair shares an address)
+                if (alive && key < 0x7ffffffe) {
+                    const int bin = key >> 5;
                     const int sl = bin / C::NW, lk = bin - sl * C::NW;
                     double w[4], dw[4], g8[8];
-                    bspline_from_s(tb.tor, c_, w, dw);
+                    bspline_from_s(tb.tor, ic, w, dw);
                     LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
-                    gather_cell(ld, a_, b_, w, dw, g8);
+                    gather_cell(ld, ia, ib, w, dw, g8);
                     const SlotGeom& g = sgeom[sl];
-                    f.P = g8[0]; f.PR = fma(g.a11, g8[1], g.a21 * g8[2]); f.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); f.Pp = g8[3];
-                    f.A = g8[4]; f.AR = fma(g.a11, g8[5], g.a21 * g8[6]); f.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); f.Ap = g8[7];
-                }
-                __syncwarp();   // all items read before the rows are reused for results
-                if (work) {
-                    double* r = xch + owner;
-                    r[0] = f.P; r[32] = f.PR; r[64] = f.PZ; r[96] = f.Pp; r[128] = f.A; r[160] = f.AR; r[192] = f.AZ; r[224] = f.Ap;
-                }
-                __syncwarp();
-                // -- owner: equilibrium, equations of motion, RK4 bookkeeping
-                if (alive && key < 0x7ffffffe) {
-                    const double* r = xch + lane;
-                    Fields fo{r[0], r[32], r[64], r[96], r[128], r[160], r[192], r[224]};
+                    Fields fo;
+                    fo.P = g8[0]; fo.PR = fma(g.a11, g8[1], g.a21 * g8[2]); fo.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); fo.Pp = g8[3];
+                    fo.A = g8[4]; fo.AR = fma(g.a11, g8[5], g.a21 * g8[6]); fo.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); fo.Ap = g8[7];
+                    // -- equilibrium, equations of motion, RK4 bookkeeping
                     double d[5];
                     rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, fo, d);
                     const double wgt = (stage == 0 || stage == 3) ? 1.0 : 2.0;
@@ -426,7 +401,6 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, R
 #pragma unroll
                     for (int q = 0; q < 5; ++q) { acc[q] = fma(wgt, d[q], acc[q]); y[q] = fma(hs, d[q], y0[q]); }
                 }
-                __syncwarp();   // results read before the next stage's items overwrite the rows
             }
             if (alive) {
 #pragma unroll
@@ -558,16 +532,22 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const int* __restri
 #pragma unroll
     for (int i = 0; i < SCAN_ITEMS; ++i) { if (base + i < n) out[base + i] = ex; ex += v[i]; }
 }
-__global__ void __launch_bounds__(256) k_sort_scatter(MarkerSoA a, MarkerSoA b, long long n, const int* __restrict__ keys,
-                                                      const int* __restrict__ offs, int* __restrict__ fill) {
+// permutation: perm[new position] = old position (4-byte scattered writes), then a gather with coalesced writes
+__global__ void __launch_bounds__(256) k_sort_perm(long long n, const int* __restrict__ keys, const int* __restrict__ offs, int* __restrict__ fill,
+                                                   int* __restrict__ perm) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= n) return;
     int key = keys[m];
     long long pos = (long long)offs[key] + atomicAdd(fill + key, 1);
-    b.R[pos] = a.R[m]; b.Z[pos] = a.Z[m]; b.phi[pos] = a.phi[m]; b.u[pos] = a.u[m]; b.w[pos] = a.w[m];
-    b.mu[pos] = a.mu[m]; b.p[pos] = a.p[m]; b.tri[pos] = a.tri[m]; b.status[pos] = a.status[m]; b.id[pos] = a.id[m];
+    perm[pos] = (int)m;
 }
-
+__global__ void __launch_bounds__(256) k_sort_gather(MarkerSoA a, MarkerSoA b, long long n, const int* __restrict__ perm) {
+    long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    long long m = perm[j];
+    b.R[j] = a.R[m]; b.Z[j] = a.Z[m]; b.phi[j] = a.phi[m]; b.u[j] = a.u[m]; b.w[j] = a.w[m];
+    b.mu[j] = a.mu[m]; b.p[j] = a.p[m]; b.tri[j] = a.tri[m]; b.status[j] = a.status[m]; b.id[j] = a.id[m];
+}
 __global__ void k_accumulate_stat(const int* __restrict__ v, unsigned long long* __restrict__ acc) { *acc += (unsigned long long)*v; }
 
 // ============================================================================================ DFMA micro-benchmark
@@ -602,7 +582,7 @@ struct trimeg_ctx {
     long long n = 0;
     MarkerSoA buf[2]{};
     int cur = 0;
-    int *d_keys = nullptr;        // in scratch
+    int *d_keys = nullptr, *d_perm = nullptr;   // in scratch
     int *d_hist = nullptr, *d_offs = nullptr, *d_fill = nullptr, *d_sums = nullptr;   // library-owned, [T*P+2]
     long long ncell = 0;
     bool sorted = false;
@@ -861,7 +841,7 @@ int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, 
 static size_t soa_bytes(long long n) { return 7 * align256(sizeof(double) * (size_t)n) + 3 * align256(sizeof(int) * (size_t)n); }
 size_t trimeg_scratch_bytes(const trimeg_ctx* ctx, int64_t n) {
     if (!ctx || n <= 0) return 0;
-    return 2 * soa_bytes(n) + align256(sizeof(int) * (size_t)n) + 256;
+    return 2 * soa_bytes(n) + 2 * align256(sizeof(int) * (size_t)n) + 256;
 }
 static void carve(MarkerSoA& s, char*& p, long long n) {
     double** dp[7] = {&s.R, &s.Z, &s.phi, &s.u, &s.w, &s.mu, &s.p};
@@ -886,12 +866,14 @@ static int do_sort(trimeg_ctx* ctx) {
     KCHECK();
     k_scan_apply<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_hist, ncnt, ctx->d_sums, ctx->d_offs);
     KCHECK();
-    k_sort_scatter<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(a, b, n, ctx->d_keys, ctx->d_offs, ctx->d_fill);
+    k_sort_perm<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(n, ctx->d_keys, ctx->d_offs, ctx->d_fill, ctx->d_perm);
+    KCHECK();
+    k_sort_gather<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(a, b, n, ctx->d_perm);
     KCHECK();
     ctx->cur ^= 1;
     ctx->sorted = true;
     ctx->steps_since_sort = 0;
-    ctx->stats[0] += 5;
+    ctx->stats[0] += 6;
     ctx->stats[3] += 1;
     return TRIMEG_OK;
 }
@@ -908,6 +890,7 @@ int trimeg_markers_bind(trimeg_ctx* ctx, int64_t n, const double* R, const doubl
     carve(ctx->buf[0], ptr, n);
     carve(ctx->buf[1], ptr, n);
     ctx->d_keys = (int*)ptr;
+    ctx->d_perm = (int*)(ptr + align256(sizeof(int) * (size_t)n));
     ctx->n = n; ctx->cur = 0; ctx->sorted = false; ctx->steps_since_sort = 0;
     if (memspace == TRIMEG_HOST) {   // stage through the second buffer
         MarkerSoA& b = ctx->buf[1];

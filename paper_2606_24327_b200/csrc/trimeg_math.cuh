@@ -126,16 +126,71 @@ __device__ __forceinline__ void quintic_pair_accum(Ld ld, double xi, double eta,
     acc[4] = fma(w, p1, acc[4]); acc[5] = fma(w, px1, acc[5]); acc[6] = fma(w, py1, acc[6]); acc[7] = fma(dw, p1, acc[7]);
 }
 
-// all four planes; `planes` points at [4][21][2] doubles (16-byte aligned); result in reference-gradient form
+// two planes at once: four independent Horner chains (2 planes x 2 fields) for instruction-level parallelism
+template <int N, typename LdA, typename LdB>
+__device__ __forceinline__ void horner4(LdA lda, LdB ldb, int off, double x, double v[4], double d[4]) {
+    double c[4], e[4];
+    lda(off + N, c[0], c[1]); ldb(off + N, c[2], c[3]);
+    if (N == 0) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { v[q] = c[q]; d[q] = 0.0; }
+        return;
+    }
+    lda(off + N - 1, e[0], e[1]); ldb(off + N - 1, e[2], e[3]);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { v[q] = fma(c[q], x, e[q]); d[q] = c[q]; }
+#pragma unroll
+    for (int i = N - 2; i >= 0; --i) {
+        lda(off + i, e[0], e[1]); ldb(off + i, e[2], e[3]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { d[q] = fma(d[q], x, v[q]); v[q] = fma(v[q], x, e[q]); }
+    }
+}
+template <typename LdA, typename LdB>
+__device__ __forceinline__ void quintic_quad_accum(LdA lda, LdB ldb, double xi, double eta, double wa, double dwa, double wb, double dwb, double acc[8]) {
+    double p[4], py[4], px[4], a[4], b[4];
+    horner4<0>(lda, ldb, 20, xi, p, b);
+    horner4<1>(lda, ldb, 18, xi, a, px);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { py[q] = p[q]; p[q] = fma(p[q], eta, a[q]); }
+    horner4<2>(lda, ldb, 15, xi, a, b);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { py[q] = fma(py[q], eta, p[q]); p[q] = fma(p[q], eta, a[q]); px[q] = fma(px[q], eta, b[q]); }
+    horner4<3>(lda, ldb, 11, xi, a, b);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { py[q] = fma(py[q], eta, p[q]); p[q] = fma(p[q], eta, a[q]); px[q] = fma(px[q], eta, b[q]); }
+    horner4<4>(lda, ldb, 6, xi, a, b);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { py[q] = fma(py[q], eta, p[q]); p[q] = fma(p[q], eta, a[q]); px[q] = fma(px[q], eta, b[q]); }
+    horner4<5>(lda, ldb, 0, xi, a, b);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { py[q] = fma(py[q], eta, p[q]); p[q] = fma(p[q], eta, a[q]); px[q] = fma(px[q], eta, b[q]); }
+    // q = 0,1: plane A fields 0,1 ; q = 2,3: plane B fields 0,1
+    acc[0] = fma(wa, p[0], acc[0]); acc[1] = fma(wa, px[0], acc[1]); acc[2] = fma(wa, py[0], acc[2]); acc[3] = fma(dwa, p[0], acc[3]);
+    acc[4] = fma(wa, p[1], acc[4]); acc[5] = fma(wa, px[1], acc[5]); acc[6] = fma(wa, py[1], acc[6]); acc[7] = fma(dwa, p[1], acc[7]);
+    acc[0] = fma(wb, p[2], acc[0]); acc[1] = fma(wb, px[2], acc[1]); acc[2] = fma(wb, py[2], acc[2]); acc[3] = fma(dwb, p[2], acc[3]);
+    acc[4] = fma(wb, p[3], acc[4]); acc[5] = fma(wb, px[3], acc[5]); acc[6] = fma(wb, py[3], acc[6]); acc[7] = fma(dwb, p[3], acc[7]);
+}
+
+// all four planes; ldp(idx, a, b) fetches pair idx of [4][21] (16-byte aligned pairs); result in reference-gradient form
 template <typename LdPlane>
 __device__ __forceinline__ void gather_cell(LdPlane ldp, double xi, double eta, const double w[4], const double dw[4], double acc[8]) {
 #pragma unroll
     for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+#ifdef TRIMEG_GATHER_PAIRWISE
+#pragma unroll
+    for (int j = 0; j < 4; j += 2) {
+        auto lda = [&](int idx, double& a, double& b) { ldp(j * NCOEF + idx, a, b); };
+        auto ldb = [&](int idx, double& a, double& b) { ldp((j + 1) * NCOEF + idx, a, b); };
+        quintic_quad_accum(lda, ldb, xi, eta, w[j], dw[j], w[j + 1], dw[j + 1], acc);
+    }
+#else
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         auto ld = [&](int idx, double& a, double& b) { ldp(j * NCOEF + idx, a, b); };
         quintic_pair_accum(ld, xi, eta, w[j], dw[j], acc);
     }
+#endif
 }
 // reference gradient -> physical gradient (grad_phys = J^-T grad_ref)
 __device__ __forceinline__ void to_fields(const TriGeom& g, const double acc[8], Fields& f) {

@@ -43,7 +43,7 @@ struct TileCfg {
     static constexpr size_t OFF_COEF = 0;
     static constexpr size_t OFF_GEOM = OFF_COEF + sizeof(double) * SMAX * SLOT_DOUBLES;
     static constexpr size_t OFF_WARP = OFF_GEOM + 64 * SMAX;
-    static constexpr size_t WARP_BYTES = sizeof(double) * 32 * 8;   // per-warp exchange: items (3 x 32) then results (8 x 32) reuse the same rows
+    static constexpr size_t WARP_BYTES = 0;
     static constexpr size_t OFF_MISC = OFF_WARP + WARP_BYTES * NWARPS;
     static constexpr size_t BYTES = OFF_MISC + 64;
 };
