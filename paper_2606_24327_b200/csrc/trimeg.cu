@@ -33,9 +33,9 @@ struct DevTables {
     long long tri_stride;    // doubles per triangle = (P+3+2*PLANE_PAD)*42
 };
 
-// tiled push configuration: patches of 16 triangles + halo (56 slots), windows of 4 toroidal intervals (+1 each side),
+// tiled push configuration: patches of 8 triangles + halo (36 slots), windows of 4 toroidal intervals (+1 each side), ring of 2 staged blocks,
 // 16 independent warps per CTA, one CTA per SM
-using Tile = TileCfg<16, 56, 4, 16>;
+using Tile = TileCfg<8, 36, 4, 16>;
 // cell numbering used by the sort: super-cell (patch, window) major, then triangle within the patch, then interval
 struct CellMap {
     int P, nwin;
@@ -235,68 +235,91 @@ struct RetireQueue {
     int cap;
 };
 
+// (re)fill ring entry b with the next non-empty super-cell; executed by one whole warp.  The entry's mbarrier completes
+// when the TMA bytes have landed (or at once, with sc = -1, when the work list is exhausted).
+template <class C>
+__device__ __forceinline__ void tile_refill(unsigned char* smem, int b, const DevTables& tb, const TileTables& tt, int* work_counter, int lane) {
+    constexpr unsigned FULL = 0xffffffffu;
+    double* coef = reinterpret_cast<double*>(smem + C::BLOCK_BYTES * b);
+    SlotGeom* sgeom = reinterpret_cast<SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
+    BlockCtrl* ctl = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL) + b;
+    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF) + 2 * b;
+    int sc = 0, begin = 0, end = 0;
+    for (;;) {
+        if (lane == 0) sc = atomicAdd(work_counter, 1);
+        sc = __shfl_sync(FULL, sc, 0);
+        if (sc >= tt.nsc) { sc = -1; break; }
+        begin = tt.offs[(long long)sc * C::CPS]; end = tt.offs[(long long)(sc + 1) * C::CPS];
+        if (begin != end) break;
+    }
+    if (sc < 0) {
+        if (lane == 0) { ctl->sc = -1; ctl->left = 0; __threadfence_block(); asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(mbar)) : "memory"); }
+        return;
+    }
+    const int patch = sc / tt.nwin, k0 = (sc - patch * tt.nwin) * C::WK;
+    const int ns = tt.nslots[patch];
+    const int* pslots = tt.slots + (long long)patch * C::SMAX;
+    if (lane == 0) { ctl->sc = sc; ctl->begin = begin; ctl->end = end; ctl->next = begin; ctl->left = 0; ctl->ns = ns; ctl->patch = patch; ctl->k0 = k0; }
+    int cnt = 0;
+    for (int sl = lane; sl < ns; sl += 32) {
+        int t = pslots[sl];
+        SlotGeom g;
+        if (t >= 0) {
+            const TriGeom tg = tb.geom[t];
+            g.v0x = tg.v0x; g.v0y = tg.v0y; g.a11 = tg.a11; g.a12 = tg.a12; g.a21 = tg.a21; g.a22 = tg.a22;
+            const short* nb = tt.nbr + ((long long)patch * C::SMAX + sl) * 4;
+            g.nbr[0] = nb[0]; g.nbr[1] = nb[1]; g.nbr[2] = nb[2]; g.nbr[3] = -1;
+            cnt++;
+        } else {
+            g.v0x = g.v0y = 1e300; g.a11 = g.a12 = g.a21 = g.a22 = 0.0; g.nbr[0] = g.nbr[1] = g.nbr[2] = g.nbr[3] = -1;
+        }
+        g.tri = t; g.pad = 0;
+        sgeom[sl] = g;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(FULL, cnt, o);
+    __threadfence_block();
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic accesses of this block vs. the async writes
+    __syncwarp();
+    if (lane == 0) mbar_expect_tx(mbar, (unsigned)(cnt * C::SLOT_DOUBLES * sizeof(double)));
+    __syncwarp();
+    for (int sl = lane; sl < ns; sl += 32) {
+        int t = pslots[sl];
+        if (t >= 0)
+            tma_bulk_g2s(coef + (size_t)sl * C::SLOT_DOUBLES, tb.coef + (long long)t * tb.tri_stride + (long long)k0 * PLANE_STRIDE,
+                         (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
+    }
+}
+
 template <class C>
 __global__ void __launch_bounds__(C::NTHREADS, 1)
 k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, RetireQueue rq, double dt, int* __restrict__ work_counter) {
     extern __shared__ __align__(128) unsigned char smem[];
-    double* coef = reinterpret_cast<double*>(smem + C::OFF_COEF);
-    SlotGeom* sgeom = reinterpret_cast<SlotGeom*>(smem + C::OFF_GEOM);
-    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + C::OFF_MISC);
-    int* sh_sc = reinterpret_cast<int*>(smem + C::OFF_MISC + 16);
-    int* sh_next = reinterpret_cast<int*>(smem + C::OFF_MISC + 20);
-
-    const int tid = threadIdx.x, lane = tid & 31;
-    if (tid == 0) { mbar_init(mbar, 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-    unsigned phase = 0;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    BlockCtrl* ctl_all = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL);
+    unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF);
+    if (tid == 0) {
+        for (int b = 0; b < C::NBUF; ++b) mbar_init(mbar_all + 2 * b, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (wid == 0) {
+        for (int b = 0; b < C::NBUF; ++b) tile_refill<C>(smem, b, tb, tt, work_counter, lane);
+    }
     const int P = tb.tor.P;
     const double h2 = 0.5 * dt, h6 = dt / 6.0;
     constexpr unsigned FULL = 0xffffffffu;
 
-    for (;;) {
-        __syncthreads();   // previous super-cell fully consumed (coefficients, geometry, sh_sc, sh_next)
-        if (tid == 0) *sh_sc = atomicAdd(work_counter, 1);
-        __syncthreads();
-        const int sc = *sh_sc;
-        if (sc >= tt.nsc) break;
-        const int begin = tt.offs[(long long)sc * C::CPS], end = tt.offs[(long long)(sc + 1) * C::CPS];
-        if (begin == end) continue;
-        const int patch = sc / tt.nwin, k0 = (sc - patch * tt.nwin) * C::WK;
-        const int ns = tt.nslots[patch];
-        const int* pslots = tt.slots + (long long)patch * C::SMAX;
-        // ---- stage geometry (generic stores) and coefficient blocks (TMA bulk copies)
-        if (tid == 0) *sh_next = begin;
-        if (tid < ns) {
-            int t = pslots[tid];
-            SlotGeom g;
-            if (t >= 0) {
-                const TriGeom tg = tb.geom[t];
-                g.v0x = tg.v0x; g.v0y = tg.v0y; g.a11 = tg.a11; g.a12 = tg.a12; g.a21 = tg.a21; g.a22 = tg.a22;
-                const short* nb = tt.nbr + ((long long)patch * C::SMAX + tid) * 4;
-                g.nbr[0] = nb[0]; g.nbr[1] = nb[1]; g.nbr[2] = nb[2]; g.nbr[3] = -1;
-            } else {
-                g.v0x = g.v0y = 1e300; g.a11 = g.a12 = g.a21 = g.a22 = 0.0; g.nbr[0] = g.nbr[1] = g.nbr[2] = g.nbr[3] = -1;
-            }
-            g.tri = t; g.pad = 0;
-            sgeom[tid] = g;
-        }
-        if (tid < 32) {
-            int cnt = 0;
-            for (int sl = tid; sl < ns; sl += 32) cnt += pslots[sl] >= 0;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(FULL, cnt, o);
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the block vs. the async writes
-            if (tid == 0) mbar_expect_tx(mbar, (unsigned)(cnt * C::SLOT_DOUBLES * sizeof(double)));
-            __syncwarp();
-            for (int sl = tid; sl < ns; sl += 32) {
-                int t = pslots[sl];
-                if (t >= 0)
-                    tma_bulk_g2s(coef + (size_t)sl * C::SLOT_DOUBLES, tb.coef + (long long)t * tb.tri_stride + (long long)k0 * PLANE_STRIDE,
-                                 (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
-            }
-        }
-        mbar_wait(mbar, phase);
-        phase ^= 1;
-        __syncthreads();
+    // every warp walks the ring in the same order; the last warp to leave an entry refills it (no block-wide barrier)
+    for (unsigned it = 0;; ++it) {
+        const int b = it % C::NBUF;
+        mbar_wait(mbar_all + 2 * b, (it / C::NBUF) & 1);
+        BlockCtrl* ctl = ctl_all + b;
+        if (ctl->sc < 0) break;
+        const double* coef = reinterpret_cast<const double*>(smem + C::BLOCK_BYTES * b);
+        const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
+        const int end = ctl->end, patch = ctl->patch, k0 = ctl->k0, ns = ctl->ns;
+        int* sh_next = &ctl->next;
 
         // ---- each warp grabs chunks of 32 markers until the super-cell is drained
         for (;;) {
@@ -413,6 +436,12 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, R
                 s.status[m] = st;
             }
         }
+        // leave the entry; the last warp out refills it with the next super-cell
+        __syncwarp();
+        int last = 0;
+        if (lane == 0) { __threadfence_block(); last = atomicAdd(&ctl->left, 1) == C::NWARPS - 1; }
+        last = __shfl_sync(FULL, last, 0);
+        if (last) { __threadfence_block(); tile_refill<C>(smem, b, tb, tt, work_counter, lane); }
     }
 }
 

@@ -36,16 +36,18 @@ struct TileCfg {
     static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD, NWARPS = NWARPS_, NTHREADS = 32 * NWARPS_;
     static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
     static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
-    static constexpr int NBINS = SMAX * NW;          // (slot, local interval) cells of the staged block
     static constexpr int CPS = TP * WK;              // cells per super-cell
     static constexpr int SLOT_DOUBLES = NPL * PLANE_STRIDE;
-    // shared memory carve-up (bytes)
-    static constexpr size_t OFF_COEF = 0;
-    static constexpr size_t OFF_GEOM = OFF_COEF + sizeof(double) * SMAX * SLOT_DOUBLES;
-    static constexpr size_t OFF_WARP = OFF_GEOM + 64 * SMAX;
-    static constexpr size_t WARP_BYTES = 0;
-    static constexpr size_t OFF_MISC = OFF_WARP + WARP_BYTES * NWARPS;
-    static constexpr size_t BYTES = OFF_MISC + 64;
+    static constexpr int NBUF = 2;                   // ring of staged blocks
+    // shared memory carve-up (bytes): NBUF x { coefficients, slot geometry }, then the control words
+    static constexpr size_t COEF_BYTES = sizeof(double) * SMAX * SLOT_DOUBLES;
+    static constexpr size_t BLOCK_BYTES = COEF_BYTES + 64 * SMAX;
+    static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;
+    static constexpr size_t BYTES = OFF_CTRL + 64 * NBUF + 16 * NBUF;
+};
+struct BlockCtrl {   // 64 B per ring entry
+    int sc, begin, end, next, left, ns, patch, k0;
+    int pad[8];
 };
 
 struct __align__(16) SlotGeom {   // 64 B
