@@ -32,6 +32,7 @@ UNIT = "marker-pushes/s"
 FLOP_PER_PUSH = 3772.0          # 943 flop per RK stage x 4
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
 KEYS = ("R", "Z", "phi", "u", "w", "mu", "p")
+TRAFFIC_BYTES_PER_LAUNCH = None   # dram__bytes_read.sum + dram__bytes_write.sum of k_push_tiled from the last ncu --set full capture (profiles/)
 SORT_EVERY = 1                  # tiled kernel: re-bin every step (BASELINE configs[2] uses 10)
 
 
@@ -200,15 +201,16 @@ def main():
     if rank == 0:
         sampler.start()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    launches, sorted_steps, slow = 0, [], 0
+    launches, slow, retired, kms = 0, 0, 0, []
     ev[0].record()
     for s in range(args.steps):
         g.push_rk4(cfg.dt, 1)
         ev[s + 1].record()
-        st = g.push_stats()
+        st = g.push_stats()          # reads device counters: synchronises the stream after the step's last kernel
+        kms.append(g.push_kernel_ms())   # CUDA events recorded by the library on its stream around each kernel group
         launches += st["launches"]
         slow += st["slow_path"]
-        sorted_steps.append(st["sorts"] > 0)
+        retired += st["retired"]
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -217,9 +219,14 @@ def main():
     step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
     total_s = shard.reduce_max_seconds(sum(step_ms) * 1e-3, dist if world > 1 else None)
     value = shard.job_rate(n * args.steps, world, total_s)
-    kern_ms = [t for t, srt in zip(step_ms, sorted_steps) if not srt] or step_ms
-    kern_s = statistics.mean(kern_ms) * 1e-3
-    achieved = FLOP_PER_PUSH * n / kern_s / 1e12
+    # dominant kernel: the push kernel proper.  Algorithmic flops per launch = 943 flop x the marker-stage evaluations it
+    # performed (all 4 n minus those left to the follow-up kernel), over its own CUDA-event duration.
+    kern_s = statistics.mean(k["push"] for k in kms) * 1e-3
+    sort_ms = statistics.mean(k["sort"] for k in kms)
+    finish_ms = statistics.mean(k["finish"] for k in kms)
+    stage_evals = 4.0 * n - slow / args.steps
+    achieved = (FLOP_PER_PUSH / 4.0) * stage_evals / kern_s / 1e12
+    step_achieved = FLOP_PER_PUSH * n * args.steps / (sum(step_ms) * 1e-3) / 1e12
 
     # ---- end to end through the C-ABI with HOST buffers (pinned): H2D marker arrays, push, D2H result
     pinned_out = {k: torch.empty(n, dtype=torch.float64, pin_memory=True).numpy() for k in ("R", "Z", "phi", "u", "w")}
@@ -253,11 +260,15 @@ def main():
                         "note": "bind(HOST) includes the first sort by cell; PCIe-bound"},
                 "gpu_launches": launches,
                 "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
-                             "traffic": None, "kernel": "k_push_tiled" if args.variant == 0 else "k_push_simple", "kernel_ms": 1e3 * kern_s,
-                             "flop_per_push": FLOP_PER_PUSH, "peak_kind": "nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (derived, DESIGN.md)",
+                             "traffic": TRAFFIC_BYTES_PER_LAUNCH if (args.variant == 0 and args.config == 3 and n == cfg.n_markers) else None,
+                             "kernel": "k_push_tiled" if args.variant == 0 else "k_push_simple", "kernel_ms": 1e3 * kern_s,
+                             "flop_per_push": FLOP_PER_PUSH, "stage_evals_per_launch": stage_evals,
+                             "peak_kind": "nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (derived, DESIGN.md)",
                              "measured_dfma_tflops": dfma, "frac_of_measured_dfma": achieved / dfma,
+                             "whole_step_frac": step_achieved / FP64_PEAK_TFLOPS,
                              "hbm_algorithmic_GBps": 121.0 * n / kern_s / 1e9},
-                "slow_path_evals": slow, "e2e_checksum": checksum}
+                "step_breakdown_ms": {"sort": sort_ms, "push": 1e3 * kern_s, "finish": finish_ms},
+                "slow_path_evals": slow, "retired_markers": retired, "e2e_checksum": checksum}
         if not args.no_cpu_baseline:
             cpu_n = min(n, args.cpu_sample)
             v, cores, secs = time_oracle(cfg, cpu_n, 4)

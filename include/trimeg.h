@@ -114,7 +114,9 @@ int trimeg_markers_get(trimeg_ctx* ctx, double* R, double* Z, double* phi, doubl
                        int memspace);
 
 /* Re-sort the marker store by cell (triangle x toroidal interval) now / every n-th RK4 step (0 = never again;
- * a sort is always done once after bind before the first push). */
+ * a sort is always done once after bind before the first push).  Inside trimeg_push_rk4 the sort is fused into
+ * the push: every step that precedes a re-sort also writes each marker's new cell key and the cell histogram,
+ * the sort proper only builds the permutation, and the next push step reads the markers through it. */
 int trimeg_sort(trimeg_ctx* ctx);
 int trimeg_set_sort_interval(trimeg_ctx* ctx, int32_t every_n_steps);
 
@@ -136,8 +138,14 @@ int trimeg_set_push_variant(trimeg_ctx* ctx, int32_t variant);
  * (a register-only DFMA loop; the roofline's measured "alu" peak). */
 int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops);
 /* Counters of the last trimeg_push_rk4 call: [0] kernel launches, [1] marker-stage evaluations that took the
- * slow (out-of-tile) gather path, [2] markers flagged lost, [3] sorts done. */
+ * slow (out-of-tile) gather path in the follow-up kernel, [2] markers that left their staged tile during a step
+ * (summed over steps), [3] sorts done. */
 int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]);
+/* Device time (CUDA events on the context's stream; blocks until they have completed) of the last RK4 step of the
+ * last trimeg_push_rk4 call, in milliseconds: [0] sort kernels of that step (keys, scan, permutation; 0 if it did
+ * not re-sort), [1] the push kernel proper (the roofline's "dominant kernel"), [2] the follow-up kernels (markers
+ * that left their staged tile, markers outside the mesh).  Errors: BAD_ARG, BAD_STATE (nothing pushed yet), CUDA. */
+int trimeg_push_kernel_ms(trimeg_ctx* ctx, double out[3]);
 
 #ifdef __cplusplus
 }

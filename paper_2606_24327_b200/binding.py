@@ -20,7 +20,7 @@ EXPORTS = [
     "trimeg_create", "trimeg_destroy", "trimeg_sync", "trimeg_last_error", "trimeg_equilibrium_set",
     "trimeg_species_set", "trimeg_mesh_load", "trimeg_fields_set", "trimeg_gather", "trimeg_scratch_bytes",
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
-    "trimeg_rhs", "trimeg_set_push_variant", "trimeg_bench_dfma", "trimeg_push_stats",
+    "trimeg_rhs", "trimeg_set_push_variant", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
 ]
 
 
@@ -77,6 +77,7 @@ def load_library():
     lib.trimeg_set_push_variant.argtypes = [vp, i32]
     lib.trimeg_bench_dfma.argtypes = [vp, C.POINTER(dbl)]
     lib.trimeg_push_stats.argtypes = [vp, C.POINTER(i64)]
+    lib.trimeg_push_kernel_ms.argtypes = [vp, C.POINTER(dbl)]
     _lib = lib
     return lib
 
@@ -244,4 +245,9 @@ class Trimeg:
     def push_stats(self):
         a = (C.c_int64 * 4)()
         self._ck(self._lib.trimeg_push_stats(self._h, a), "trimeg_push_stats")
-        return dict(launches=a[0], slow_path=a[1], lost=a[2], sorts=a[3])
+        return dict(launches=a[0], slow_path=a[1], retired=a[2], sorts=a[3])
+
+    def push_kernel_ms(self):
+        a = (C.c_double * 3)()
+        self._ck(self._lib.trimeg_push_kernel_ms(self._h, a), "trimeg_push_kernel_ms")
+        return dict(sort=a[0], push=a[1], finish=a[2])

@@ -182,13 +182,53 @@ __global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, Sp
 }
 
 
+// queues of retired markers, one per RK stage at which the marker left the staged block (so that the finish kernel's
+// remaining-stage loop is warp-uniform); SoA with capacity cap per sub-queue, entry e = stage * cap + slot
+struct RetireQueue {
+    double* y;      // [5][4 cap] stage position
+    double* acc;    // [5][4 cap] weighted sum of the k's so far
+    int* m;         // [4 cap] marker index (position in the destination store)
+    int* st;        // [4 cap] status so far
+    int* count;     // [4] device counters
+    int cap;
+};
+// where the sort key of the updated marker goes (the next step's counting sort is fused into the push)
+struct KeyOut {
+    int* keys;      // [n] cell of the updated position, indexed like the destination store
+    int* hist;      // [ncell + 2] histogram of the keys
+    int ncell;
+    int enabled;
+};
+__device__ __forceinline__ double wrap_phi(const TorP& tp, double phi) {
+    double ph = fma(-tp.period, floor(phi * tp.inv_period), phi);
+    if (ph < 0.0) ph += tp.period;
+    if (ph >= tp.period) ph -= tp.period;
+    return ph;
+}
+// final store of one marker: state, triangle of the updated position, status, and (if enabled) its sort key
+__device__ __forceinline__ void store_marker(const DevTables& tb, const CellMap& cm, const KeyOut& ko, const MarkerSoA& d, long long j, const double y[5],
+                                             double ph, int t, int st) {
+    d.R[j] = y[0]; d.Z[j] = y[1]; d.phi[j] = ph; d.u[j] = y[3]; d.w[j] = y[4];
+    d.tri[j] = t; d.status[j] = st;
+    if (ko.enabled) {
+        double sf;
+        int k = toroidal_interval(tb.tor, ph, sf);
+        int key = t < 0 ? ko.ncell : cm.cell(t, k);
+        ko.keys[j] = key;
+        atomicAdd(ko.hist + key, 1);
+    }
+}
+
 // markers outside the mesh (sorted behind the last cell): same arithmetic through the simple path
-__global__ void __launch_bounds__(128) k_push_lost(DevTables tb, EquilP ep, SpeciesP sp, MarkerSoA s, const int* __restrict__ first, long long n, double dt) {
+__global__ void __launch_bounds__(128) k_push_lost(DevTables tb, EquilP ep, SpeciesP sp, MarkerSoA src, MarkerSoA dst, const int* __restrict__ perm,
+                                                   KeyOut ko, CellMap cm, const int* __restrict__ first, long long n, double dt) {
     long long m0 = *first;
     for (long long m = m0 + (long long)blockIdx.x * blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
-        double y0[5] = {s.R[m], s.Z[m], s.phi[m], s.u[m], s.w[m]};
-        double mu = s.mu[m], p = s.p[m];
-        int t = s.tri[m], st = s.status[m];
+        const long long ms = perm ? (long long)perm[m] : m;
+        double y0[5] = {src.R[ms], src.Z[ms], src.phi[ms], src.u[ms], src.w[ms]};
+        double mu = src.mu[ms], p = src.p[ms];
+        int t = src.tri[ms], st = src.status[ms];
+        if (perm) { dst.mu[m] = mu; dst.p[m] = p; dst.id[m] = src.id[ms]; }
         double k[5], acc[5], y[5];
         st |= stage_simple(tb, ep, sp, t, y0[0], y0[1], y0[2], y0[3], y0[4], mu, p, k);
 #pragma unroll
@@ -203,12 +243,9 @@ __global__ void __launch_bounds__(128) k_push_lost(DevTables tb, EquilP ep, Spec
         const double h6 = dt / 6.0;
 #pragma unroll
         for (int q = 0; q < 5; ++q) y[q] = fma(h6, acc[q] + k[q], y0[q]);
-        double ph = fma(-tb.tor.period, floor(y[2] * tb.tor.inv_period), y[2]);
-        if (ph < 0.0) ph += tb.tor.period;
-        if (ph >= tb.tor.period) ph -= tb.tor.period;
-        s.R[m] = y[0]; s.Z[m] = y[1]; s.phi[m] = ph; s.u[m] = y[3]; s.w[m] = y[4];
-        s.tri[m] = t;
-        s.status[m] = st;
+        const double ph = wrap_phi(tb.tor, y[2]);
+        t = locate_walk(tb.bg, tb.geom, t, y[0], y[1]);
+        store_marker(tb, cm, ko, dst, m, y, ph, t, st);
     }
 }
 
@@ -225,16 +262,6 @@ __global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP s
 
 
 // ============================================================================================ tiled push (variant 0)
-// queue of retired markers (lives in the inactive marker buffer): SoA with capacity cap
-struct RetireQueue {
-    double* y;      // [5][cap] stage position
-    double* acc;    // [5][cap] weighted sum of the k's so far
-    int* m;         // [cap] marker index
-    int* info;      // [cap] stage | status << 8
-    int* count;     // device counter
-    int cap;
-};
-
 // (re)fill ring entry b with the next non-empty super-cell; executed by one whole warp.  The entry's mbarrier completes
 // when the TMA bytes have landed (or at once, with sc = -1, when the work list is exhausted).
 template <class C>
@@ -291,9 +318,30 @@ __device__ __forceinline__ void tile_refill(unsigned char* smem, int b, const De
     }
 }
 
+// slot-space edge walk inside the staged block: returns the slot containing (R, Z) or -1 (left the staged set / hop cap)
+__device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int sl, double R, double Z, double& xi, double& eta) {
+    if (sl < 0) return -1;
+    for (int hop = 0; hop < 16; ++hop) {
+        const SlotGeom& g = sgeom[sl];
+        double dx = R - g.v0x, dy = Z - g.v0y;
+        xi = fma(g.a11, dx, g.a12 * dy);
+        eta = fma(g.a21, dx, g.a22 * dy);
+        double l0 = 1.0 - xi - eta;
+        if (fmin(fmin(xi, eta), l0) >= INSIDE_TOL) return sl;
+        int e = (eta <= xi && eta <= l0) ? 0 : ((l0 <= xi) ? 1 : 2);
+        sl = g.nbr[e];
+        if (sl < 0) return -1;
+    }
+    return -1;
+}
+
+// One RK4 step for the markers of one super-cell after another.  Markers are read from `src` through the sort
+// permutation (perm[j] = position in src of the marker that belongs at position j of the cell-sorted order; null =
+// src is already in that order and src == dst) and written to dst[j]: the sort's data movement is fused into the push.
 template <class C>
 __global__ void __launch_bounds__(C::NTHREADS, 1)
-k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, RetireQueue rq, double dt, int* __restrict__ work_counter) {
+k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA src, MarkerSoA dst, const int* __restrict__ perm, RetireQueue rq,
+             KeyOut ko, CellMap cm, double dt, int* __restrict__ work_counter) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     BlockCtrl* ctl_all = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL);
@@ -328,19 +376,20 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, R
             chunk = __shfl_sync(FULL, chunk, 0);
             if (chunk >= end) break;
             const int m = chunk + lane;
-            bool alive = m < end;   // owner role: this lane still integrates a marker
+            bool alive = m < end;   // this lane still integrates a marker
             double y0[5], y[5], acc[5], mu = 0.0, pw = 0.0;
-            int st = 0, home = -1, cur = -1, tri_last = -1;
+            int st = 0, cur = -1, tri_last = -1;
             if (alive) {
-                y0[0] = s.R[m]; y0[1] = s.Z[m]; y0[2] = s.phi[m]; y0[3] = s.u[m]; y0[4] = s.w[m];
-                mu = s.mu[m]; pw = s.p[m]; st = s.status[m];
-                tri_last = s.tri[m];
+                const long long ms = perm ? (long long)perm[m] : (long long)m;
+                y0[0] = src.R[ms]; y0[1] = src.Z[ms]; y0[2] = src.phi[ms]; y0[3] = src.u[ms]; y0[4] = src.w[ms];
+                mu = src.mu[ms]; pw = src.p[ms]; st = src.status[ms];
+                tri_last = src.tri[ms];
+                if (perm) { dst.mu[m] = mu; dst.p[m] = pw; dst.id[m] = src.id[ms]; }
                 int sl = tri_last - patch * C::TP;
-                if (sl >= 0 && sl < C::TP) home = sl;
+                if (sl >= 0 && sl < C::TP) cur = sl;
                 else {   // drifted since the last sort: look for the triangle in the halo
-                    for (int q = C::TP; q < ns; ++q) if (sgeom[q].tri == tri_last) { home = q; break; }
+                    for (int q = C::TP; q < ns; ++q) if (sgeom[q].tri == tri_last) { cur = q; break; }
                 }
-                cur = home;
             } else {
 #pragma unroll
                 for (int q = 0; q < 5; ++q) y0[q] = 0.0;
@@ -350,90 +399,61 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, R
 
 #pragma unroll 1
             for (int stage = 0; stage < 4; ++stage) {
-                // -- owner: locate in slot space, toroidal cell
-                int key = 0x7fffffff;
-                double ia = 0.0, ib = 0.0, ic = 0.0;
                 if (alive) {
-                    int sl = cur >= 0 ? cur : home;
-                    double xi = 0.0, eta = 0.0;
-                    if (sl >= 0) {
-                        int hop = 0;
-                        for (; hop < 16; ++hop) {
-                            const SlotGeom& g = sgeom[sl];
-                            double dx = y[0] - g.v0x, dy = y[1] - g.v0y;
-                            xi = fma(g.a11, dx, g.a12 * dy);
-                            eta = fma(g.a21, dx, g.a22 * dy);
-                            double l0 = 1.0 - xi - eta;
-                            if (fmin(fmin(xi, eta), l0) >= INSIDE_TOL) break;
-                            int e = (eta <= xi && eta <= l0) ? 0 : ((l0 <= xi) ? 1 : 2);
-                            sl = g.nbr[e];
-                            if (sl < 0) break;
-                        }
-                        if (hop == 16) sl = -1;
-                    }
-                    double sf;
+                    double xi = 0.0, eta = 0.0, sf;
+                    int sl = slot_walk(sgeom, cur, y[0], y[1], xi, eta);
                     int k = toroidal_interval(tb.tor, y[2], sf);
                     int dk = k - k0;
                     if (dk > P / 2) dk -= P; else if (dk < -(P / 2)) dk += P;
                     int lk = dk + C::HK;
-                    if (sl >= 0 && lk >= 0 && lk < C::NW) {
+                    bool in_tile = sl >= 0 && lk >= 0 && lk < C::NW;
+                    double d[5];
+                    if (in_tile) {
+                        // -- gather from the staged block (each lane its own marker)
                         cur = sl;
-                        key = ((sl * C::NW + lk) << 5) | lane;
-                        ia = xi; ib = eta; ic = sf;
-                        tri_last = sgeom[sl].tri;
+                        const SlotGeom& g = sgeom[sl];
+                        tri_last = g.tri;
+                        double w[4], dw[4], g8[8];
+                        bspline_from_s(tb.tor, sf, w, dw);
+                        LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
+                        gather_cell(ld, xi, eta, w, dw, g8);
+                        Fields fo;
+                        fo.P = g8[0]; fo.PR = fma(g.a11, g8[1], g.a21 * g8[2]); fo.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); fo.Pp = g8[3];
+                        fo.A = g8[4]; fo.AR = fma(g.a11, g8[5], g.a21 * g8[6]); fo.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); fo.Ap = g8[7];
+                        rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, fo, d);
                     } else {
                         // left the staged block: retire (the follow-up kernel finishes this step from here)
-                        int slot = atomicAdd(rq.count, 1);
+                        int slot = atomicAdd(rq.count + stage, 1);
                         if (slot < rq.cap) {
+                            const size_t e = (size_t)stage * rq.cap + slot, tot = 4 * (size_t)rq.cap;
 #pragma unroll
-                            for (int q = 0; q < 5; ++q) { rq.y[(size_t)q * rq.cap + slot] = y[q]; rq.acc[(size_t)q * rq.cap + slot] = acc[q]; }
-                            rq.m[slot] = m;
-                            rq.info[slot] = stage | (st << 8);
+                            for (int q = 0; q < 5; ++q) { rq.y[q * tot + e] = y[q]; rq.acc[q * tot + e] = acc[q]; }
+                            rq.m[e] = m;
+                            rq.st[e] = st;
                             alive = false;
                         } else {   // queue full (pathological): evaluate in place through the global tables
                             int t = tri_last;
-                            double d[5];
                             st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, pw, d);
                             if (t >= 0) tri_last = t;
-                            const double wgt = (stage == 0 || stage == 3) ? 1.0 : 2.0;
-                            const double hs = stage == 2 ? dt : h2;
-#pragma unroll
-                            for (int q = 0; q < 5; ++q) { acc[q] = fma(wgt, d[q], acc[q]); y[q] = fma(hs, d[q], y0[q]); }
-                            key = 0x7ffffffe;   // participates in the exchange as a no-op
                         }
                     }
-                }
-                // -- gather from the staged block (each lane its own marker: regrouping the lanes of a warp by cell was
-                //    measured to buy nothing, LDS.128 costs 4 wavefronts unless every aligned lane pair shares an address)
-                if (alive && key < 0x7ffffffe) {
-                    const int bin = key >> 5;
-                    const int sl = bin / C::NW, lk = bin - sl * C::NW;
-                    double w[4], dw[4], g8[8];
-                    bspline_from_s(tb.tor, ic, w, dw);
-                    LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
-                    gather_cell(ld, ia, ib, w, dw, g8);
-                    const SlotGeom& g = sgeom[sl];
-                    Fields fo;
-                    fo.P = g8[0]; fo.PR = fma(g.a11, g8[1], g.a21 * g8[2]); fo.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); fo.Pp = g8[3];
-                    fo.A = g8[4]; fo.AR = fma(g.a11, g8[5], g.a21 * g8[6]); fo.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); fo.Ap = g8[7];
-                    // -- equilibrium, equations of motion, RK4 bookkeeping
-                    double d[5];
-                    rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, fo, d);
-                    const double wgt = (stage == 0 || stage == 3) ? 1.0 : 2.0;
-                    const double hs = stage == 2 ? dt : h2;
+                    if (alive) {
+                        const double wgt = (stage == 0 || stage == 3) ? 1.0 : 2.0;
+                        const double hs = stage == 2 ? dt : h2;
 #pragma unroll
-                    for (int q = 0; q < 5; ++q) { acc[q] = fma(wgt, d[q], acc[q]); y[q] = fma(hs, d[q], y0[q]); }
+                        for (int q = 0; q < 5; ++q) { acc[q] = fma(wgt, d[q], acc[q]); y[q] = fma(hs, d[q], y0[q]); }
+                    }
                 }
             }
             if (alive) {
 #pragma unroll
                 for (int q = 0; q < 5; ++q) y[q] = fma(h6, acc[q], y0[q]);
-                double ph = fma(-tb.tor.period, floor(y[2] * tb.tor.inv_period), y[2]);
-                if (ph < 0.0) ph += tb.tor.period;
-                if (ph >= tb.tor.period) ph -= tb.tor.period;
-                s.R[m] = y[0]; s.Z[m] = y[1]; s.phi[m] = ph; s.u[m] = y[3]; s.w[m] = y[4];
-                s.tri[m] = tri_last;
-                s.status[m] = st;
+                const double ph = wrap_phi(tb.tor, y[2]);
+                // triangle of the updated position: staged walk, else the global walk (rare)
+                double xi, eta;
+                int sl = slot_walk(sgeom, cur, y[0], y[1], xi, eta);
+                int t = sl >= 0 ? sgeom[sl].tri : locate_walk(tb.bg, tb.geom, tri_last, y[0], y[1]);
+                store_marker(tb, cm, ko, dst, m, y, ph, t, st);
             }
         }
         // leave the entry; the last warp out refills it with the next super-cell
@@ -445,33 +465,42 @@ k_push_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, MarkerSoA s, R
     }
 }
 
-// finish the step of the retired markers through the global tables (same arithmetic as the simple path)
-__global__ void __launch_bounds__(128) k_push_finish(DevTables tb, EquilP ep, SpeciesP sp, MarkerSoA s, RetireQueue rq, double dt) {
-    const int count = min(*rq.count, rq.cap);
+// finish the step of the retired markers through the global tables (same arithmetic as the simple path).
+// Sub-queue q holds the markers that left at stage q; each is padded to whole warps so that the stage loop is warp-uniform.
+__global__ void __launch_bounds__(128) k_push_finish(DevTables tb, EquilP ep, SpeciesP sp, MarkerSoA src, MarkerSoA dst, const int* __restrict__ perm,
+                                                     RetireQueue rq, KeyOut ko, CellMap cm, double dt) {
+    int cnt[4], start[5];
+    start[0] = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { cnt[q] = min(rq.count[q], rq.cap); start[q + 1] = start[q] + ((cnt[q] + 31) & ~31); }
     const double h2 = 0.5 * dt, h6 = dt / 6.0;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < count; i += gridDim.x * blockDim.x) {
-        const int m = rq.m[i], info = rq.info[i];
-        int st = info >> 8, t = s.tri[m];
-        double y0[5] = {s.R[m], s.Z[m], s.phi[m], s.u[m], s.w[m]};
-        const double mu = s.mu[m], p = s.p[m];
+    const size_t tot = 4 * (size_t)rq.cap;
+    for (int v = blockIdx.x * blockDim.x + threadIdx.x; v < start[4]; v += gridDim.x * blockDim.x) {
+        const int q = v >= start[3] ? 3 : (v >= start[2] ? 2 : (v >= start[1] ? 1 : 0));
+        const int i = v - start[q];
+        if (i >= cnt[q]) continue;
+        const size_t e = (size_t)q * rq.cap + i;
+        const int m = rq.m[e];
+        int st = rq.st[e];
+        const long long ms = perm ? (long long)perm[m] : (long long)m;
+        int t = src.tri[ms];
+        double y0[5] = {src.R[ms], src.Z[ms], src.phi[ms], src.u[ms], src.w[ms]};
+        const double mu = src.mu[ms], p = src.p[ms];
         double y[5], acc[5], d[5];
 #pragma unroll
-        for (int q = 0; q < 5; ++q) { y[q] = rq.y[(size_t)q * rq.cap + i]; acc[q] = rq.acc[(size_t)q * rq.cap + i]; }
-        for (int stage = info & 0xff; stage < 4; ++stage) {
+        for (int c = 0; c < 5; ++c) { y[c] = rq.y[c * tot + e]; acc[c] = rq.acc[c * tot + e]; }
+        for (int stage = q; stage < 4; ++stage) {
             st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, d);
             const double wgt = (stage == 0 || stage == 3) ? 1.0 : 2.0;
             const double hs = stage == 2 ? dt : h2;
 #pragma unroll
-            for (int q = 0; q < 5; ++q) { acc[q] = fma(wgt, d[q], acc[q]); y[q] = fma(hs, d[q], y0[q]); }
+            for (int c = 0; c < 5; ++c) { acc[c] = fma(wgt, d[c], acc[c]); y[c] = fma(hs, d[c], y0[c]); }
         }
 #pragma unroll
-        for (int q = 0; q < 5; ++q) y[q] = fma(h6, acc[q], y0[q]);
-        double ph = fma(-tb.tor.period, floor(y[2] * tb.tor.inv_period), y[2]);
-        if (ph < 0.0) ph += tb.tor.period;
-        if (ph >= tb.tor.period) ph -= tb.tor.period;
-        s.R[m] = y[0]; s.Z[m] = y[1]; s.phi[m] = ph; s.u[m] = y[3]; s.w[m] = y[4];
-        if (t >= 0) s.tri[m] = t;
-        s.status[m] = st;
+        for (int c = 0; c < 5; ++c) y[c] = fma(h6, acc[c], y0[c]);
+        const double ph = wrap_phi(tb.tor, y[2]);
+        t = locate_walk(tb.bg, tb.geom, t, y[0], y[1]);
+        store_marker(tb, cm, ko, dst, m, y, ph, t, st);
     }
 }
 
@@ -577,7 +606,12 @@ __global__ void __launch_bounds__(256) k_sort_gather(MarkerSoA a, MarkerSoA b, l
     b.R[j] = a.R[m]; b.Z[j] = a.Z[m]; b.phi[j] = a.phi[m]; b.u[j] = a.u[m]; b.w[j] = a.w[m];
     b.mu[j] = a.mu[m]; b.p[j] = a.p[m]; b.tri[j] = a.tri[m]; b.status[j] = a.status[m]; b.id[j] = a.id[m];
 }
-__global__ void k_accumulate_stat(const int* __restrict__ v, unsigned long long* __restrict__ acc) { *acc += (unsigned long long)*v; }
+// per step: acc[0] += marker-stage evaluations left to the follow-up kernel, acc[1] += markers retired (4 threads, one per sub-queue)
+__global__ void k_accumulate_stat(const int* __restrict__ v, int cap, unsigned long long* __restrict__ acc) {
+    unsigned long long c = (unsigned long long)min(v[threadIdx.x], cap);
+    atomicAdd(acc, c * (4 - threadIdx.x));
+    atomicAdd(acc + 1, c);
+}
 
 // ============================================================================================ DFMA micro-benchmark
 __global__ void __launch_bounds__(512) k_dfma(double* out, int iters, double a, double b) {
@@ -615,7 +649,13 @@ struct trimeg_ctx {
     int *d_hist = nullptr, *d_offs = nullptr, *d_fill = nullptr, *d_sums = nullptr;   // library-owned, [T*P+2]
     long long ncell = 0;
     bool sorted = false;
+    bool keys_valid = false;    // d_keys / d_hist describe the current store (written by the last push step)
     int sort_every = 0;
+    // retire queues (in scratch)
+    RetireQueue rq{};
+    // per-kernel timing of the last step of trimeg_push_rk4 (events on the context's stream)
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
     long long steps_since_sort = 0;
     int variant = 0;
     long long stats[4] = {0, 0, 0, 0};
@@ -682,6 +722,7 @@ int trimeg_create(trimeg_ctx** out, int device, void* cuda_stream) {
         delete c;
         return TRIMEG_ERR_CUDA;
     }
+    for (auto& e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
     *out = c;
     return TRIMEG_OK;
 }
@@ -690,6 +731,7 @@ int trimeg_destroy(trimeg_ctx* ctx) {
     if (!ctx) return TRIMEG_ERR_BAD_ARG;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
+    for (auto& e : ctx->ev) if (e) cudaEventDestroy(e);
     free_mesh(ctx);
     delete ctx;
     return TRIMEG_OK;
@@ -741,7 +783,10 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     CU(cudaStreamSynchronize(ctx->stream));
     free_mesh(ctx);
     trimeg_host::HostMesh hm;
-    int rc = trimeg_host::build_mesh(n_nodes, RZ, n_tri, tri, hm);
+    // with the equilibrium known, number triangles along flux surfaces and shape the patch halos along the poloidal field
+    const double axis[2] = {ctx->eq_in.R0, 0.0};
+    const double* axis_p = ctx->have_eq ? axis : nullptr;
+    int rc = trimeg_host::build_mesh(n_nodes, RZ, n_tri, tri, axis_p, hm);
     if (rc) return fail(ctx, TRIMEG_ERR_BAD_MESH, "mesh_load: vertex index out of range, non-finite node, clockwise/degenerate triangle or non-manifold edge");
     trimeg_host::ElementConsts ec;
     trimeg_host::element_consts(ec);
@@ -764,7 +809,7 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     const long long tri_stride = (long long)(n_planes + 3 + 2 * PLANE_PAD) * PLANE_STRIDE;
     const size_t coef_bytes = (size_t)T * tri_stride * sizeof(double);
     trimeg_host::HostPatches hp;
-    trimeg_host::build_patches(hm, RZ, n_nodes, T, Tile::TP, Tile::SMAX, hp);
+    trimeg_host::build_patches(hm, RZ, n_nodes, T, Tile::TP, Tile::SMAX, axis_p, 3.0, hp);
     const int nwin = (n_planes + Tile::WK - 1) / Tile::WK;
     ctx->cm.P = n_planes; ctx->cm.nwin = nwin;
     ctx->ncell = (long long)hp.npatch * nwin * Tile::CPS;
@@ -786,7 +831,7 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     CU(cudaMalloc(&ctx->d_pslots, sizeof(int) * hp.slots.size()));
     CU(cudaMalloc(&ctx->d_pnslots, sizeof(int) * hp.nslots.size()));
     CU(cudaMalloc(&ctx->d_pnbr, sizeof(short) * hp.nbr.size()));
-    CU(cudaMalloc(&ctx->d_work, sizeof(int) * 4));
+    CU(cudaMalloc(&ctx->d_work, sizeof(int) * 8));
     CU(cudaMalloc(&ctx->d_stats, sizeof(unsigned long long) * 4));
     CU(cudaMemcpyAsync(ctx->d_pslots, hp.slots.data(), sizeof(int) * hp.slots.size(), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_pnslots, hp.nslots.data(), sizeof(int) * hp.nslots.size(), cudaMemcpyHostToDevice, ctx->stream));
@@ -867,10 +912,13 @@ int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, 
 }
 
 // scratch layout: two MarkerSoA buffers (7 doubles + 3 ints per marker each) + keys
+// retire queues: four sub-queues of cap entries each (10 doubles + 2 ints per entry); cap = n/32 per stage (>= 1024)
+static int retire_cap(long long n) { return (int)std::max<long long>(1024, n / 32); }
+static size_t retire_bytes(int cap) { return align256((size_t)4 * cap * (10 * sizeof(double) + 2 * sizeof(int))); }
 static size_t soa_bytes(long long n) { return 7 * align256(sizeof(double) * (size_t)n) + 3 * align256(sizeof(int) * (size_t)n); }
 size_t trimeg_scratch_bytes(const trimeg_ctx* ctx, int64_t n) {
     if (!ctx || n <= 0) return 0;
-    return 2 * soa_bytes(n) + 2 * align256(sizeof(int) * (size_t)n) + 256;
+    return 2 * soa_bytes(n) + 2 * align256(sizeof(int) * (size_t)n) + retire_bytes(retire_cap(n)) + 256;
 }
 static void carve(MarkerSoA& s, char*& p, long long n) {
     double** dp[7] = {&s.R, &s.Z, &s.phi, &s.u, &s.w, &s.mu, &s.p};
@@ -879,15 +927,19 @@ static void carve(MarkerSoA& s, char*& p, long long n) {
     for (auto q : ip) { *q = (int*)p; p += align256(sizeof(int) * (size_t)n); }
 }
 
-static int do_sort(trimeg_ctx* ctx) {
-    const long long n = ctx->n;
-    const long long ncnt = ctx->ncell + 2;   // cells + lost bin + end sentinel
-    MarkerSoA& a = ctx->buf[ctx->cur];
-    MarkerSoA& b = ctx->buf[ctx->cur ^ 1];
+// counting sort by cell, in three parts: keys + histogram of the current store (skipped when the last push step
+// already produced them), offsets + permutation, and the data movement (fused into the tiled push, or k_sort_gather)
+static int sort_keys(trimeg_ctx* ctx) {
+    const long long n = ctx->n, ncnt = ctx->ncell + 2;   // cells + lost bin + end sentinel
     CU(cudaMemsetAsync(ctx->d_hist, 0, sizeof(int) * ncnt, ctx->stream));
-    CU(cudaMemsetAsync(ctx->d_fill, 0, sizeof(int) * ncnt, ctx->stream));
-    k_sort_keys<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, ctx->cm, (int)ctx->ncell, a, n, ctx->d_keys, ctx->d_hist);
+    k_sort_keys<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, ctx->cm, (int)ctx->ncell, ctx->buf[ctx->cur], n, ctx->d_keys, ctx->d_hist);
     KCHECK();
+    ctx->stats[0] += 1;
+    return TRIMEG_OK;
+}
+static int sort_perm(trimeg_ctx* ctx) {
+    const long long n = ctx->n, ncnt = ctx->ncell + 2;
+    CU(cudaMemsetAsync(ctx->d_fill, 0, sizeof(int) * ncnt, ctx->stream));
     int nb = (int)((ncnt + SCAN_CHUNK - 1) / SCAN_CHUNK);
     k_scan_reduce<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_hist, ncnt, ctx->d_sums);
     KCHECK();
@@ -897,13 +949,22 @@ static int do_sort(trimeg_ctx* ctx) {
     KCHECK();
     k_sort_perm<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(n, ctx->d_keys, ctx->d_offs, ctx->d_fill, ctx->d_perm);
     KCHECK();
-    k_sort_gather<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(a, b, n, ctx->d_perm);
+    ctx->stats[0] += 4;
+    ctx->stats[3] += 1;
+    return TRIMEG_OK;
+}
+static int do_sort(trimeg_ctx* ctx) {   // full sort with a separate gather pass
+    int rc = ctx->keys_valid ? TRIMEG_OK : sort_keys(ctx);
+    if (rc) return rc;
+    rc = sort_perm(ctx);
+    if (rc) return rc;
+    k_sort_gather<<<blocks_for(ctx->n, 256), 256, 0, ctx->stream>>>(ctx->buf[ctx->cur], ctx->buf[ctx->cur ^ 1], ctx->n, ctx->d_perm);
     KCHECK();
     ctx->cur ^= 1;
     ctx->sorted = true;
+    ctx->keys_valid = false;
     ctx->steps_since_sort = 0;
-    ctx->stats[0] += 6;
-    ctx->stats[3] += 1;
+    ctx->stats[0] += 1;
     return TRIMEG_OK;
 }
 
@@ -920,7 +981,15 @@ int trimeg_markers_bind(trimeg_ctx* ctx, int64_t n, const double* R, const doubl
     carve(ctx->buf[1], ptr, n);
     ctx->d_keys = (int*)ptr;
     ctx->d_perm = (int*)(ptr + align256(sizeof(int) * (size_t)n));
-    ctx->n = n; ctx->cur = 0; ctx->sorted = false; ctx->steps_since_sort = 0;
+    {
+        char* q = ptr + 2 * align256(sizeof(int) * (size_t)n);
+        RetireQueue& rq = ctx->rq;
+        rq.cap = retire_cap(n);
+        rq.y = (double*)q; rq.acc = rq.y + 5 * 4 * (size_t)rq.cap;
+        rq.m = (int*)(rq.acc + 5 * 4 * (size_t)rq.cap); rq.st = rq.m + 4 * (size_t)rq.cap;
+        rq.count = ctx->d_work + 4;
+    }
+    ctx->n = n; ctx->cur = 0; ctx->sorted = false; ctx->keys_valid = false; ctx->steps_since_sort = 0;
     if (memspace == TRIMEG_HOST) {   // stage through the second buffer
         MarkerSoA& b = ctx->buf[1];
         const double* src[7] = {R, Z, phi, u, w, mu, p};
@@ -988,37 +1057,72 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps) {
     ctx->stats[0] = ctx->stats[1] = ctx->stats[2] = ctx->stats[3] = 0;
     CU(cudaMemsetAsync(ctx->d_stats, 0, sizeof(unsigned long long) * 4, ctx->stream));
     const long long n = ctx->n;
+    ctx->ev_valid = false;
     for (int s = 0; s < nsteps; ++s) {
-        if (!ctx->sorted || (ctx->sort_every > 0 && ctx->steps_since_sort >= ctx->sort_every)) {
-            int rc = do_sort(ctx);
-            if (rc) return rc;
-        }
+        const bool need_sort = !ctx->sorted || (ctx->sort_every > 0 && ctx->steps_since_sort >= ctx->sort_every);
+        const bool timed = (s == nsteps - 1);
+        if (timed) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
         if (ctx->variant == 0 && ctx->tiled_ok) {
-            // retire queue lives in the inactive marker buffer (free between sorts)
-            MarkerSoA& spare = ctx->buf[ctx->cur ^ 1];
-            RetireQueue rq;
-            const size_t pool = (size_t)((char*)spare.tri - (char*)spare.R);   // the seven double arrays are contiguous
-            rq.cap = (int)std::min<size_t>((size_t)n, pool / (10 * sizeof(double) + 2 * sizeof(int)));
-            rq.y = spare.R; rq.acc = rq.y + 5 * (size_t)rq.cap;
-            rq.m = (int*)(rq.acc + 5 * (size_t)rq.cap); rq.info = rq.m + rq.cap;
-            rq.count = ctx->d_work + 1;
-            CU(cudaMemsetAsync(ctx->d_work, 0, 2 * sizeof(int), ctx->stream));
-            k_push_tiled<Tile><<<ctx->num_sms, Tile::NTHREADS, Tile::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, ctx->buf[ctx->cur], rq, dt, ctx->d_work);
+            // the sort only builds the permutation; the push reads the markers through it and writes the other buffer
+            const int* perm = nullptr;
+            if (need_sort) {
+                int rc = ctx->keys_valid ? TRIMEG_OK : sort_keys(ctx);
+                if (rc) return rc;
+                rc = sort_perm(ctx);
+                if (rc) return rc;
+                perm = ctx->d_perm;
+                ctx->sorted = true;
+                ctx->steps_since_sort = 0;
+            }
+            MarkerSoA& src = ctx->buf[ctx->cur];
+            MarkerSoA& dst = need_sort ? ctx->buf[ctx->cur ^ 1] : ctx->buf[ctx->cur];
+            KeyOut ko;
+            ko.keys = ctx->d_keys; ko.hist = ctx->d_hist; ko.ncell = (int)ctx->ncell;
+            ko.enabled = (ctx->sort_every > 0 && ctx->steps_since_sort + 1 >= ctx->sort_every) ? 1 : 0;
+            if (ko.enabled) CU(cudaMemsetAsync(ctx->d_hist, 0, sizeof(int) * (ctx->ncell + 2), ctx->stream));
+            CU(cudaMemsetAsync(ctx->d_work, 0, 8 * sizeof(int), ctx->stream));
+            if (timed) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+            k_push_tiled<Tile><<<ctx->num_sms, Tile::NTHREADS, Tile::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, src, dst, perm, ctx->rq, ko, ctx->cm, dt, ctx->d_work);
             KCHECK();
-            k_push_finish<<<ctx->num_sms * 8, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->buf[ctx->cur], rq, dt);
+            if (timed) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
+            k_push_finish<<<ctx->num_sms * 8, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, src, dst, perm, ctx->rq, ko, ctx->cm, dt);
             KCHECK();
-            k_accumulate_stat<<<1, 1, 0, ctx->stream>>>(ctx->d_work + 1, ctx->d_stats + 1);
+            k_accumulate_stat<<<1, 4, 0, ctx->stream>>>(ctx->rq.count, ctx->rq.cap, ctx->d_stats + 1);
             KCHECK();
             // markers outside the mesh sit behind the last cell: push them through the simple path
-            k_push_lost<<<148 * 4, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->buf[ctx->cur], ctx->d_offs + ctx->ncell, n, dt);
+            k_push_lost<<<148 * 4, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, src, dst, perm, ko, ctx->cm, ctx->d_offs + ctx->ncell, n, dt);
             KCHECK();
+            if (timed) CU(cudaEventRecord(ctx->ev[3], ctx->stream));
+            if (need_sort) ctx->cur ^= 1;
+            ctx->keys_valid = ko.enabled != 0;
             ctx->stats[0] += 4;
         } else {
+            if (need_sort) {
+                int rc = do_sort(ctx);
+                if (rc) return rc;
+            }
+            if (timed) { CU(cudaEventRecord(ctx->ev[1], ctx->stream)); }
             k_push_simple<<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->buf[ctx->cur], n, dt);
             KCHECK();
+            if (timed) { CU(cudaEventRecord(ctx->ev[2], ctx->stream)); CU(cudaEventRecord(ctx->ev[3], ctx->stream)); }
+            ctx->keys_valid = false;
             ctx->stats[0] += 1;
         }
+        if (timed) ctx->ev_valid = true;
         ctx->steps_since_sort += 1;
+    }
+    return TRIMEG_OK;
+}
+
+int trimeg_push_kernel_ms(trimeg_ctx* ctx, double out[3]) {
+    if (!ctx || !out) return fail(ctx, TRIMEG_ERR_BAD_ARG, "push_kernel_ms: null argument");
+    if (!ctx->ev_valid) return fail(ctx, TRIMEG_ERR_BAD_STATE, "push_kernel_ms: no step has been pushed");
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaEventSynchronize(ctx->ev[3]));
+    for (int i = 0; i < 3; ++i) {
+        float ms = 0;
+        CU(cudaEventElapsedTime(&ms, ctx->ev[i], ctx->ev[i + 1]));
+        out[i] = ms;
     }
     return TRIMEG_OK;
 }
@@ -1078,6 +1182,7 @@ int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]) {
         CU(cudaMemcpyAsync(h, ctx->d_stats, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         out[1] = (int64_t)h[1];
+        out[2] = (int64_t)h[2];
     }
     return TRIMEG_OK;
 }

@@ -123,7 +123,10 @@ struct HostMesh {
     std::vector<int32_t> head, list;                 // box grid CSR
 };
 // returns 0 or a negative error code (-3 = bad mesh)
-inline int build_mesh(int64_t n_nodes, const double* RZ, int64_t T, const int32_t* tri_in, HostMesh& hm) {
+// `axis` (nullable): (R, Z) of the magnetic axis.  With it triangles are numbered along flux surfaces: radial bins one
+// element wide (sqrt(2 x mean triangle area)), poloidal angle within a bin, so that consecutive triangles follow the
+// poloidal field direction -- the direction markers move in during an RK4 step.  Without it: Morton order.
+inline int build_mesh(int64_t n_nodes, const double* RZ, int64_t T, const int32_t* tri_in, const double* axis, HostMesh& hm) {
     double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
     for (int64_t n = 0; n < n_nodes; n++) {
         double x = RZ[2 * n], y = RZ[2 * n + 1];
@@ -141,11 +144,28 @@ inline int build_mesh(int64_t n_nodes, const double* RZ, int64_t T, const int32_
     if (!(wx > 0) || !(wy > 0)) return -3;
     // renumber
     std::vector<uint64_t> key(T);
+    double area_sum = 0;
+    for (int64_t t = 0; t < T; t++) {
+        const int32_t* tv = tri_in + 3 * t;
+        double ax = RZ[2 * tv[1]] - RZ[2 * tv[0]], ay = RZ[2 * tv[1] + 1] - RZ[2 * tv[0] + 1];
+        double bx = RZ[2 * tv[2]] - RZ[2 * tv[0]], by = RZ[2 * tv[2] + 1] - RZ[2 * tv[0] + 1];
+        area_sum += 0.5 * (ax * by - ay * bx);
+    }
+    const double bin_w = std::sqrt(2.0 * area_sum / (double)T);
     for (int64_t t = 0; t < T; t++) {
         const int32_t* tv = tri_in + 3 * t;
         double cx = (RZ[2 * tv[0]] + RZ[2 * tv[1]] + RZ[2 * tv[2]]) / 3, cy = (RZ[2 * tv[0] + 1] + RZ[2 * tv[1] + 1] + RZ[2 * tv[2] + 1]) / 3;
-        uint32_t ix = (uint32_t)std::min(32767.0, (cx - xmin) / wx * 32768.0), iy = (uint32_t)std::min(32767.0, (cy - ymin) / wy * 32768.0);
-        key[t] = morton2(ix, iy);
+        if (axis) {
+            double x = cx - axis[0], y = cy - axis[1];
+            double rho = std::sqrt(x * x + y * y), th = std::atan2(y, x);
+            if (th < 0) th += 6.283185307179586;
+            uint64_t bin = (uint64_t)std::min(4.0e9, rho / bin_w);
+            uint64_t ang = (uint64_t)std::min(4294967295.0, th / 6.283185307179586 * 4294967296.0);
+            key[t] = (bin << 32) | ang;
+        } else {
+            uint32_t ix = (uint32_t)std::min(32767.0, (cx - xmin) / wx * 32768.0), iy = (uint32_t)std::min(32767.0, (cy - ymin) / wy * 32768.0);
+            key[t] = morton2(ix, iy);
+        }
     }
     hm.orig_of_new.resize(T); std::iota(hm.orig_of_new.begin(), hm.orig_of_new.end(), 0);
     std::stable_sort(hm.orig_of_new.begin(), hm.orig_of_new.end(), [&](int32_t a, int32_t b) { return key[a] < key[b]; });
@@ -196,11 +216,14 @@ inline int build_mesh(int64_t n_nodes, const double* RZ, int64_t T, const int32_
 }  // namespace trimeg_host
 
 // ---------------------------------------------------------------------------------------------------------
-// Static patches for the tiled push kernel: a patch is a run of TP consecutive triangles in the spatial
-// (Morton) numbering; its slot list = own triangles (slots 0..TP-1) followed by a halo of nearby triangles
-// (first the ring of triangles sharing a vertex with the patch, edge-neighbours first, then further rings,
-// nearest to the patch centroid first) up to SMAX slots.  nbr gives, per slot and edge, the slot across that
-// edge or -1 when that triangle is not staged (or the edge is on the mesh boundary).
+// Static patches for the tiled push kernel: a patch is a run of TP consecutive triangles in the library's
+// numbering; its slot list = own triangles (slots 0..TP-1) followed by a halo of nearby triangles up to SMAX slots.
+// Halo choice: candidates are collected ring by ring (triangles sharing a vertex with the set so far) and ranked
+// by an anisotropic distance to the nearest own triangle: with the magnetic axis known, the distance along the
+// poloidal field direction (tangent to the flux surface) counts 1/aspect of the distance across it, because
+// within one RK4 step markers move mainly along the field (parallel streaming) and hardly across it (drifts).
+// nbr gives, per slot and edge, the slot across that edge or -1 when that triangle is not staged (or the edge is
+// on the mesh boundary).
 namespace trimeg_host {
 struct HostPatches {
     int TP = 0, SMAX = 0, npatch = 0;
@@ -208,7 +231,8 @@ struct HostPatches {
     std::vector<int16_t> nbr;      // [npatch][SMAX][4] (4th = pad)
     std::vector<int32_t> nslots;   // [npatch]
 };
-inline void build_patches(const HostMesh& hm, const double* RZ, int64_t n_nodes, int64_t T, int TP, int SMAX, HostPatches& hp) {
+inline void build_patches(const HostMesh& hm, const double* RZ, int64_t n_nodes, int64_t T, int TP, int SMAX, const double* axis, double aspect,
+                          HostPatches& hp) {
     hp.TP = TP; hp.SMAX = SMAX; hp.npatch = (int)((T + TP - 1) / TP);
     hp.slots.assign((size_t)hp.npatch * SMAX, -1);
     hp.nbr.assign((size_t)hp.npatch * SMAX * 4, -1);
@@ -221,42 +245,51 @@ inline void build_patches(const HostMesh& hm, const double* RZ, int64_t n_nodes,
     std::vector<double> cx(T), cy(T);
     for (int64_t t = 0; t < T; t++) { cx[t] = (RZ[2 * hm.tri[3 * t]] + RZ[2 * hm.tri[3 * t + 1]] + RZ[2 * hm.tri[3 * t + 2]]) / 3; cy[t] = (RZ[2 * hm.tri[3 * t] + 1] + RZ[2 * hm.tri[3 * t + 1] + 1] + RZ[2 * hm.tri[3 * t + 2] + 1]) / 3; }
     std::vector<int32_t> slot_of(T, -1), mark(T, -1);
-    std::vector<int32_t> cur, frontier, next;
+    std::vector<int32_t> frontier, next;
     struct Cand { double key; int32_t t; };
     std::vector<Cand> cand;
+    const double inv_asp2 = 1.0 / (aspect * aspect);
     for (int p = 0; p < hp.npatch; p++) {
         int64_t t0 = (int64_t)p * TP, t1 = std::min<int64_t>(T, t0 + TP);
         int32_t* sl = &hp.slots[(size_t)p * SMAX];
         int ns = 0;
-        double pcx = 0, pcy = 0;
-        for (int64_t t = t0; t < t1; t++) { sl[ns] = (int32_t)t; slot_of[t] = ns; mark[t] = p; ns++; pcx += cx[t]; pcy += cy[t]; }
-        pcx /= (t1 - t0); pcy /= (t1 - t0);
+        for (int64_t t = t0; t < t1; t++) { sl[ns] = (int32_t)t; slot_of[t] = ns; mark[t] = p; ns++; }
         int own = ns;
         // pad unused own slots (last patch) so that own triangles always sit at slot = t - t0
         for (; ns < TP && ns < SMAX; ns++) sl[ns] = -1;
         frontier.assign(sl, sl + own);
-        for (int ring = 0; ring < 4 && ns < SMAX && !frontier.empty(); ring++) {
-            cand.clear();
+        cand.clear();
+        for (int ring = 0; ring < 8 && (int)cand.size() < 5 * SMAX && !frontier.empty(); ring++) {
+            next.clear();
             for (int32_t t : frontier) for (int v = 0; v < 3; v++) {
                 int32_t node = hm.tri[3 * t + v];
                 for (int32_t q = nhead[node]; q < nhead[node + 1]; q++) {
                     int32_t o = nlist[q];
                     if (mark[o] == p) continue;
                     mark[o] = p;
-                    bool edge_nb = false;
-                    for (int e = 0; e < 3; e++) { int32_t nb = hm.nbr[3 * o + e]; if (nb >= 0 && slot_of[nb] >= 0 && slot_of[nb] < own && nb >= t0 && nb < t1) edge_nb = true; }
-                    double d2 = (cx[o] - pcx) * (cx[o] - pcx) + (cy[o] - pcy) * (cy[o] - pcy);
-                    cand.push_back({(ring == 0 && edge_nb ? 0.0 : 1.0) + 1e-3 * d2 / (1e-300 + d2 + 1.0) + ring, o});
-                    cand.back().key = ring * 10.0 + (edge_nb && ring == 0 ? 0.0 : 1.0) + d2 / (d2 + 1.0);
+                    next.push_back(o);
+                    double best = 1e300;
+                    for (int64_t h = t0; h < t1; h++) {
+                        double dx = cx[o] - cx[h], dy = cy[o] - cy[h], d2;
+                        if (axis) {
+                            double ex = -(cy[h] - axis[1]), ey = cx[h] - axis[0], en = std::sqrt(ex * ex + ey * ey);
+                            if (en > 0) {
+                                ex /= en; ey /= en;
+                                double dpar = dx * ex + dy * ey, dperp = -dx * ey + dy * ex;
+                                d2 = dpar * dpar * inv_asp2 + dperp * dperp;
+                            } else d2 = dx * dx + dy * dy;
+                        } else d2 = dx * dx + dy * dy;
+                        best = std::min(best, d2);
+                    }
+                    cand.push_back({best, o});
                 }
             }
-            std::sort(cand.begin(), cand.end(), [](const Cand& a, const Cand& b) { return a.key < b.key; });
-            next.clear();
-            for (const Cand& c : cand) {
-                if (ns >= SMAX) break;
-                sl[ns] = c.t; slot_of[c.t] = ns; ns++; next.push_back(c.t);
-            }
             frontier.swap(next);
+        }
+        std::sort(cand.begin(), cand.end(), [](const Cand& a, const Cand& b) { return a.key < b.key || (a.key == b.key && a.t < b.t); });
+        for (const Cand& c : cand) {
+            if (ns >= SMAX) break;
+            sl[ns] = c.t; slot_of[c.t] = ns; ns++;
         }
         hp.nslots[p] = ns;
         for (int s = 0; s < ns; s++) {

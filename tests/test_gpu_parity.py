@@ -182,6 +182,26 @@ def test_push_unstructured_em_with_resort(variant):
     _check_push(o, g, m, cfg, 0.05, 10, variant, sort_every=3)
 
 
+@pytest.mark.parametrize("sort_every", [1, 2])
+def test_push_sort_fused_into_push(sort_every):
+    """Tiled variant with a re-sort every step / every other step: the sort only builds the permutation and the push
+    kernel reads the markers through it (and writes the next sort's keys); trajectories, the caller's ordering and
+    the lost set must not change.  Also checks markers_get / rhs between pushes (they read the current buffer)."""
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, n_markers=40_013)
+    RZ, tri, o, g, m = _make(cfg)
+    _check_push(o, g, m, cfg, 0.05, 10, 0, sort_every=sort_every)
+    # continue in two further calls (keys carried across calls), then compare against 10 + 3 + 2 oracle steps
+    g.push_rk4(0.05, 3)
+    mid = g.markers_get(host=True)
+    g.push_rk4(0.05, 2)
+    res = g.markers_get(host=True)
+    exp = o.push_rk4(*[m[k] for k in KEYS], 0.05, 15)
+    assert ((res["status"] != 0) == (exp[5] != 0)).all()
+    for q, k in enumerate(("R", "Z", "phi", "u", "w")):
+        assert _rel(res[k], exp[q], cfg.phi_period if k == "phi" else None) < 2e-10, k
+    assert not np.array_equal(mid["R"], res["R"])
+
+
 @pytest.mark.parametrize("variant", [0, 1])
 def test_push_degenerate_cases(variant):
     """n = 1; nsteps = 0 (state unchanged); negative charge; nonlinear weight mode; literal-L53 b*; zero fields."""
