@@ -1,0 +1,616 @@
+// Device kernels of the marker push: marker store, setup, gather, the two-phase RK4 push and the counting sort.
+// Compiled for sm_100a only.  DESIGN.md "Kernels" describes the split of one RK4 step into two phases.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "trimeg_math.cuh"
+#include "trimeg_tile.cuh"
+
+namespace trimeg {
+
+// ============================================================================================ marker store
+// One 128-byte record per marker (array of structures: a marker is always read and written whole, through a sort
+// permutation, so one record = one cache line = four full 32-byte sectors).  Two buffers: a phase that re-sorts reads
+// buffer A through the permutation and writes buffer B in cell order, so the data movement of the sort costs no pass
+// of its own and the next permutation is nearly the identity.  What y and k hold depends on where the step stands:
+//   between steps / before phase A:  y = state y_n (R, Z, phi, u, w),       k = k1 = f(y_n)
+//   between phase A and phase B:     y = Y = y_n + dt/6 (k1 + 2 k2 + 2 k3),  k = y4 = y_n + dt k3 (stage-4 position)
+// tri = triangle (library numbering) of the next phase's first evaluation point, -1 unknown / outside.
+struct __align__(16) Rec {
+    double y[5];
+    double k[5];
+    double mu, p;
+    int tri, st;
+    int id, pad0;            // id = index in the caller's arrays
+    double pad[2];
+};
+static_assert(sizeof(Rec) == 128, "marker record is one 128-byte line");
+
+struct DevTables {
+    const TriGeom* geom;     // [T]
+    const double* coef;      // [T][P+3+2*PLANE_PAD][21][2]; see PLANE_PAD in trimeg_math.cuh
+    BoxGrid bg;
+    TorP tor;
+    int T;
+    long long tri_stride;    // doubles per triangle = (P+3+2*PLANE_PAD)*42
+};
+
+// tiled push configuration: patches of 8 triangles + halo (36 slots), windows of 4 toroidal intervals (+1 each side),
+// ring of 2 staged blocks, 16 independent warps per CTA, one CTA per SM
+using Tile = TileCfg<8, 36, 4, 16>;
+// cell numbering used by the sort: super-cell (patch, window) major, then triangle within the patch, then interval
+struct CellMap {
+    int P, nwin;
+    __host__ __device__ __forceinline__ int cell(int t, int k) const {
+        int patch = t / Tile::TP, tl = t - patch * Tile::TP, wdw = k / Tile::WK, kl = k - wdw * Tile::WK;
+        return ((patch * nwin + wdw) * Tile::TP + tl) * Tile::WK + kl;
+    }
+};
+// where the sort key of a marker's next evaluation point goes (the counting sort's first pass is fused into the push)
+struct KeyOut {
+    int* keys;      // [n] cell of the next phase's first evaluation point, indexed like the destination buffer
+    int* hist;      // [ncell + 2] histogram of the keys; bin ncell = outside the mesh
+    int ncell;
+    int enabled;
+};
+
+__constant__ double c_Aplus[21 * 18];
+__constant__ double c_Nul[21 * 3];
+
+__device__ __forceinline__ void rec_load(const Rec* __restrict__ p, Rec& r) {
+    const double2* s = reinterpret_cast<const double2*>(p);
+    double2* d = reinterpret_cast<double2*>(&r);
+#pragma unroll
+    for (int i = 0; i < 7; ++i) d[i] = __ldcs(s + i);   // 13 doubles are live; the padding is never read
+}
+__device__ __forceinline__ void rec_store(Rec* __restrict__ p, const Rec& r) {
+    double2* d = reinterpret_cast<double2*>(p);
+    const double2* s = reinterpret_cast<const double2*>(&r);
+#pragma unroll
+    for (int i = 0; i < 7; ++i) d[i] = s[i];
+}
+
+// ============================================================================================ setup kernels
+// fields_set: nodal DOFs -> per-triangle reference-frame polynomial coefficients, for one field.
+// One thread per (triangle, plane).  c = c0 - Nul (K c0_5),  c0 = Aplus d_ref,  d_ref = DOFs pulled back with J.
+__global__ void k_fields_set(int T, int P, int which, const int* __restrict__ tri, const double* __restrict__ RZ,
+                             const double* __restrict__ Kmat, const double* __restrict__ dof, long long n_nodes,
+                             double* __restrict__ coef) {
+    long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (long long)T * P) return;
+    int t = (int)(gid / P), k = (int)(gid % P);
+    int nd[3] = {tri[3 * t], tri[3 * t + 1], tri[3 * t + 2]};
+    double x0 = RZ[2 * nd[0]], y0 = RZ[2 * nd[0] + 1];
+    double j11 = RZ[2 * nd[1]] - x0, j21 = RZ[2 * nd[1] + 1] - y0, j12 = RZ[2 * nd[2]] - x0, j22 = RZ[2 * nd[2] + 1] - y0;
+    double d[18];
+#pragma unroll
+    for (int v = 0; v < 3; ++v) {
+        const double* s = dof + ((long long)k * n_nodes + nd[v]) * 6;
+        double f = s[0], fR = s[1], fZ = s[2], fRR = s[3], fRZ = s[4], fZZ = s[5];
+        d[6 * v + 0] = f;
+        d[6 * v + 1] = j11 * fR + j21 * fZ;                       // J^T grad
+        d[6 * v + 2] = j12 * fR + j22 * fZ;
+        double hR1 = fRR * j11 + fRZ * j21, hZ1 = fRZ * j11 + fZZ * j21;   // H J (column 1)
+        double hR2 = fRR * j12 + fRZ * j22, hZ2 = fRZ * j12 + fZZ * j22;   // H J (column 2)
+        d[6 * v + 3] = j11 * hR1 + j21 * hZ1;                     // J^T H J
+        d[6 * v + 4] = j11 * hR2 + j21 * hZ2;
+        d[6 * v + 5] = j12 * hR2 + j22 * hZ2;
+    }
+    double c[21];
+#pragma unroll
+    for (int i = 0; i < 21; ++i) {
+        double s = 0.0;
+#pragma unroll
+        for (int q = 0; q < 18; ++q) s = fma(c_Aplus[i * 18 + q], d[q], s);
+        c[i] = s;
+    }
+    // quintic part: monomial m = (5-m, m) sits at j-major index off[m] + 5 - m
+    const int qi[6] = {5, 6 + 4, 11 + 3, 15 + 2, 18 + 1, 20};
+    const double* K = Kmat + (long long)t * 18;
+    double z[3];
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        double s = 0.0;
+#pragma unroll
+        for (int m = 0; m < 6; ++m) s = fma(K[r * 6 + m], c[qi[m]], s);
+        z[r] = s;
+    }
+    const int NPP = P + 3 + 2 * PLANE_PAD;
+    long long tri_stride = (long long)NPP * PLANE_STRIDE;
+    double* base = coef + (long long)t * tri_stride;
+    int slots[3];
+#pragma unroll
+    for (int s = 0; s < 3; ++s) { int pp = k + 1 + PLANE_PAD + (s - 1) * P; slots[s] = (pp >= 0 && pp < NPP) ? pp : -1; }
+#pragma unroll
+    for (int i = 0; i < 21; ++i) {
+        double v = c[i] - (c_Nul[i * 3] * z[0] + c_Nul[i * 3 + 1] * z[1] + c_Nul[i * 3 + 2] * z[2]);
+#pragma unroll
+        for (int s = 0; s < 3; ++s) if (slots[s] >= 0) base[(long long)slots[s] * PLANE_STRIDE + 2 * i + which] = v;
+    }
+}
+
+// SoA caller arrays -> records [first, first + cnt)
+__global__ void k_bind(Rec* __restrict__ recs, long long first, long long cnt, const double* R, const double* Z, const double* phi,
+                       const double* u, const double* w, const double* mu, const double* p) {
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= cnt) return;
+    Rec r;
+    r.y[0] = R[i]; r.y[1] = Z[i]; r.y[2] = phi[i]; r.y[3] = u[i]; r.y[4] = w[i];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) r.k[q] = 0.0;
+    r.mu = mu[i]; r.p = p[i]; r.tri = -1; r.st = 0;
+    r.id = (int)(first + i); r.pad0 = 0;
+    r.pad[0] = r.pad[1] = 0.0;
+    double2* d = reinterpret_cast<double2*>(recs + first + i);
+    const double2* s = reinterpret_cast<const double2*>(&r);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) d[q] = s[q];
+}
+// records -> SoA arrays in the caller's order (any may be null)
+__global__ void k_get(const Rec* __restrict__ recs, long long n, double* R, double* Z, double* phi, double* u, double* w, int* status) {
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    Rec r;
+    rec_load(recs + i, r);
+    const long long o = r.id;
+    if (R) R[o] = r.y[0];
+    if (Z) Z[o] = r.y[1];
+    if (phi) phi[o] = r.y[2];
+    if (u) u[o] = r.y[3];
+    if (w) w[o] = r.y[4];
+    if (status) status[o] = r.st;
+}
+
+// ============================================================================================ gather / global path
+struct LdGlobal {   // coefficient pair fetch from the global table (L1/L2)
+    const double2* p;
+    __device__ __forceinline__ void operator()(int idx, double& a, double& b) const {
+        double2 v = __ldg(p + idx);
+        a = v.x; b = v.y;
+    }
+};
+
+__device__ __forceinline__ void gather_at(const DevTables& tb, int t, double R, double Z, double phi, Fields& f) {
+    if (t < 0) { f = Fields{0, 0, 0, 0, 0, 0, 0, 0}; return; }
+    const TriGeom g = tb.geom[t];
+    double xi, eta;
+    ref_coords(g, R, Z, xi, eta);
+    double w[4], dw[4];
+    int kk = bspline_weights(tb.tor, phi, w, dw);
+    LdGlobal ld{reinterpret_cast<const double2*>(tb.coef + (long long)t * tb.tri_stride + (long long)(kk + PLANE_PAD) * PLANE_STRIDE)};
+    double acc[8];
+    gather_cell(ld, xi, eta, w, dw, acc);
+    to_fields(g, acc, f);
+}
+
+__global__ void __launch_bounds__(256) k_gather(DevTables tb, long long n, const double* __restrict__ R, const double* __restrict__ Z,
+                                                const double* __restrict__ phi, double* __restrict__ out, int* __restrict__ tri_out) {
+    long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    double r = R[m], z = Z[m];
+    int t = locate_box(tb.bg, tb.geom, r, z);
+    Fields f;
+    gather_at(tb, t, r, z, phi[m], f);
+    out[m] = f.P; out[n + m] = f.PR; out[2 * n + m] = f.PZ; out[3 * n + m] = f.Pp;
+    out[4 * n + m] = f.A; out[5 * n + m] = f.AR; out[6 * n + m] = f.AZ; out[7 * n + m] = f.Ap;
+    if (tri_out) tri_out[m] = t < 0 ? -1 : tb.geom[t].orig;
+}
+
+// one right-hand-side evaluation for one marker, fields through L1/L2; updates the triangle hint; returns 1 if outside
+__device__ __forceinline__ int stage_simple(const DevTables& tb, const EquilP& ep, const SpeciesP& sp, int& t, double R, double Z,
+                                            double phi, double u, double w, double mu, double p, double d[5]) {
+    t = locate_walk(tb.bg, tb.geom, t, R, Z);
+    Fields f;
+    gather_at(tb, t, R, Z, phi, f);
+    rhs_eval(ep, sp, R, Z, u, w, mu, p, f, d);
+    return t < 0;
+}
+
+__device__ __forceinline__ double wrap_phi(const TorP& tp, double phi) {
+    double ph = fma(-tp.period, floor(phi * tp.inv_period), phi);
+    if (ph < 0.0) ph += tp.period;
+    if (ph >= tp.period) ph -= tp.period;
+    return ph;
+}
+
+// ============================================================================================ two-phase RK4 step
+// Classical RK4 evaluates f at three places per step: y_n (k1), the half-step points y_n + dt/2 k1 and y_n + dt/2 k2
+// (k2, k3), and the full-step points y_n + dt k3 (k4) and y_{n+1} (the next step's k1).  The two half-step points lie
+// within O(dt^2) of each other, and so do the two full-step points, but at dt = 0.05 the half- and full-step points of
+// the ITG configurations are about one mesh cell apart.  The step is therefore split where the cell changes:
+//   phase A (markers ordered by the cell of y_n + dt/2 k1):   k2, k3          -> Y = y_n + dt/6 (k1 + 2 k2 + 2 k3), y4
+//   phase B (markers ordered by the cell of y4):              k4, y_{n+1}, k1' = f(y_{n+1})
+// so that both evaluations of a phase read the coefficient block of (almost always) one cell and all lanes of a warp
+// read the same few cells.  PHASE_INIT computes k1 = f(y_n) for a freshly bound store.
+// The arithmetic of a step is the textbook one; only the order in which markers are visited changes.
+enum { PHASE_A = 0, PHASE_B = 1, PHASE_INIT = 2 };
+
+// Advances record r through one phase.  eval(y, d) evaluates the right-hand side at y and returns false if it cannot
+// (the tiled kernel: evaluation point outside the staged block); then r is left untouched and false is returned.
+// next[0..2] = (R, Z, phi) of the following phase's first evaluation point.
+template <int PHASE, class Eval>
+__device__ __forceinline__ bool phase_step(const TorP& tor, double dt, Rec& r, Eval&& eval, double next[3]) {
+    const double h2 = 0.5 * dt, h6 = dt / 6.0;
+    double a[5], b[5], y[5];
+    if (PHASE == PHASE_A) {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) y[q] = fma(h2, r.k[q], r.y[q]);
+        if (!eval(y, a)) return false;                                  // k2
+#pragma unroll
+        for (int q = 0; q < 5; ++q) y[q] = fma(h2, a[q], r.y[q]);
+        if (!eval(y, b)) return false;                                  // k3
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+            double acc = fma(2.0, b[q], fma(2.0, a[q], r.k[q]));
+            double y0 = r.y[q];
+            r.y[q] = fma(h6, acc, y0);                                  // Y
+            r.k[q] = fma(dt, b[q], y0);                                 // y4
+        }
+        next[0] = r.k[0]; next[1] = r.k[1]; next[2] = r.k[2];
+    } else {
+        if (PHASE == PHASE_B) {
+            if (!eval(r.k, a)) return false;                            // k4
+#pragma unroll
+            for (int q = 0; q < 5; ++q) y[q] = fma(h6, a[q], r.y[q]);   // y_{n+1}
+            y[2] = wrap_phi(tor, y[2]);
+        } else {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) y[q] = r.y[q];
+        }
+        if (!eval(y, b)) return false;                                  // k1 of the next step
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { r.y[q] = y[q]; r.k[q] = b[q]; }
+        next[0] = fma(h2, b[0], y[0]); next[1] = fma(h2, b[1], y[1]); next[2] = fma(h2, b[2], y[2]);
+    }
+    return true;
+}
+
+// final store of one record: the record itself and (if enabled) the sort key of its next evaluation point
+__device__ __forceinline__ void store_rec(const DevTables& tb, const CellMap& cm, const KeyOut& ko, Rec* __restrict__ recs, long long ri,
+                                          Rec& r, int t, const double next[3]) {
+    r.tri = t;
+    rec_store(recs + ri, r);
+    if (ko.enabled) {
+        double sf;
+        int k = toroidal_interval(tb.tor, next[2], sf);
+        int key = t < 0 ? ko.ncell : cm.cell(t, k);
+        ko.keys[ri] = key;
+        atomicAdd(ko.hist + key, 1);
+    }
+}
+
+// one phase for one record through the global tables (L1/L2): the follow-up path of the tiled kernel (markers that
+// left their staged block, markers outside the mesh), the initial k1, and un-sorted operation
+template <int PHASE>
+__device__ __forceinline__ void phase_global(const DevTables& tb, const EquilP& ep, const SpeciesP& sp, const CellMap& cm, const KeyOut& ko,
+                                             const Rec* __restrict__ src, Rec* __restrict__ dst, long long ri, long long m, double dt) {
+    Rec r;
+    rec_load(src + ri, r);
+    int t = r.tri, st = r.st;
+    const double mu = r.mu, p = r.p;
+    auto eval = [&](const double y[5], double d[5]) {
+        st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, d);
+        return true;
+    };
+    double next[3];
+    phase_step<PHASE>(tb.tor, dt, r, eval, next);
+    t = locate_walk(tb.bg, tb.geom, t, next[0], next[1]);
+    r.st = st;
+    store_rec(tb, cm, ko, dst, m, r, t, next);
+}
+// positions m = index[i] (or i if index is null) of the cell order for i in [*first (or 0), *count (or n)):
+// record src[perm[m]] (or src[m] if perm is null) -> dst[m]
+template <int PHASE>
+__global__ void __launch_bounds__(128) k_phase_global(DevTables tb, EquilP ep, SpeciesP sp, CellMap cm, KeyOut ko, const Rec* __restrict__ src,
+                                                      Rec* __restrict__ dst, const int* __restrict__ perm, const int* __restrict__ index,
+                                                      const int* __restrict__ first, const int* __restrict__ count, long long n, double dt) {
+    const long long lo = first ? (long long)*first : 0, hi = count ? (long long)*count : n;
+    for (long long i = lo + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < hi; i += (long long)gridDim.x * blockDim.x) {
+        const long long m = index ? (long long)index[i] : i;
+        phase_global<PHASE>(tb, ep, sp, cm, ko, src, dst, perm ? (long long)perm[m] : m, m, dt);
+    }
+}
+
+// variant 1: the whole classical RK4 step, one thread per marker, in place, coefficients through L1/L2 (reference for the
+// two-phase path; leaves the records' k stale)
+__global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, SpeciesP sp, Rec* __restrict__ recs, long long n, double dt) {
+    long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    Rec r;
+    rec_load(recs + m, r);
+    double y0[5], k[5], acc[5], y[5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) y0[q] = r.y[q];
+    const double mu = r.mu, p = r.p;
+    int t = r.tri, st = r.st;
+    st |= stage_simple(tb, ep, sp, t, y0[0], y0[1], y0[2], y0[3], y0[4], mu, p, k);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { acc[q] = k[q]; y[q] = fma(0.5 * dt, k[q], y0[q]); }
+    st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { acc[q] = fma(2.0, k[q], acc[q]); y[q] = fma(0.5 * dt, k[q], y0[q]); }
+    st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { acc[q] = fma(2.0, k[q], acc[q]); y[q] = fma(dt, k[q], y0[q]); }
+    st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k);
+    const double h6 = dt / 6.0;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) r.y[q] = fma(h6, acc[q] + k[q], y0[q]);
+    r.y[2] = wrap_phi(tb.tor, r.y[2]);
+    r.tri = t; r.st = st;
+    rec_store(recs + m, r);
+}
+
+// the paper's own kernel boundary (L89): the five time derivatives at the current state, caller order
+__global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP sp, const Rec* __restrict__ recs, long long n, double* __restrict__ out) {
+    long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    Rec r;
+    rec_load(recs + m, r);
+    int t = r.tri;
+    double d[5];
+    stage_simple(tb, ep, sp, t, r.y[0], r.y[1], r.y[2], r.y[3], r.y[4], r.mu, r.p, d);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) out[(long long)q * n + r.id] = d[q];
+}
+
+// ============================================================================================ tiled phase kernel
+// markers that left their staged block during a phase: positions in the cell order, finished by k_phase_global
+struct RetireList {
+    int* list;      // [n]
+    int* count;     // device counter
+};
+
+// (re)fill ring entry b with the next non-empty super-cell; executed by one whole warp.  The entry's mbarrier completes
+// when the TMA bytes have landed (or at once, with sc = -1, when the work list is exhausted).
+template <class C>
+__device__ __forceinline__ void tile_refill(unsigned char* smem, int b, const DevTables& tb, const TileTables& tt, int* work_counter, int lane) {
+    constexpr unsigned FULL = 0xffffffffu;
+    double* coef = reinterpret_cast<double*>(smem + C::BLOCK_BYTES * b);
+    SlotGeom* sgeom = reinterpret_cast<SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
+    BlockCtrl* ctl = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL) + b;
+    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF) + 2 * b;
+    int sc = 0, begin = 0, end = 0;
+    for (;;) {
+        if (lane == 0) sc = atomicAdd(work_counter, 1);
+        sc = __shfl_sync(FULL, sc, 0);
+        if (sc >= tt.nsc) { sc = -1; break; }
+        begin = tt.offs[(long long)sc * C::CPS]; end = tt.offs[(long long)(sc + 1) * C::CPS];
+        if (begin != end) break;
+    }
+    if (sc < 0) {
+        if (lane == 0) { ctl->sc = -1; ctl->left = 0; __threadfence_block(); asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(mbar)) : "memory"); }
+        return;
+    }
+    const int patch = sc / tt.nwin, k0 = (sc - patch * tt.nwin) * C::WK;
+    const int ns = tt.nslots[patch];
+    const int* pslots = tt.slots + (long long)patch * C::SMAX;
+    if (lane == 0) { ctl->sc = sc; ctl->begin = begin; ctl->end = end; ctl->next = begin; ctl->left = 0; ctl->ns = ns; ctl->patch = patch; ctl->k0 = k0; }
+    int cnt = 0;
+    for (int sl = lane; sl < ns; sl += 32) {
+        int t = pslots[sl];
+        SlotGeom g;
+        if (t >= 0) {
+            const TriGeom tg = tb.geom[t];
+            g.v0x = tg.v0x; g.v0y = tg.v0y; g.a11 = tg.a11; g.a12 = tg.a12; g.a21 = tg.a21; g.a22 = tg.a22;
+            const short* nb = tt.nbr + ((long long)patch * C::SMAX + sl) * 4;
+            g.nbr[0] = nb[0]; g.nbr[1] = nb[1]; g.nbr[2] = nb[2]; g.nbr[3] = -1;
+            cnt++;
+        } else {
+            g.v0x = g.v0y = 1e300; g.a11 = g.a12 = g.a21 = g.a22 = 0.0; g.nbr[0] = g.nbr[1] = g.nbr[2] = g.nbr[3] = -1;
+        }
+        g.tri = t; g.pad = 0;
+        sgeom[sl] = g;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(FULL, cnt, o);
+    __threadfence_block();
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic accesses of this block vs. the async writes
+    __syncwarp();
+    if (lane == 0) mbar_expect_tx(mbar, (unsigned)(cnt * C::SLOT_DOUBLES * sizeof(double)));
+    __syncwarp();
+    for (int sl = lane; sl < ns; sl += 32) {
+        int t = pslots[sl];
+        if (t >= 0)
+            tma_bulk_g2s(coef + (size_t)sl * C::SLOT_DOUBLES, tb.coef + (long long)t * tb.tri_stride + (long long)k0 * PLANE_STRIDE,
+                         (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
+    }
+}
+
+// slot-space edge walk inside the staged block: returns the slot containing (R, Z) or -1 (left the staged set / hop cap)
+__device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int sl, double R, double Z, double& xi, double& eta) {
+    if (sl < 0) return -1;
+    for (int hop = 0; hop < 16; ++hop) {
+        const SlotGeom& g = sgeom[sl];
+        double dx = R - g.v0x, dy = Z - g.v0y;
+        xi = fma(g.a11, dx, g.a12 * dy);
+        eta = fma(g.a21, dx, g.a22 * dy);
+        double l0 = 1.0 - xi - eta;
+        if (fmin(fmin(xi, eta), l0) >= INSIDE_TOL) return sl;
+        int e = (eta <= xi && eta <= l0) ? 0 : ((l0 <= xi) ? 1 : 2);
+        sl = g.nbr[e];
+        if (sl < 0) return -1;
+    }
+    return -1;
+}
+
+// One phase of the RK4 step for the markers of one super-cell after another.  Position j of the cell order is record
+// src[perm[j]] (perm null: src[j]) and is written to dst[j].  Persistent: one CTA per SM, every warp runs on its own.
+template <class C, int PHASE>
+__global__ void __launch_bounds__(C::NTHREADS, 1)
+k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __restrict__ src, Rec* __restrict__ dst, const int* __restrict__ perm,
+              RetireList rq, KeyOut ko, CellMap cm, double dt, int* __restrict__ work_counter) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    BlockCtrl* ctl_all = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL);
+    unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF);
+    if (tid == 0) {
+        for (int b = 0; b < C::NBUF; ++b) mbar_init(mbar_all + 2 * b, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (wid == 0) {
+        for (int b = 0; b < C::NBUF; ++b) tile_refill<C>(smem, b, tb, tt, work_counter, lane);
+    }
+    const int P = tb.tor.P;
+    constexpr unsigned FULL = 0xffffffffu;
+
+    // every warp walks the ring in the same order; the last warp to leave an entry refills it (no block-wide barrier)
+    for (unsigned it = 0;; ++it) {
+        const int b = it % C::NBUF;
+        mbar_wait(mbar_all + 2 * b, (it / C::NBUF) & 1);
+        BlockCtrl* ctl = ctl_all + b;
+        if (ctl->sc < 0) break;
+        const double* coef = reinterpret_cast<const double*>(smem + C::BLOCK_BYTES * b);
+        const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
+        const int end = ctl->end, patch = ctl->patch, k0 = ctl->k0, ns = ctl->ns;
+        int* sh_next = &ctl->next;
+
+        // ---- each warp grabs chunks of 32 markers until the super-cell is drained
+        for (;;) {
+            int chunk = 0;
+            if (lane == 0) chunk = atomicAdd(sh_next, 32);
+            chunk = __shfl_sync(FULL, chunk, 0);
+            if (chunk >= end) break;
+            const int m = chunk + lane;
+            if (m < end) {
+                const long long ri = perm ? (long long)perm[m] : (long long)m;
+                Rec r;
+                rec_load(src + ri, r);
+                const double mu = r.mu, pw = r.p;
+                int st = r.st, cur = -1, tri_last = r.tri;
+                {
+                    int sl = tri_last - patch * C::TP;
+                    if (sl >= 0 && sl < C::TP) cur = sl;
+                    else {   // not sorted since it moved: look for the triangle in the halo
+                        for (int q = C::TP; q < ns; ++q) if (sgeom[q].tri == tri_last) { cur = q; break; }
+                    }
+                }
+                auto eval = [&](const double y[5], double d[5]) {
+                    double xi = 0.0, eta = 0.0, sf;
+                    const int sl = slot_walk(sgeom, cur, y[0], y[1], xi, eta);
+                    const int k = toroidal_interval(tb.tor, y[2], sf);
+                    int dk = k - k0;
+                    if (dk > P / 2) dk -= P; else if (dk < -(P / 2)) dk += P;
+                    const int lk = dk + C::HK;
+                    if (!(sl >= 0 && lk >= 0 && lk < C::NW)) return false;
+                    cur = sl;
+                    const SlotGeom& g = sgeom[sl];
+                    tri_last = g.tri;
+                    double w[4], dw[4], g8[8];
+                    bspline_from_s(tb.tor, sf, w, dw);
+                    LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
+                    gather_cell(ld, xi, eta, w, dw, g8);
+                    Fields fo;
+                    fo.P = g8[0]; fo.PR = fma(g.a11, g8[1], g.a21 * g8[2]); fo.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); fo.Pp = g8[3];
+                    fo.A = g8[4]; fo.AR = fma(g.a11, g8[5], g.a21 * g8[6]); fo.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); fo.Ap = g8[7];
+                    rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, fo, d);
+                    return true;
+                };
+                double next[3];
+                if (phase_step<PHASE>(tb.tor, dt, r, eval, next)) {
+                    // triangle of the next phase's first evaluation point: staged walk, else the global walk (rare)
+                    double xi, eta;
+                    const int sl = slot_walk(sgeom, cur, next[0], next[1], xi, eta);
+                    const int t = sl >= 0 ? sgeom[sl].tri : locate_walk(tb.bg, tb.geom, tri_last, next[0], next[1]);
+                    r.st = st;
+                    store_rec(tb, cm, ko, dst, m, r, t, next);
+                } else {
+                    rq.list[atomicAdd(rq.count, 1)] = m;   // the follow-up kernel redoes this phase through the global tables
+                }
+            }
+        }
+        // leave the entry; the last warp out refills it with the next super-cell
+        __syncwarp();
+        int last = 0;
+        if (lane == 0) { __threadfence_block(); last = atomicAdd(&ctl->left, 1) == C::NWARPS - 1; }
+        last = __shfl_sync(FULL, last, 0);
+        if (last) { __threadfence_block(); tile_refill<C>(smem, b, tb, tt, work_counter, lane); }
+    }
+}
+
+// ============================================================================================ counting sort by cell
+// exclusive scan of int counts, three passes over chunks of SCAN_CHUNK
+constexpr int SCAN_THREADS = 512, SCAN_ITEMS = 8, SCAN_CHUNK = SCAN_THREADS * SCAN_ITEMS;
+__device__ __forceinline__ int block_exclusive_scan(int v, int* total) {   // SCAN_THREADS threads
+    __shared__ int warp_sums[SCAN_THREADS / 32];
+    int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) warp_sums[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+        int s = lane < SCAN_THREADS / 32 ? warp_sums[lane] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += y; }
+        if (lane < SCAN_THREADS / 32) warp_sums[lane] = s;
+    }
+    __syncthreads();
+    int base = wid ? warp_sums[wid - 1] : 0;
+    if (total) *total = warp_sums[SCAN_THREADS / 32 - 1];
+    __syncthreads();
+    return base + x - v;
+}
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(const int* __restrict__ in, long long n, int* __restrict__ sums) {
+    long long base = (long long)blockIdx.x * SCAN_CHUNK + (long long)threadIdx.x * SCAN_ITEMS;
+    int s = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) if (base + i < n) s += in[base + i];
+    int tot;
+    block_exclusive_scan(s, &tot);
+    if (threadIdx.x == 0) sums[blockIdx.x] = tot;
+}
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(int* __restrict__ sums, int nb) {   // single block
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < nb; b0 += SCAN_THREADS) {
+        int i = b0 + threadIdx.x, v = i < nb ? sums[i] : 0, tot;
+        int ex = block_exclusive_scan(v, &tot);
+        int c = carry;
+        if (i < nb) sums[i] = ex + c;
+        __syncthreads();
+        if (threadIdx.x == 0) carry = c + tot;
+        __syncthreads();
+    }
+}
+// writes the exclusive offsets and clears the histogram and the fill counters for the next pass
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(int* __restrict__ in, long long n, const int* __restrict__ sums,
+                                                             int* __restrict__ out, int* __restrict__ fill) {
+    long long base = (long long)blockIdx.x * SCAN_CHUNK + (long long)threadIdx.x * SCAN_ITEMS;
+    int v[SCAN_ITEMS], s = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { v[i] = base + i < n ? in[base + i] : 0; s += v[i]; }
+    int ex = block_exclusive_scan(s, nullptr) + sums[blockIdx.x];
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) {
+        if (base + i < n) { out[base + i] = ex; in[base + i] = 0; fill[base + i] = 0; }
+        ex += v[i];
+    }
+}
+// permutation: perm[position in cell order] = record index (4-byte scattered writes)
+__global__ void __launch_bounds__(256) k_sort_perm(long long n, const int* __restrict__ keys, const int* __restrict__ offs, int* __restrict__ fill,
+                                                   int* __restrict__ perm) {
+    long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    int key = keys[m];
+    long long pos = (long long)offs[key] + atomicAdd(fill + key, 1);
+    perm[pos] = (int)m;
+}
+// per phase: acc[0] += markers left to the follow-up kernel
+__global__ void k_accumulate_stat(const int* __restrict__ v, unsigned long long* __restrict__ acc) {
+    atomicAdd(acc, (unsigned long long)*v);
+}
+
+// ============================================================================================ DFMA micro-benchmark
+__global__ void __launch_bounds__(512) k_dfma(double* out, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
+}  // namespace trimeg
