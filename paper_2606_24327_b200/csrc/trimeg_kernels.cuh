@@ -35,9 +35,9 @@ struct DevTables {
     long long tri_stride;    // doubles per triangle = (P+3+2*PLANE_PAD)*42
 };
 
-// tiled push configuration: patches of 8 triangles + halo (36 slots), windows of 4 toroidal intervals (+1 each side),
+// tiled push configuration: patches of 8 triangles + halo (16 slots), windows of 4 toroidal intervals (+1 each side),
 // ring of 2 staged blocks, 16 independent warps per CTA, one CTA per SM
-using Tile = TileCfg<8, 36, 4, 16>;
+using Tile = TileCfg<8, 16, 4, 16>;
 // cell numbering used by the sort: super-cell (patch, window) major, then triangle within the patch, then interval
 struct CellMap {
     int P, nwin;
@@ -57,17 +57,23 @@ struct KeyOut {
 __constant__ double c_Aplus[21 * 18];
 __constant__ double c_Nul[21 * 3];
 
-__device__ __forceinline__ void rec_load(const Rec* __restrict__ p, Rec& r) {
-    const double2* s = reinterpret_cast<const double2*>(p);
+// In memory the eight 16-byte chunks of record i are stored XOR-swizzled by (i & 7): logical chunk j sits at chunk
+// position j ^ (i & 7).  With that the tiled kernel's shared-memory image of 32 consecutive records (row stride 128 B) is
+// at once bank-conflict free for per-lane 16-byte accesses and the verbatim image of the records in global memory, so a
+// chunk of 32 updated records leaves the SM as ONE 4-KB bulk copy.
+__device__ __forceinline__ void rec_load(const Rec* __restrict__ base, long long i, Rec& r) {
+    const double2* s = reinterpret_cast<const double2*>(base + i);
     double2* d = reinterpret_cast<double2*>(&r);
+    const int sw = (int)(i & 7);
 #pragma unroll
-    for (int i = 0; i < 7; ++i) d[i] = __ldcs(s + i);   // 13 doubles are live; the padding is never read
+    for (int j = 0; j < 7; ++j) d[j] = __ldcs(s + (j ^ sw));   // 14 doubles are live; the last chunk is padding
 }
-__device__ __forceinline__ void rec_store(Rec* __restrict__ p, const Rec& r) {
-    double2* d = reinterpret_cast<double2*>(p);
+__device__ __forceinline__ void rec_store(Rec* __restrict__ base, long long i, const Rec& r) {
+    double2* d = reinterpret_cast<double2*>(base + i);
     const double2* s = reinterpret_cast<const double2*>(&r);
+    const int sw = (int)(i & 7);
 #pragma unroll
-    for (int i = 0; i < 7; ++i) d[i] = s[i];
+    for (int j = 0; j < 7; ++j) d[j ^ sw] = s[j];
 }
 
 // ============================================================================================ setup kernels
@@ -141,17 +147,14 @@ __global__ void k_bind(Rec* __restrict__ recs, long long first, long long cnt, c
     r.mu = mu[i]; r.p = p[i]; r.tri = -1; r.st = 0;
     r.id = (int)(first + i); r.pad0 = 0;
     r.pad[0] = r.pad[1] = 0.0;
-    double2* d = reinterpret_cast<double2*>(recs + first + i);
-    const double2* s = reinterpret_cast<const double2*>(&r);
-#pragma unroll
-    for (int q = 0; q < 8; ++q) d[q] = s[q];
+    rec_store(recs, first + i, r);
 }
 // records -> SoA arrays in the caller's order (any may be null)
 __global__ void k_get(const Rec* __restrict__ recs, long long n, double* R, double* Z, double* phi, double* u, double* w, int* status) {
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     Rec r;
-    rec_load(recs + i, r);
+    rec_load(recs, i, r);
     const long long o = r.id;
     if (R) R[o] = r.y[0];
     if (Z) Z[o] = r.y[1];
@@ -269,7 +272,7 @@ __device__ __forceinline__ bool phase_step(const TorP& tor, double dt, Rec& r, E
 __device__ __forceinline__ void store_rec(const DevTables& tb, const CellMap& cm, const KeyOut& ko, Rec* __restrict__ recs, long long ri,
                                           Rec& r, int t, const double next[3]) {
     r.tri = t;
-    rec_store(recs + ri, r);
+    rec_store(recs, ri, r);
     if (ko.enabled) {
         double sf;
         int k = toroidal_interval(tb.tor, next[2], sf);
@@ -285,7 +288,7 @@ template <int PHASE>
 __device__ __forceinline__ void phase_global(const DevTables& tb, const EquilP& ep, const SpeciesP& sp, const CellMap& cm, const KeyOut& ko,
                                              const Rec* __restrict__ src, Rec* __restrict__ dst, long long ri, long long m, double dt) {
     Rec r;
-    rec_load(src + ri, r);
+    rec_load(src, ri, r);
     int t = r.tri, st = r.st;
     const double mu = r.mu, p = r.p;
     auto eval = [&](const double y[5], double d[5]) {
@@ -317,7 +320,7 @@ __global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, Sp
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= n) return;
     Rec r;
-    rec_load(recs + m, r);
+    rec_load(recs, m, r);
     double y0[5], k[5], acc[5], y[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) y0[q] = r.y[q];
@@ -338,7 +341,7 @@ __global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, Sp
     for (int q = 0; q < 5; ++q) r.y[q] = fma(h6, acc[q] + k[q], y0[q]);
     r.y[2] = wrap_phi(tb.tor, r.y[2]);
     r.tri = t; r.st = st;
-    rec_store(recs + m, r);
+    rec_store(recs, m, r);
 }
 
 // the paper's own kernel boundary (L89): the five time derivatives at the current state, caller order
@@ -346,7 +349,7 @@ __global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP s
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= n) return;
     Rec r;
-    rec_load(recs + m, r);
+    rec_load(recs, m, r);
     int t = r.tri;
     double d[5];
     stage_simple(tb, ep, sp, t, r.y[0], r.y[1], r.y[2], r.y[3], r.y[4], r.mu, r.p, d);
@@ -436,6 +439,11 @@ __device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int
 
 // One phase of the RK4 step for the markers of one super-cell after another.  Position j of the cell order is record
 // src[perm[j]] (perm null: src[j]) and is written to dst[j].  Persistent: one CTA per SM, every warp runs on its own.
+// Per warp the work is software-pipelined over chunks of 32 markers:
+//   records of the NEXT chunk travel global -> shared by per-lane bulk copies (TMA) while the current chunk is computed,
+//   updated records travel registers -> shared -> global by per-lane bulk stores (no LSU wavefronts for 32 scattered lines).
+struct ChunkRef { int m0, end, b; unsigned it; };
+
 template <class C, int PHASE>
 __global__ void __launch_bounds__(C::NTHREADS, 1)
 k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __restrict__ src, Rec* __restrict__ dst, const int* __restrict__ perm,
@@ -444,6 +452,8 @@ k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     BlockCtrl* ctl_all = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL);
     unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF);
+    unsigned char* in_buf = smem + C::OFF_STAGE + (size_t)wid * 2 * C::WSTAGE;
+    unsigned char* out_buf = in_buf + C::WSTAGE;
     if (tid == 0) {
         for (int b = 0; b < C::NBUF; ++b) mbar_init(mbar_all + 2 * b, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -455,78 +465,170 @@ k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __
     const int P = tb.tor.P;
     constexpr unsigned FULL = 0xffffffffu;
 
-    // every warp walks the ring in the same order; the last warp to leave an entry refills it (no block-wide barrier)
-    for (unsigned it = 0;; ++it) {
-        const int b = it % C::NBUF;
-        mbar_wait(mbar_all + 2 * b, (it / C::NBUF) & 1);
-        BlockCtrl* ctl = ctl_all + b;
-        if (ctl->sc < 0) break;
-        const double* coef = reinterpret_cast<const double*>(smem + C::BLOCK_BYTES * b);
-        const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
-        const int end = ctl->end, patch = ctl->patch, k0 = ctl->k0, ns = ctl->ns;
-        int* sh_next = &ctl->next;
-
-        // ---- each warp grabs chunks of 32 markers until the super-cell is drained
+    // ---- ring bookkeeping (all warp-uniform).  acq_it: ring iteration the warp takes chunks from; leave_it: first iteration
+    // it has not left yet.  An entry is left once the warp will take no more chunks from it AND is not computing on it;
+    // the last warp to leave refills it.
+    unsigned acq_it = 0, leave_it = 0;
+    bool exhausted = false;
+    auto leave_upto = [&](unsigned upto) {   // leave every entry with iteration < upto
+        for (; leave_it < upto; ++leave_it) {
+            const int b = leave_it % C::NBUF;
+            BlockCtrl* ctl = ctl_all + b;
+            __syncwarp();
+            int last = 0;
+            if (lane == 0) { __threadfence_block(); last = atomicAdd(&ctl->left, 1) == C::NWARPS - 1; }
+            last = __shfl_sync(FULL, last, 0);
+            if (last) { __threadfence_block(); tile_refill<C>(smem, b, tb, tt, work_counter, lane); }
+        }
+    };
+    // take the next chunk.  hold >= 0: the warp still computes on ring iteration `hold`; it then looks at most NBUF - 1 entries
+    // ahead (an entry further on can only be refilled after this warp has left `hold`) and leaves nothing at or after `hold`.
+    // Returns 1 = got one, 0 = nothing within the look-ahead, -1 = no work left.
+    auto acquire = [&](ChunkRef& c, long long hold) -> int {
         for (;;) {
+            if (exhausted) return -1;
+            if (hold >= 0 && (long long)acq_it > hold + C::NBUF - 1) return 0;
+            const int b = acq_it % C::NBUF;
+            mbar_wait(mbar_all + 2 * b, (acq_it / C::NBUF) & 1);
+            BlockCtrl* ctl = ctl_all + b;
+            if (ctl->sc < 0) { exhausted = true; return -1; }
+            const int end = ctl->end;
             int chunk = 0;
-            if (lane == 0) chunk = atomicAdd(sh_next, 32);
+            if (lane == 0) chunk = atomicAdd(&ctl->next, 32);
             chunk = __shfl_sync(FULL, chunk, 0);
-            if (chunk >= end) break;
-            const int m = chunk + lane;
-            if (m < end) {
-                const long long ri = perm ? (long long)perm[m] : (long long)m;
-                Rec r;
-                rec_load(src + ri, r);
-                const double mu = r.mu, pw = r.p;
-                int st = r.st, cur = -1, tri_last = r.tri;
-                {
-                    int sl = tri_last - patch * C::TP;
-                    if (sl >= 0 && sl < C::TP) cur = sl;
-                    else {   // not sorted since it moved: look for the triangle in the halo
-                        for (int q = C::TP; q < ns; ++q) if (sgeom[q].tri == tri_last) { cur = q; break; }
-                    }
-                }
-                auto eval = [&](const double y[5], double d[5]) {
-                    double xi = 0.0, eta = 0.0, sf;
-                    const int sl = slot_walk(sgeom, cur, y[0], y[1], xi, eta);
-                    const int k = toroidal_interval(tb.tor, y[2], sf);
-                    int dk = k - k0;
-                    if (dk > P / 2) dk -= P; else if (dk < -(P / 2)) dk += P;
-                    const int lk = dk + C::HK;
-                    if (!(sl >= 0 && lk >= 0 && lk < C::NW)) return false;
-                    cur = sl;
-                    const SlotGeom& g = sgeom[sl];
-                    tri_last = g.tri;
-                    double w[4], dw[4], g8[8];
-                    bspline_from_s(tb.tor, sf, w, dw);
-                    LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
-                    gather_cell(ld, xi, eta, w, dw, g8);
-                    Fields fo;
-                    fo.P = g8[0]; fo.PR = fma(g.a11, g8[1], g.a21 * g8[2]); fo.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); fo.Pp = g8[3];
-                    fo.A = g8[4]; fo.AR = fma(g.a11, g8[5], g.a21 * g8[6]); fo.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); fo.Ap = g8[7];
-                    rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, fo, d);
-                    return true;
-                };
-                double next[3];
-                if (phase_step<PHASE>(tb.tor, dt, r, eval, next)) {
-                    // triangle of the next phase's first evaluation point: staged walk, else the global walk (rare)
-                    double xi, eta;
-                    const int sl = slot_walk(sgeom, cur, next[0], next[1], xi, eta);
-                    const int t = sl >= 0 ? sgeom[sl].tri : locate_walk(tb.bg, tb.geom, tri_last, next[0], next[1]);
-                    r.st = st;
-                    store_rec(tb, cm, ko, dst, m, r, t, next);
-                } else {
-                    rq.list[atomicAdd(rq.count, 1)] = m;   // the follow-up kernel redoes this phase through the global tables
-                }
+            if (chunk < end) { c.m0 = chunk; c.end = end; c.b = b; c.it = acq_it; return 1; }
+            ++acq_it;
+            leave_upto(hold >= 0 ? (unsigned)min((long long)acq_it, hold) : acq_it);
+        }
+    };
+    // start the record loads of chunk c into the warp's in-buffer: eight 16-byte cp.async per lane; a group of 8 lanes
+    // copies one whole record per instruction (4 lines per warp instruction instead of 32)
+    auto fetch = [&](const ChunkRef& c) {
+        const int nvalid = min(32, c.end - c.m0);
+        int pr = 0;
+        if (lane < nvalid) { const int m = c.m0 + lane; pr = perm ? perm[m] : m; }
+        const unsigned ib = smem_u32(in_buf);
+        const int ch = lane & 7, g = lane >> 3;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int R = 4 * k + g;
+            const int ri = __shfl_sync(FULL, pr, R);
+            if (R < nvalid) {
+                const unsigned d = ib + R * 128 + 16 * ((ch ^ (ri & 7)) ^ (R & 7));
+                const char* s = reinterpret_cast<const char*>(src + ri) + 16 * ch;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(s) : "memory");
             }
         }
-        // leave the entry; the last warp out refills it with the next super-cell
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    ChunkRef cur, nxt;
+    int have = acquire(cur, -1);
+    if (have == 1) fetch(cur);
+    while (have == 1) {
+        // ---- records of the current chunk: shared -> registers
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncwarp();
-        int last = 0;
-        if (lane == 0) { __threadfence_block(); last = atomicAdd(&ctl->left, 1) == C::NWARPS - 1; }
-        last = __shfl_sync(FULL, last, 0);
-        if (last) { __threadfence_block(); tile_refill<C>(smem, b, tb, tt, work_counter, lane); }
+        const int m = cur.m0 + lane;
+        const bool valid = m < cur.end;
+        Rec r;
+        if (valid) {
+            const unsigned a = smem_u32(in_buf) + lane * 128;
+            double* rd = reinterpret_cast<double*>(&r);
+#pragma unroll
+            for (int j = 0; j < 7; ++j) lds128(a + 16 * (j ^ (lane & 7)), rd[2 * j], rd[2 * j + 1]);
+        }
+        __syncwarp();   // every lane has its record in registers before the next chunk's copies may land
+        // ---- next chunk: take it and start its loads (at most one ring entry ahead of the one being computed on)
+        int have_next = acquire(nxt, (long long)cur.it);
+        if (have_next == 1) fetch(nxt);
+
+        // ---- compute
+        const double* coef = reinterpret_cast<const double*>(smem + C::BLOCK_BYTES * cur.b);
+        const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * cur.b + C::COEF_BYTES);
+        const BlockCtrl* ctl = ctl_all + cur.b;
+        const int patch = ctl->patch, k0 = ctl->k0, ns = ctl->ns;
+        // the previous chunk's bulk store must have read the out-buffer before it is overwritten
+        if (lane == 0) bulk_wait_read0();
+        __syncwarp();
+        if (valid) {
+            const double mu = r.mu, pw = r.p;
+            int st = r.st, slot = -1, tri_last = r.tri;
+            {
+                int sl = tri_last - patch * C::TP;
+                if (sl >= 0 && sl < C::TP) slot = sl;
+                else {   // not sorted since it moved: look for the triangle in the halo
+                    for (int q = C::TP; q < ns; ++q) if (sgeom[q].tri == tri_last) { slot = q; break; }
+                }
+            }
+            auto eval = [&](const double y[5], double d[5]) {
+                double xi = 0.0, eta = 0.0, sf;
+                const int sl = slot_walk(sgeom, slot, y[0], y[1], xi, eta);
+                const int k = toroidal_interval(tb.tor, y[2], sf);
+                int dk = k - k0;
+                if (dk > P / 2) dk -= P; else if (dk < -(P / 2)) dk += P;
+                const int lk = dk + C::HK;
+                if (!(sl >= 0 && lk >= 0 && lk < C::NW)) return false;
+                slot = sl;
+                const SlotGeom& g = sgeom[sl];
+                tri_last = g.tri;
+                double w[4], dw[4], g8[8];
+                bspline_from_s(tb.tor, sf, w, dw);
+                LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
+                gather_cell(ld, xi, eta, w, dw, g8);
+                Fields fo;
+                fo.P = g8[0]; fo.PR = fma(g.a11, g8[1], g.a21 * g8[2]); fo.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); fo.Pp = g8[3];
+                fo.A = g8[4]; fo.AR = fma(g.a11, g8[5], g.a21 * g8[6]); fo.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); fo.Ap = g8[7];
+                rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, fo, d);
+                return true;
+            };
+            double next[3];
+            if (phase_step<PHASE>(tb.tor, dt, r, eval, next)) {
+                // triangle of the next phase's first evaluation point: staged walk, else the global walk (rare)
+                double xi, eta;
+                const int sl = slot_walk(sgeom, slot, next[0], next[1], xi, eta);
+                const int t = sl >= 0 ? sgeom[sl].tri : locate_walk(tb.bg, tb.geom, tri_last, next[0], next[1]);
+                r.st = st; r.tri = t;
+                if (ko.enabled) {
+                    double sf;
+                    const int k = toroidal_interval(tb.tor, next[2], sf);
+                    const int key = t < 0 ? ko.ncell : cm.cell(t, k);
+                    ko.keys[m] = key;
+                    atomicAdd(ko.hist + key, 1);
+                }
+            } else {
+                // the follow-up kernel redoes this phase through the global tables; r is unchanged and goes to dst[m] as it
+                // is (when the phase works in place dst[m] is also what the follow-up kernel reads)
+                rq.list[atomicAdd(rq.count, 1)] = m;
+            }
+            // registers -> the warp's out-buffer, in the swizzle of the record's position in dst
+            const unsigned a = smem_u32(out_buf) + lane * 128;
+            const double* rs = reinterpret_cast<const double*>(&r);
+#pragma unroll
+            for (int j = 0; j < 7; ++j) sts128(a + 16 * (j ^ (m & 7)), rs[2 * j], rs[2 * j + 1]);
+        }
+        // the chunk's records leave as one bulk copy
+        fence_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+            tma_bulk_s2g(dst + cur.m0, out_buf, (unsigned)(min(32, cur.end - cur.m0) * 128));
+            bulk_commit();
+        }
+        // ---- done computing on cur.it: leave every entry the warp is through with
+        if (have_next == 1) {
+            leave_upto(nxt.it);
+            cur = nxt;
+            have = 1;
+        } else {
+            leave_upto(cur.it + 1);
+            if (have_next == 0) {   // nothing within the look-ahead limit: look again now that the entry is left
+                have = acquire(cur, -1);
+                if (have == 1) fetch(cur);
+            } else have = -1;
+        }
     }
+    // leave whatever is still held so that the ring drains for the other warps (entries up to the terminating one)
+    leave_upto(acq_it);
+    if (lane == 0) bulk_wait0();
 }
 
 // ============================================================================================ counting sort by cell

@@ -43,7 +43,11 @@ struct TileCfg {
     static constexpr size_t COEF_BYTES = sizeof(double) * SMAX * SLOT_DOUBLES;
     static constexpr size_t BLOCK_BYTES = COEF_BYTES + 64 * SMAX;
     static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;
-    static constexpr size_t BYTES = OFF_CTRL + 64 * NBUF + 16 * NBUF;
+    static constexpr size_t OFF_WBAR = OFF_CTRL + 64 * NBUF + 16 * NBUF;          // one mbarrier per warp (record loads)
+    // per-warp marker staging: 32 records in (cp.async), 32 records out (one bulk store), 128 B each, XOR-swizzled rows
+    static constexpr size_t WSTAGE = 32 * 128;
+    static constexpr size_t OFF_STAGE = (OFF_WBAR + 8 * NWARPS + 127) / 128 * 128;
+    static constexpr size_t BYTES = OFF_STAGE + 2 * WSTAGE * NWARPS;
 };
 struct BlockCtrl {   // 64 B per ring entry
     int sc, begin, end, next, left, ns, patch, k0;
@@ -72,7 +76,20 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigne
                  "r"(smem_u32(bar))
                  : "memory");
 }
-__device__ __forceinline__ void group_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+// 16 <= bytes, multiple of 16; completion is tracked by the issuing thread's bulk async-group
+__device__ __forceinline__ void tma_bulk_s2g(void* dst, const void* src, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void lds128(unsigned addr, double& a, double& b) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "r"(addr));
+}
+__device__ __forceinline__ void sts128(unsigned addr, double a, double b) {
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(a), "d"(b) : "memory");
+}
 
 struct LdShared {   // coefficient pair fetch from the staged block
     unsigned base;  // shared-space byte address of the cell's first plane
