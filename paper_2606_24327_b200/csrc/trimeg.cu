@@ -433,7 +433,7 @@ static int run_phase(trimeg_ctx* ctx, double dt, bool sort_now, bool keys_out, c
     Rec* dst = ctx->recs[sort_now ? ctx->cur ^ 1 : ctx->cur];
     const int* perm = sort_now ? ctx->d_perm : nullptr;
     if (ev) CU(cudaEventRecord(ev[0], ctx->stream));
-    k_phase_tiled<Tile, PHASE><<<ctx->num_sms, Tile::NTHREADS, Tile::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, src, dst, perm, rq, ko, ctx->cm, dt,
+    k_phase_tiled<Tile, PHASE><<<ctx->num_sms * TRIMEG_CTAS_PER_SM, Tile::NTHREADS, Tile::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, src, dst, perm, rq, ko, ctx->cm, dt,
                                                                                            ctx->d_work);
     KCHECK();
     if (ev) CU(cudaEventRecord(ev[1], ctx->stream));

@@ -36,8 +36,20 @@ struct DevTables {
 };
 
 // tiled push configuration: patches of 8 triangles + halo (16 slots), windows of 4 toroidal intervals (+1 each side),
-// ring of 2 staged blocks, 16 independent warps per CTA, one CTA per SM
-using Tile = TileCfg<8, 16, 4, 16>;
+// ring of 3 staged blocks, 16 independent warps per CTA, one CTA per SM
+#ifndef TRIMEG_SMAX
+#define TRIMEG_SMAX 16
+#endif
+#ifndef TRIMEG_NWARPS
+#define TRIMEG_NWARPS 16
+#endif
+#ifndef TRIMEG_NBUF
+#define TRIMEG_NBUF 3
+#endif
+#ifndef TRIMEG_CTAS_PER_SM
+#define TRIMEG_CTAS_PER_SM 1
+#endif
+using Tile = TileCfg<8, TRIMEG_SMAX, 4, TRIMEG_NWARPS, TRIMEG_NBUF>;
 // cell numbering used by the sort: super-cell (patch, window) major, then triangle within the patch, then interval
 struct CellMap {
     int P, nwin;
@@ -58,9 +70,8 @@ __constant__ double c_Aplus[21 * 18];
 __constant__ double c_Nul[21 * 3];
 
 // In memory the eight 16-byte chunks of record i are stored XOR-swizzled by (i & 7): logical chunk j sits at chunk
-// position j ^ (i & 7).  With that the tiled kernel's shared-memory image of 32 consecutive records (row stride 128 B) is
-// at once bank-conflict free for per-lane 16-byte accesses and the verbatim image of the records in global memory, so a
-// chunk of 32 updated records leaves the SM as ONE 4-KB bulk copy.
+// position j ^ (i & 7) (a record is only ever handled whole, so the swizzle costs nothing; it lets row-per-lane shared-memory
+// images of records be read and written 16 bytes per lane without bank conflicts).
 __device__ __forceinline__ void rec_load(const Rec* __restrict__ base, long long i, Rec& r) {
     const double2* s = reinterpret_cast<const double2*>(base + i);
     double2* d = reinterpret_cast<double2*>(&r);
@@ -445,15 +456,14 @@ __device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int
 struct ChunkRef { int m0, end, b; unsigned it; };
 
 template <class C, int PHASE>
-__global__ void __launch_bounds__(C::NTHREADS, 1)
+__global__ void __launch_bounds__(C::NTHREADS, TRIMEG_CTAS_PER_SM)
 k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __restrict__ src, Rec* __restrict__ dst, const int* __restrict__ perm,
               RetireList rq, KeyOut ko, CellMap cm, double dt, int* __restrict__ work_counter) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     BlockCtrl* ctl_all = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL);
     unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF);
-    unsigned char* in_buf = smem + C::OFF_STAGE + (size_t)wid * 2 * C::WSTAGE;
-    unsigned char* out_buf = in_buf + C::WSTAGE;
+    unsigned char* in_buf = smem + C::OFF_STAGE + (size_t)wid * C::WSTAGE;
     if (tid == 0) {
         for (int b = 0; b < C::NBUF; ++b) mbar_init(mbar_all + 2 * b, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -547,9 +557,6 @@ k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __
         const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * cur.b + C::COEF_BYTES);
         const BlockCtrl* ctl = ctl_all + cur.b;
         const int patch = ctl->patch, k0 = ctl->k0, ns = ctl->ns;
-        // the previous chunk's bulk store must have read the out-buffer before it is overwritten
-        if (lane == 0) bulk_wait_read0();
-        __syncwarp();
         if (valid) {
             const double mu = r.mu, pw = r.p;
             int st = r.st, slot = -1, tri_last = r.tri;
@@ -582,12 +589,22 @@ k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __
                 return true;
             };
             double next[3];
+#ifdef TRIMEG_EXP_NOEVAL
+            next[0] = r.y[0]; next[1] = r.y[1]; next[2] = r.y[2];
+            if (r.y[0] > -1e300) {
+#else
             if (phase_step<PHASE>(tb.tor, dt, r, eval, next)) {
+#endif
                 // triangle of the next phase's first evaluation point: staged walk, else the global walk (rare)
                 double xi, eta;
                 const int sl = slot_walk(sgeom, slot, next[0], next[1], xi, eta);
                 const int t = sl >= 0 ? sgeom[sl].tri : locate_walk(tb.bg, tb.geom, tri_last, next[0], next[1]);
                 r.st = st; r.tri = t;
+#ifndef TRIMEG_EXP_NOSTORE
+                rec_store(dst, m, r);
+#else
+                if (r.y[0] == 1.2345e-200) rec_store(dst, m, r);
+#endif
                 if (ko.enabled) {
                     double sf;
                     const int k = toroidal_interval(tb.tor, next[2], sf);
@@ -596,22 +613,9 @@ k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __
                     atomicAdd(ko.hist + key, 1);
                 }
             } else {
-                // the follow-up kernel redoes this phase through the global tables; r is unchanged and goes to dst[m] as it
-                // is (when the phase works in place dst[m] is also what the follow-up kernel reads)
+                // the follow-up kernel redoes this phase through the global tables, reading src again and writing dst[m]
                 rq.list[atomicAdd(rq.count, 1)] = m;
             }
-            // registers -> the warp's out-buffer, in the swizzle of the record's position in dst
-            const unsigned a = smem_u32(out_buf) + lane * 128;
-            const double* rs = reinterpret_cast<const double*>(&r);
-#pragma unroll
-            for (int j = 0; j < 7; ++j) sts128(a + 16 * (j ^ (m & 7)), rs[2 * j], rs[2 * j + 1]);
-        }
-        // the chunk's records leave as one bulk copy
-        fence_async_smem();
-        __syncwarp();
-        if (lane == 0) {
-            tma_bulk_s2g(dst + cur.m0, out_buf, (unsigned)(min(32, cur.end - cur.m0) * 128));
-            bulk_commit();
         }
         // ---- done computing on cur.it: leave every entry the warp is through with
         if (have_next == 1) {
@@ -628,7 +632,6 @@ k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __
     }
     // leave whatever is still held so that the ring drains for the other warps (entries up to the terminating one)
     leave_upto(acq_it);
-    if (lane == 0) bulk_wait0();
 }
 
 // ============================================================================================ counting sort by cell

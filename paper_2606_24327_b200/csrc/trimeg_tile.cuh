@@ -31,23 +31,23 @@ struct TileTables {
     int npatch, nwin, nsc;   // super-cells = npatch * nwin
 };
 
-template <int TP_, int SMAX_, int WK_, int NWARPS_>
+template <int TP_, int SMAX_, int WK_, int NWARPS_, int NBUF_>
 struct TileCfg {
     static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD, NWARPS = NWARPS_, NTHREADS = 32 * NWARPS_;
     static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
     static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
     static constexpr int CPS = TP * WK;              // cells per super-cell
     static constexpr int SLOT_DOUBLES = NPL * PLANE_STRIDE;
-    static constexpr int NBUF = 2;                   // ring of staged blocks
+    static constexpr int NBUF = NBUF_;               // ring of staged blocks
     // shared memory carve-up (bytes): NBUF x { coefficients, slot geometry }, then the control words
     static constexpr size_t COEF_BYTES = sizeof(double) * SMAX * SLOT_DOUBLES;
     static constexpr size_t BLOCK_BYTES = COEF_BYTES + 64 * SMAX;
     static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;
     static constexpr size_t OFF_WBAR = OFF_CTRL + 64 * NBUF + 16 * NBUF;          // one mbarrier per warp (record loads)
-    // per-warp marker staging: 32 records in (cp.async), 32 records out (one bulk store), 128 B each, XOR-swizzled rows
+    // per-warp marker staging: the 32 records of the next chunk (cp.async), 128 B each, XOR-swizzled rows
     static constexpr size_t WSTAGE = 32 * 128;
     static constexpr size_t OFF_STAGE = (OFF_WBAR + 8 * NWARPS + 127) / 128 * 128;
-    static constexpr size_t BYTES = OFF_STAGE + 2 * WSTAGE * NWARPS;
+    static constexpr size_t BYTES = OFF_STAGE + WSTAGE * NWARPS;
 };
 struct BlockCtrl {   // 64 B per ring entry
     int sc, begin, end, next, left, ns, patch, k0;
