@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtrimeg_b200.so")
 SOURCES = ["trimeg.cu"]
-DEPS = ["trimeg.cu", "trimeg_kernels.cuh", "trimeg_math.cuh", "trimeg_host_setup.hpp", "trimeg_tile.cuh", "../../include/trimeg.h"]
+DEPS = ["trimeg.cu", "trimeg_kernels.cuh", "trimeg_ws.cuh", "trimeg_math.cuh", "trimeg_host_setup.hpp", "trimeg_tile.cuh", "../../include/trimeg.h"]
 EXTRA_DEFS = os.environ.get("TRIMEG_DEFS", "").split()
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false".replace("=false", "")][:-1]

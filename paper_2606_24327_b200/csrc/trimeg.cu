@@ -242,8 +242,8 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     CU(cudaMemsetAsync(ctx->d_fill, 0, sizeof(int) * ncnt, ctx->stream));
     ctx->tt.slots = ctx->d_pslots; ctx->tt.nbr = ctx->d_pnbr; ctx->tt.nslots = ctx->d_pnslots; ctx->tt.offs = ctx->d_offs;
     ctx->tt.npatch = hp.npatch; ctx->tt.nwin = nwin; ctx->tt.nsc = hp.npatch * nwin;
-    CU(cudaFuncSetAttribute(k_phase_tiled<Tile, PHASE_A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tile::BYTES));
-    CU(cudaFuncSetAttribute(k_phase_tiled<Tile, PHASE_B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tile::BYTES));
+    CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WsLayout<Tile>::BYTES));
+    CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WsLayout<Tile>::BYTES));
     CU(cudaMemcpyAsync(ctx->d_geom, geom.data(), sizeof(TriGeom) * T, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_tri, hm.tri.data(), sizeof(int) * 3 * T, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_head, hm.head.data(), sizeof(int) * hm.head.size(), cudaMemcpyHostToDevice, ctx->stream));
@@ -433,7 +433,7 @@ static int run_phase(trimeg_ctx* ctx, double dt, bool sort_now, bool keys_out, c
     Rec* dst = ctx->recs[sort_now ? ctx->cur ^ 1 : ctx->cur];
     const int* perm = sort_now ? ctx->d_perm : nullptr;
     if (ev) CU(cudaEventRecord(ev[0], ctx->stream));
-    k_phase_tiled<Tile, PHASE><<<ctx->num_sms * TRIMEG_CTAS_PER_SM, Tile::NTHREADS, Tile::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, src, dst, perm, rq, ko, ctx->cm, dt,
+    k_phase_ws<Tile, PHASE><<<ctx->num_sms, Tile::NTHREADS, WsLayout<Tile>::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, src, dst, perm, rq, ko, ctx->cm, dt,
                                                                                            ctx->d_work);
     KCHECK();
     if (ev) CU(cudaEventRecord(ev[1], ctx->stream));

@@ -245,36 +245,36 @@ enum { PHASE_A = 0, PHASE_B = 1, PHASE_INIT = 2 };
 template <int PHASE, class Eval>
 __device__ __forceinline__ bool phase_step(const TorP& tor, double dt, Rec& r, Eval&& eval, double next[3]) {
     const double h2 = 0.5 * dt, h6 = dt / 6.0;
-    double a[5], b[5], y[5];
+    double a[5], d[5], y[5];
+    // first evaluation point: A: y_n + dt/2 k1;  B: y4;  INIT: (none, only the second evaluation, at y_n)
+#pragma unroll
+    for (int q = 0; q < 5; ++q) y[q] = PHASE == PHASE_A ? fma(h2, r.k[q], r.y[q]) : (PHASE == PHASE_B ? r.k[q] : r.y[q]);
+    // the two evaluations run through ONE copy of the evaluation code (a rolled loop): the kernel body then fits the
+    // instruction cache, which two inlined copies did not (profiles/r01c_summary.md, stall_no_instruction)
+#pragma unroll 1
+    for (int e = (PHASE == PHASE_INIT ? 1 : 0); e < 2; ++e) {
+        if (!eval(y, d)) return false;
+        if (e == 0) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+                a[q] = d[q];                                                            // A: k2;  B: k4
+                y[q] = PHASE == PHASE_A ? fma(h2, d[q], r.y[q]) : fma(h6, d[q], r.y[q]);  // A: y_n + dt/2 k2;  B: y_{n+1}
+            }
+            if (PHASE == PHASE_B) y[2] = wrap_phi(tor, y[2]);
+        }
+    }
     if (PHASE == PHASE_A) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) y[q] = fma(h2, r.k[q], r.y[q]);
-        if (!eval(y, a)) return false;                                  // k2
-#pragma unroll
-        for (int q = 0; q < 5; ++q) y[q] = fma(h2, a[q], r.y[q]);
-        if (!eval(y, b)) return false;                                  // k3
-#pragma unroll
         for (int q = 0; q < 5; ++q) {
-            double acc = fma(2.0, b[q], fma(2.0, a[q], r.k[q]));
-            double y0 = r.y[q];
-            r.y[q] = fma(h6, acc, y0);                                  // Y
-            r.k[q] = fma(dt, b[q], y0);                                 // y4
+            const double acc = fma(2.0, d[q], fma(2.0, a[q], r.k[q])), y0 = r.y[q];
+            r.y[q] = fma(h6, acc, y0);                                                  // Y
+            r.k[q] = fma(dt, d[q], y0);                                                 // y4 = y_n + dt k3
         }
         next[0] = r.k[0]; next[1] = r.k[1]; next[2] = r.k[2];
     } else {
-        if (PHASE == PHASE_B) {
-            if (!eval(r.k, a)) return false;                            // k4
 #pragma unroll
-            for (int q = 0; q < 5; ++q) y[q] = fma(h6, a[q], r.y[q]);   // y_{n+1}
-            y[2] = wrap_phi(tor, y[2]);
-        } else {
-#pragma unroll
-            for (int q = 0; q < 5; ++q) y[q] = r.y[q];
-        }
-        if (!eval(y, b)) return false;                                  // k1 of the next step
-#pragma unroll
-        for (int q = 0; q < 5; ++q) { r.y[q] = y[q]; r.k[q] = b[q]; }
-        next[0] = fma(h2, b[0], y[0]); next[1] = fma(h2, b[1], y[1]); next[2] = fma(h2, b[2], y[2]);
+        for (int q = 0; q < 5; ++q) { r.y[q] = y[q]; r.k[q] = d[q]; }                  // y_{n+1} (INIT: y_n), k1 = f(it)
+        next[0] = fma(h2, d[0], y[0]); next[1] = fma(h2, d[1], y[1]); next[2] = fma(h2, d[2], y[2]);
     }
     return true;
 }
@@ -633,6 +633,10 @@ k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __
     // leave whatever is still held so that the ring drains for the other warps (entries up to the terminating one)
     leave_upto(acq_it);
 }
+
+}  // namespace trimeg
+#include "trimeg_ws.cuh"
+namespace trimeg {
 
 // ============================================================================================ counting sort by cell
 // exclusive scan of int counts, three passes over chunks of SCAN_CHUNK

@@ -1,0 +1,261 @@
+// Warp-specialised phase kernel (included by trimeg_kernels.cuh after the tile helpers).
+//
+// Measured on the plain tiled kernel (profiles/r01c_summary.md): with 16 warps per SM every warp spent more time in the
+// per-chunk skeleton (ring waits, permutation load, record copies, block refills: 8.7 ms per pass with the arithmetic
+// compiled out) than in the arithmetic itself (6.6 ms), and the two added up instead of overlapping.  Here the skeleton
+// is taken off the compute warps:
+//   warp 0  "stager"    : takes super-cells off the work list, waits until a ring entry is free, fills it (slot geometry
+//                         + TMA bulk copies of the coefficient blocks);
+//   warp 1  "publisher" : once an entry has landed, cuts its marker range into chunks of 32 and, for each, copies the
+//                         32 records into a free chunk slot (cp.async through the sort permutation; completion is
+//                         signalled on the slot's mbarrier by cp.async.mbarrier.arrive);
+//   warps 2.. "compute" : take chunk slots in ticket order, pull their record into registers, free the slot, evaluate
+//                         the phase, store the record, and count the chunk done on its ring entry.
+// A ring entry is refilled when all chunks cut from it are done, not when every warp has walked past it.
+#pragma once
+
+namespace trimeg {
+
+struct ChunkDesc { int m0, end, b, pad; };   // m0 < 0: no more work
+
+template <class C>
+struct WsLayout {
+    static constexpr int K = C::NWARPS;                                  // chunk slots (4 KB each, in the staging area)
+    static constexpr int NCONS = C::NWARPS - 2;
+    static constexpr size_t OFF_DESC = C::OFF_STAGE + C::WSTAGE * C::NWARPS;
+    static constexpr size_t OFF_FULL = OFF_DESC + 16 * K;
+    static constexpr size_t OFF_EMPTY = OFF_FULL + 8 * K;
+    static constexpr size_t OFF_HEAD = OFF_EMPTY + 8 * K;
+    static constexpr size_t BYTES = OFF_HEAD + 64;
+};
+
+__device__ __forceinline__ void mbar_arrive(void* bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory"); }
+
+// stager: fill ring entry b with the next non-empty super-cell (whole warp).  Returns false when the work list is
+// exhausted (the entry then carries sc = -1 and its barrier completes at once).
+template <class C>
+__device__ __forceinline__ bool ws_stage(unsigned char* smem, int b, const DevTables& tb, const TileTables& tt, int* work_counter, int lane) {
+    constexpr unsigned FULL = 0xffffffffu;
+    double* coef = reinterpret_cast<double*>(smem + C::BLOCK_BYTES * b);
+    SlotGeom* sgeom = reinterpret_cast<SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
+    BlockCtrl* ctl = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL) + b;
+    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF) + 2 * b;
+    int sc = 0, begin = 0, end = 0;
+    for (;;) {
+        if (lane == 0) sc = atomicAdd(work_counter, 1);
+        sc = __shfl_sync(FULL, sc, 0);
+        if (sc >= tt.nsc) { sc = -1; break; }
+        begin = tt.offs[(long long)sc * C::CPS]; end = tt.offs[(long long)(sc + 1) * C::CPS];
+        if (begin != end) break;
+    }
+    if (sc < 0) {
+        if (lane == 0) { ctl->sc = -1; __threadfence_block(); mbar_arrive(mbar); }
+        return false;
+    }
+    const int patch = sc / tt.nwin, k0 = (sc - patch * tt.nwin) * C::WK;
+    const int ns = tt.nslots[patch];
+    const int* pslots = tt.slots + (long long)patch * C::SMAX;
+    if (lane == 0) {
+        ctl->sc = sc; ctl->begin = begin; ctl->end = end; ctl->next = begin; ctl->ns = ns; ctl->patch = patch; ctl->k0 = k0;
+        ctl->pad[0] = (end - begin + 31) >> 5;                        // chunks that will be cut from this entry
+        *reinterpret_cast<volatile int*>(&ctl->left) = 0;             // chunks done
+    }
+    int cnt = 0;
+    for (int sl = lane; sl < ns; sl += 32) {
+        int t = pslots[sl];
+        SlotGeom g;
+        if (t >= 0) {
+            const TriGeom tg = tb.geom[t];
+            g.v0x = tg.v0x; g.v0y = tg.v0y; g.a11 = tg.a11; g.a12 = tg.a12; g.a21 = tg.a21; g.a22 = tg.a22;
+            const short* nb = tt.nbr + ((long long)patch * C::SMAX + sl) * 4;
+            g.nbr[0] = nb[0]; g.nbr[1] = nb[1]; g.nbr[2] = nb[2]; g.nbr[3] = -1;
+            cnt++;
+        } else {
+            g.v0x = g.v0y = 1e300; g.a11 = g.a12 = g.a21 = g.a22 = 0.0; g.nbr[0] = g.nbr[1] = g.nbr[2] = g.nbr[3] = -1;
+        }
+        g.tri = t; g.pad = 0;
+        sgeom[sl] = g;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(FULL, cnt, o);
+    __threadfence_block();
+    fence_async_smem();   // earlier generic accesses of this block vs. the async writes
+    __syncwarp();
+    if (lane == 0) mbar_expect_tx(mbar, (unsigned)(cnt * C::SLOT_DOUBLES * sizeof(double)));
+    __syncwarp();
+    for (int sl = lane; sl < ns; sl += 32) {
+        int t = pslots[sl];
+        if (t >= 0)
+            tma_bulk_g2s(coef + (size_t)sl * C::SLOT_DOUBLES, tb.coef + (long long)t * tb.tri_stride + (long long)k0 * PLANE_STRIDE,
+                         (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
+    }
+    return true;
+}
+
+template <class C, int PHASE>
+__global__ void __launch_bounds__(C::NTHREADS, 1)
+k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __restrict__ src, Rec* __restrict__ dst, const int* __restrict__ perm,
+           RetireList rq, KeyOut ko, CellMap cm, double dt, int* __restrict__ work_counter) {
+    using L = WsLayout<C>;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    BlockCtrl* ctl_all = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL);
+    unsigned long long* blk_bar = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF);   // stride 2
+    ChunkDesc* desc = reinterpret_cast<ChunkDesc*>(smem + L::OFF_DESC);
+    unsigned long long* full_bar = reinterpret_cast<unsigned long long*>(smem + L::OFF_FULL);
+    unsigned long long* empty_bar = reinterpret_cast<unsigned long long*>(smem + L::OFF_EMPTY);
+    int* cons_head = reinterpret_cast<int*>(smem + L::OFF_HEAD);
+    constexpr unsigned FULL = 0xffffffffu;
+    if (tid == 0) {
+        for (int b = 0; b < C::NBUF; ++b) mbar_init(blk_bar + 2 * b, 1);
+        for (int s = 0; s < L::K; ++s) { mbar_init(full_bar + s, 32); mbar_init(empty_bar + s, 1); }
+        *cons_head = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (wid == 0) {
+        // ------------------------------------------------------------------ stager
+        for (unsigned it = 0;; ++it) {
+            const int b = it % C::NBUF;
+            if (it >= (unsigned)C::NBUF) {   // previous occupant: all chunks cut from it are done
+                BlockCtrl* ctl = ctl_all + b;
+                if (lane == 0) {
+                    const int need = ctl->pad[0];
+                    while (*reinterpret_cast<volatile int*>(&ctl->left) < need) __nanosleep(64);
+                }
+                __syncwarp();
+            }
+            if (!ws_stage<C>(smem, b, tb, tt, work_counter, lane)) break;
+        }
+    } else if (wid == 1) {
+        // ------------------------------------------------------------------ publisher
+        unsigned ticket = 0;
+        auto slot_acquire = [&](unsigned t) {   // wait until the previous user of the slot has pulled its records out
+            const unsigned s = t % L::K, g = t / L::K;
+            if (g >= 1) mbar_wait(empty_bar + s, (g - 1) & 1);
+            return (int)s;
+        };
+        for (unsigned it = 0;; ++it) {
+            const int b = it % C::NBUF;
+            mbar_wait(blk_bar + 2 * b, (it / C::NBUF) & 1);
+            const BlockCtrl* ctl = ctl_all + b;
+            if (ctl->sc < 0) break;
+            const int begin = ctl->begin, end = ctl->end;
+            int pr_next = 0;
+            if (begin + lane < end) pr_next = perm ? perm[begin + lane] : begin + lane;
+            for (int c0 = begin; c0 < end; c0 += 32, ++ticket) {
+                const int pr = pr_next;
+                const int n0 = c0 + 32 + lane;
+                if (n0 < end) pr_next = perm ? perm[n0] : n0;      // next chunk's permutation entries: in flight during this one
+                const int s = slot_acquire(ticket);
+                if (lane == 0) { desc[s].m0 = c0; desc[s].end = end; desc[s].b = b; __threadfence_block(); }
+                __syncwarp();
+                const int nvalid = min(32, end - c0);
+                const unsigned ib = smem_u32(smem + C::OFF_STAGE + (size_t)s * C::WSTAGE);
+                const int ch = lane & 7, g = lane >> 3;
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int R = 4 * k + g;
+                    const int ri = __shfl_sync(FULL, pr, R);
+                    if (R < nvalid) {
+                        const unsigned d = ib + R * 128 + 16 * ((ch ^ (ri & 7)) ^ (R & 7));
+                        const char* gp = reinterpret_cast<const char*>(src + ri) + 16 * ch;
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gp) : "memory");
+                    }
+                }
+                asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(full_bar + s)) : "memory");
+            }
+        }
+        // one end-of-work ticket per compute warp
+        for (int q = 0; q < L::NCONS; ++q, ++ticket) {
+            const int s = slot_acquire(ticket);
+            if (lane == 0) { desc[s].m0 = -1; __threadfence_block(); }
+            __syncwarp();
+            mbar_arrive(full_bar + s);
+        }
+    } else {
+        // ------------------------------------------------------------------ compute warps
+        const int P = tb.tor.P;
+        for (;;) {
+            unsigned t = 0;
+            if (lane == 0) t = (unsigned)atomicAdd(cons_head, 1);
+            t = __shfl_sync(FULL, t, 0);
+            const unsigned s = t % L::K, g = t / L::K;
+            mbar_wait(full_bar + s, g & 1);
+            const int m0 = desc[s].m0, end = desc[s].end, b = desc[s].b;
+            if (m0 < 0) break;
+            const int m = m0 + lane;
+            const bool valid = m < end;
+            Rec r;
+            if (valid) {
+                const unsigned a = smem_u32(smem + C::OFF_STAGE + (size_t)s * C::WSTAGE) + lane * 128;
+                double* rd = reinterpret_cast<double*>(&r);
+#pragma unroll
+                for (int j = 0; j < 7; ++j) lds128(a + 16 * (j ^ (lane & 7)), rd[2 * j], rd[2 * j + 1]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar + s);   // the slot may be refilled
+
+            const double* coef = reinterpret_cast<const double*>(smem + C::BLOCK_BYTES * b);
+            const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
+            BlockCtrl* ctl = ctl_all + b;
+            const int patch = ctl->patch, k0 = ctl->k0, ns = ctl->ns;
+            if (valid) {
+                const double mu = r.mu, pw = r.p;
+                int st = r.st, slot = -1, tri_last = r.tri;
+                {
+                    int sl = tri_last - patch * C::TP;
+                    if (sl >= 0 && sl < C::TP) slot = sl;
+                    else {   // not sorted since it moved: look for the triangle in the halo
+                        for (int q = C::TP; q < ns; ++q) if (sgeom[q].tri == tri_last) { slot = q; break; }
+                    }
+                }
+                auto eval = [&](const double y[5], double d[5]) {
+                    double xi = 0.0, eta = 0.0, sf;
+                    const int sl = slot_walk(sgeom, slot, y[0], y[1], xi, eta);
+                    const int k = toroidal_interval(tb.tor, y[2], sf);
+                    int dk = k - k0;
+                    if (dk > P / 2) dk -= P; else if (dk < -(P / 2)) dk += P;
+                    const int lk = dk + C::HK;
+                    if (!(sl >= 0 && lk >= 0 && lk < C::NW)) return false;
+                    slot = sl;
+                    const SlotGeom& gg = sgeom[sl];
+                    tri_last = gg.tri;
+                    double w[4], dw[4], g8[8];
+                    bspline_from_s(tb.tor, sf, w, dw);
+                    LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
+                    gather_cell(ld, xi, eta, w, dw, g8);
+                    Fields fo;
+                    fo.P = g8[0]; fo.PR = fma(gg.a11, g8[1], gg.a21 * g8[2]); fo.PZ = fma(gg.a12, g8[1], gg.a22 * g8[2]); fo.Pp = g8[3];
+                    fo.A = g8[4]; fo.AR = fma(gg.a11, g8[5], gg.a21 * g8[6]); fo.AZ = fma(gg.a12, g8[5], gg.a22 * g8[6]); fo.Ap = g8[7];
+                    rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, fo, d);
+                    return true;
+                };
+                double next[3];
+                if (phase_step<PHASE>(tb.tor, dt, r, eval, next)) {
+                    // triangle of the next phase's first evaluation point: staged walk, else the global walk
+                    double xi, eta;
+                    const int sl = slot_walk(sgeom, slot, next[0], next[1], xi, eta);
+                    const int tn = sl >= 0 ? sgeom[sl].tri : locate_walk(tb.bg, tb.geom, tri_last, next[0], next[1]);
+                    r.st = st; r.tri = tn;
+                    rec_store(dst, m, r);
+                    if (ko.enabled) {
+                        double sf;
+                        const int k = toroidal_interval(tb.tor, next[2], sf);
+                        const int key = tn < 0 ? ko.ncell : cm.cell(tn, k);
+                        ko.keys[m] = key;
+                        atomicAdd(ko.hist + key, 1);
+                    }
+                } else {
+                    // the follow-up kernel redoes this phase through the global tables, reading src again and writing dst[m]
+                    rq.list[atomicAdd(rq.count, 1)] = m;
+                }
+            }
+            __syncwarp();
+            if (lane == 0) { __threadfence_block(); atomicAdd(&ctl->left, 1); }   // one more chunk of this ring entry done
+        }
+    }
+}
+
+}  // namespace trimeg
