@@ -222,8 +222,8 @@ inline int build_mesh(int64_t n_nodes, const double* RZ, int64_t T, const int32_
 // by an anisotropic distance to the nearest own triangle: with the magnetic axis known, the distance along the
 // poloidal field direction (tangent to the flux surface) counts 1/aspect of the distance across it, because
 // within one RK4 step markers move mainly along the field (parallel streaming) and hardly across it (drifts).
-// nbr gives, per slot and edge, the slot across that edge or -1 when that triangle is not staged (or the edge is
-// on the mesh boundary).
+// nbr gives, per slot and edge, the slot across that edge, -1 when that triangle is not staged, -2 when the edge is
+// on the mesh boundary.
 namespace trimeg_host {
 struct HostPatches {
     int TP = 0, SMAX = 0, npatch = 0;
@@ -297,7 +297,7 @@ inline void build_patches(const HostMesh& hm, const double* RZ, int64_t n_nodes,
             if (t < 0) continue;
             for (int e = 0; e < 3; e++) {
                 int32_t nb = hm.nbr[3 * t + e];
-                hp.nbr[((size_t)p * SMAX + s) * 4 + e] = (nb >= 0 && slot_of[nb] >= 0) ? (int16_t)slot_of[nb] : (int16_t)-1;
+                hp.nbr[((size_t)p * SMAX + s) * 4 + e] = nb < 0 ? (int16_t)-2 : (slot_of[nb] >= 0 ? (int16_t)slot_of[nb] : (int16_t)-1);   // -2: mesh boundary, -1: not staged
             }
         }
         for (int s = 0; s < ns; s++) if (sl[s] >= 0) slot_of[sl[s]] = -1;

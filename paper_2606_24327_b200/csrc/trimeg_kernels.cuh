@@ -431,11 +431,13 @@ __device__ __forceinline__ void tile_refill(unsigned char* smem, int b, const De
     }
 }
 
-// slot-space edge walk inside the staged block: returns the slot containing (R, Z) or -1 (left the staged set / hop cap)
-__device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int sl, double R, double Z, double& xi, double& eta) {
+// slot-space edge walk inside the staged block: returns the slot containing (R, Z) or a negative code: -1 left the staged
+// set (or hop cap), -2 crossed the mesh boundary.  `last` = the last staged slot visited.
+__device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int sl, double R, double Z, double& xi, double& eta, int& last) {
     if (sl < 0) return -1;
     for (int hop = 0; hop < 16; ++hop) {
         const SlotGeom& g = sgeom[sl];
+        last = sl;
         double dx = R - g.v0x, dy = Z - g.v0y;
         xi = fma(g.a11, dx, g.a12 * dy);
         eta = fma(g.a21, dx, g.a22 * dy);
@@ -443,9 +445,13 @@ __device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int
         if (fmin(fmin(xi, eta), l0) >= INSIDE_TOL) return sl;
         int e = (eta <= xi && eta <= l0) ? 0 : ((l0 <= xi) ? 1 : 2);
         sl = g.nbr[e];
-        if (sl < 0) return -1;
+        if (sl < 0) return sl;
     }
     return -1;
+}
+__device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int sl, double R, double Z, double& xi, double& eta) {
+    int last;
+    return slot_walk(sgeom, sl, R, Z, xi, eta, last);
 }
 
 // One phase of the RK4 step for the markers of one super-cell after another.  Position j of the cell order is record

@@ -31,65 +31,63 @@ struct WsLayout {
 
 __device__ __forceinline__ void mbar_arrive(void* bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory"); }
 
-// stager: fill ring entry b with the next non-empty super-cell (whole warp).  Returns false when the work list is
-// exhausted (the entry then carries sc = -1 and its barrier completes at once).
+// stager, part 1: take the next non-empty super-cell off the work list and pull everything its ring entry needs out of
+// global memory into registers (lane sl holds slot sl).  Done BEFORE a ring entry is free, so that only shared-memory
+// writes and the TMA issue remain once it is.  Returns false when the work list is exhausted.
+struct StageWork { int sc, begin, end, patch, k0, ns, t; SlotGeom g; };
 template <class C>
-__device__ __forceinline__ bool ws_stage(unsigned char* smem, int b, const DevTables& tb, const TileTables& tt, int* work_counter, int lane) {
+__device__ __forceinline__ bool ws_fetch(const DevTables& tb, const TileTables& tt, int* work_counter, int lane, StageWork& w) {
+    static_assert(C::SMAX <= 32, "one slot per lane");
+    constexpr unsigned FULL = 0xffffffffu;
+    int sc = 0, begin = 0, end = 0;
+    for (;;) {
+        if (lane == 0) sc = atomicAdd(work_counter, 1);
+        sc = __shfl_sync(FULL, sc, 0);
+        if (sc >= tt.nsc) return false;
+        begin = tt.offs[(long long)sc * C::CPS]; end = tt.offs[(long long)(sc + 1) * C::CPS];
+        if (begin != end) break;
+    }
+    w.sc = sc; w.begin = begin; w.end = end;
+    w.patch = sc / tt.nwin; w.k0 = (sc - w.patch * tt.nwin) * C::WK;
+    w.ns = tt.nslots[w.patch];
+    w.t = -1;
+    SlotGeom& g = w.g;
+    g.v0x = g.v0y = 1e300; g.a11 = g.a12 = g.a21 = g.a22 = 0.0; g.nbr[0] = g.nbr[1] = g.nbr[2] = g.nbr[3] = -1;
+    if (lane < w.ns) {
+        w.t = tt.slots[(long long)w.patch * C::SMAX + lane];
+        if (w.t >= 0) {
+            const TriGeom tg = tb.geom[w.t];
+            g.v0x = tg.v0x; g.v0y = tg.v0y; g.a11 = tg.a11; g.a12 = tg.a12; g.a21 = tg.a21; g.a22 = tg.a22;
+            const short* nb = tt.nbr + ((long long)w.patch * C::SMAX + lane) * 4;
+            g.nbr[0] = nb[0]; g.nbr[1] = nb[1]; g.nbr[2] = nb[2];
+        }
+    }
+    g.tri = w.t; g.pad = 0;
+    return true;
+}
+// stager, part 2: fill the (free) ring entry b from registers and start the TMA bulk copies of its coefficient blocks
+template <class C>
+__device__ __forceinline__ void ws_commit(unsigned char* smem, int b, const DevTables& tb, const StageWork& w, int lane) {
     constexpr unsigned FULL = 0xffffffffu;
     double* coef = reinterpret_cast<double*>(smem + C::BLOCK_BYTES * b);
     SlotGeom* sgeom = reinterpret_cast<SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
     BlockCtrl* ctl = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL) + b;
     unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF) + 2 * b;
-    int sc = 0, begin = 0, end = 0;
-    for (;;) {
-        if (lane == 0) sc = atomicAdd(work_counter, 1);
-        sc = __shfl_sync(FULL, sc, 0);
-        if (sc >= tt.nsc) { sc = -1; break; }
-        begin = tt.offs[(long long)sc * C::CPS]; end = tt.offs[(long long)(sc + 1) * C::CPS];
-        if (begin != end) break;
-    }
-    if (sc < 0) {
-        if (lane == 0) { ctl->sc = -1; __threadfence_block(); mbar_arrive(mbar); }
-        return false;
-    }
-    const int patch = sc / tt.nwin, k0 = (sc - patch * tt.nwin) * C::WK;
-    const int ns = tt.nslots[patch];
-    const int* pslots = tt.slots + (long long)patch * C::SMAX;
     if (lane == 0) {
-        ctl->sc = sc; ctl->begin = begin; ctl->end = end; ctl->next = begin; ctl->ns = ns; ctl->patch = patch; ctl->k0 = k0;
-        ctl->pad[0] = (end - begin + 31) >> 5;                        // chunks that will be cut from this entry
+        ctl->sc = w.sc; ctl->begin = w.begin; ctl->end = w.end; ctl->next = w.begin; ctl->ns = w.ns; ctl->patch = w.patch; ctl->k0 = w.k0;
+        ctl->pad[0] = (w.end - w.begin + 31) >> 5;                    // chunks that will be cut from this entry
         *reinterpret_cast<volatile int*>(&ctl->left) = 0;             // chunks done
     }
-    int cnt = 0;
-    for (int sl = lane; sl < ns; sl += 32) {
-        int t = pslots[sl];
-        SlotGeom g;
-        if (t >= 0) {
-            const TriGeom tg = tb.geom[t];
-            g.v0x = tg.v0x; g.v0y = tg.v0y; g.a11 = tg.a11; g.a12 = tg.a12; g.a21 = tg.a21; g.a22 = tg.a22;
-            const short* nb = tt.nbr + ((long long)patch * C::SMAX + sl) * 4;
-            g.nbr[0] = nb[0]; g.nbr[1] = nb[1]; g.nbr[2] = nb[2]; g.nbr[3] = -1;
-            cnt++;
-        } else {
-            g.v0x = g.v0y = 1e300; g.a11 = g.a12 = g.a21 = g.a22 = 0.0; g.nbr[0] = g.nbr[1] = g.nbr[2] = g.nbr[3] = -1;
-        }
-        g.tri = t; g.pad = 0;
-        sgeom[sl] = g;
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(FULL, cnt, o);
+    if (lane < w.ns) sgeom[lane] = w.g;
+    const int cnt = __popc(__ballot_sync(FULL, w.t >= 0));
     __threadfence_block();
     fence_async_smem();   // earlier generic accesses of this block vs. the async writes
     __syncwarp();
     if (lane == 0) mbar_expect_tx(mbar, (unsigned)(cnt * C::SLOT_DOUBLES * sizeof(double)));
     __syncwarp();
-    for (int sl = lane; sl < ns; sl += 32) {
-        int t = pslots[sl];
-        if (t >= 0)
-            tma_bulk_g2s(coef + (size_t)sl * C::SLOT_DOUBLES, tb.coef + (long long)t * tb.tri_stride + (long long)k0 * PLANE_STRIDE,
-                         (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
-    }
-    return true;
+    if (w.t >= 0)
+        tma_bulk_g2s(coef + (size_t)lane * C::SLOT_DOUBLES, tb.coef + (long long)w.t * tb.tri_stride + (long long)w.k0 * PLANE_STRIDE,
+                     (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
 }
 
 template <class C, int PHASE>
@@ -116,6 +114,8 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
 
     if (wid == 0) {
         // ------------------------------------------------------------------ stager
+        StageWork w;
+        bool have = ws_fetch<C>(tb, tt, work_counter, lane, w);
         for (unsigned it = 0;; ++it) {
             const int b = it % C::NBUF;
             if (it >= (unsigned)C::NBUF) {   // previous occupant: all chunks cut from it are done
@@ -126,7 +126,16 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
                 }
                 __syncwarp();
             }
-            if (!ws_stage<C>(smem, b, tb, tt, work_counter, lane)) break;
+            if (!have) {   // end of work: the entry carries sc = -1 and its barrier completes at once
+                if (lane == 0) {
+                    ctl_all[b].sc = -1;
+                    __threadfence_block();
+                    mbar_arrive(blk_bar + 2 * b);
+                }
+                break;
+            }
+            ws_commit<C>(smem, b, tb, w, lane);
+            have = ws_fetch<C>(tb, tt, work_counter, lane, w);   // the next entry's global loads overlap the compute warps' work
         }
     } else if (wid == 1) {
         // ------------------------------------------------------------------ publisher
@@ -177,10 +186,10 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
     } else {
         // ------------------------------------------------------------------ compute warps
         const int P = tb.tor.P;
+        unsigned t_next = 0;
+        if (lane == 0) t_next = (unsigned)atomicAdd(cons_head, 1);
         for (;;) {
-            unsigned t = 0;
-            if (lane == 0) t = (unsigned)atomicAdd(cons_head, 1);
-            t = __shfl_sync(FULL, t, 0);
+            const unsigned t = __shfl_sync(FULL, t_next, 0);
             const unsigned s = t % L::K, g = t / L::K;
             mbar_wait(full_bar + s, g & 1);
             const int m0 = desc[s].m0, end = desc[s].end, b = desc[s].b;
@@ -195,7 +204,10 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
                 for (int j = 0; j < 7; ++j) lds128(a + 16 * (j ^ (lane & 7)), rd[2 * j], rd[2 * j + 1]);
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(empty_bar + s);   // the slot may be refilled
+            if (lane == 0) {
+                mbar_arrive(empty_bar + s);                        // the slot may be refilled
+                t_next = (unsigned)atomicAdd(cons_head, 1);        // next ticket: its latency hides behind the arithmetic
+            }
 
             const double* coef = reinterpret_cast<const double*>(smem + C::BLOCK_BYTES * b);
             const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
@@ -235,6 +247,8 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
                 double next[3];
                 if (phase_step<PHASE>(tb.tor, dt, r, eval, next)) {
                     // triangle of the next phase's first evaluation point: staged walk, else the global walk
+                    // (binning by the last staged triangle instead was tried: 8.6 % of the markers then start the next
+                    // phase outside their patch's halo and retire)
                     double xi, eta;
                     const int sl = slot_walk(sgeom, slot, next[0], next[1], xi, eta);
                     const int tn = sl >= 0 ? sgeom[sl].tri : locate_walk(tb.bg, tb.geom, tri_last, next[0], next[1]);
