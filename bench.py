@@ -32,8 +32,9 @@ UNIT = "marker-pushes/s"
 FLOP_PER_PUSH = 3772.0          # 943 flop per RK stage x 4
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
 KEYS = ("R", "Z", "phi", "u", "w", "mu", "p")
-TRAFFIC_BYTES_PER_LAUNCH = None   # dram__bytes_read.sum + dram__bytes_write.sum of k_push_tiled from the last ncu --set full capture (profiles/)
-SORT_EVERY = 1                  # tiled kernel: re-bin every step (BASELINE configs[2] uses 10)
+TRAFFIC_BYTES_PER_LAUNCH = 31.95e9   # dram__bytes_read.sum + dram__bytes_write.sum of one k_phase_ws launch (profiles/r01c_summary.md)
+ALGO_BYTES_PER_LAUNCH = 2 * 112 + 8 + 17   # per marker: 112 live record bytes in and out, permutation + key, one pass over the coefficient table
+SORT_EVERY = 1                  # two-phase kernel: both phases re-bin every step (BASELINE configs[2] uses 10)
 
 
 def make_inputs(cfg, n, start, pinned):
@@ -152,7 +153,7 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--markers", type=int, default=None, help="markers per GPU (default: the config's)")
     ap.add_argument("--dt", type=float, default=None)
-    ap.add_argument("--variant", type=int, default=0, help="0 tiled push kernel, 1 simple")
+    ap.add_argument("--variant", type=int, default=0, help="0 two-phase warp-specialised push, 1 simple")
     ap.add_argument("--sort-every", type=int, default=SORT_EVERY, help="re-sort the marker store every n RK4 steps (inside the timed region)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample", type=int, default=400_000, help="markers of the oracle cpu_baseline leg (x 4 steps)")
@@ -219,12 +220,14 @@ def main():
     step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
     total_s = shard.reduce_max_seconds(sum(step_ms) * 1e-3, dist if world > 1 else None)
     value = shard.job_rate(n * args.steps, world, total_s)
-    # dominant kernel: the push kernel proper.  Algorithmic flops per launch = 943 flop x the marker-stage evaluations it
-    # performed (all 4 n minus those left to the follow-up kernel), over its own CUDA-event duration.
-    kern_s = statistics.mean(k["push"] for k in kms) * 1e-3
+    # dominant kernel: the phase kernel k_phase_ws, launched twice per step (phase A: k2, k3; phase B: k4, next k1).
+    # Algorithmic flops per launch = 943 flop x the right-hand-side evaluations it performed (2 n minus those left to the
+    # follow-up kernel), over its average launch duration from the library's CUDA events (sum of the two launches / 2).
+    launches_per_step = 2 if args.variant == 0 else 1
+    kern_s = statistics.mean(k["push"] for k in kms) * 1e-3 / launches_per_step
     sort_ms = statistics.mean(k["sort"] for k in kms)
     finish_ms = statistics.mean(k["finish"] for k in kms)
-    stage_evals = 4.0 * n - slow / args.steps
+    stage_evals = (4.0 * n - slow / args.steps) / launches_per_step
     achieved = (FLOP_PER_PUSH / 4.0) * stage_evals / kern_s / 1e12
     step_achieved = FLOP_PER_PUSH * n * args.steps / (sum(step_ms) * 1e-3) / 1e12
 
@@ -261,13 +264,14 @@ def main():
                 "gpu_launches": launches,
                 "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
                              "traffic": TRAFFIC_BYTES_PER_LAUNCH if (args.variant == 0 and args.config == 3 and n == cfg.n_markers) else None,
-                             "kernel": "k_push_tiled" if args.variant == 0 else "k_push_simple", "kernel_ms": 1e3 * kern_s,
+                             "kernel": "k_phase_ws" if args.variant == 0 else "k_push_simple", "kernel_ms": 1e3 * kern_s,
+                             "kernel_launches_per_step": launches_per_step,
                              "flop_per_push": FLOP_PER_PUSH, "stage_evals_per_launch": stage_evals,
                              "peak_kind": "nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (derived, DESIGN.md)",
                              "measured_dfma_tflops": dfma, "frac_of_measured_dfma": achieved / dfma,
                              "whole_step_frac": step_achieved / FP64_PEAK_TFLOPS,
-                             "hbm_algorithmic_GBps": 121.0 * n / kern_s / 1e9},
-                "step_breakdown_ms": {"sort": sort_ms, "push": 1e3 * kern_s, "finish": finish_ms},
+                             "hbm_algorithmic_GBps": ALGO_BYTES_PER_LAUNCH * n / kern_s / 1e9},
+                "step_breakdown_ms": {"sort": sort_ms, "push": 1e3 * kern_s * launches_per_step, "finish": finish_ms},
                 "slow_path_evals": slow, "retired_markers": retired, "e2e_checksum": checksum}
         if not args.no_cpu_baseline:
             cpu_n = min(n, args.cpu_sample)

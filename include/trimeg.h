@@ -99,8 +99,8 @@ int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, 
 size_t trimeg_scratch_bytes(const trimeg_ctx* ctx, int64_t n);
 
 /* Hand n markers to the library (L89: R, Z, phi, v_par, w per marker; mu and p are constants of the motion).
- * The seven arrays [n] live in `memspace` and are read once (copied into the library's structure-of-arrays
- * store, which lives in `scratch`: DEVICE memory owned by the caller that must stay valid until the next
+ * The seven arrays [n] live in `memspace` and are read once (copied into the library's marker store
+ * (one 128-byte record per marker), which lives in `scratch`: DEVICE memory owned by the caller that must stay valid until the next
  * bind/destroy; with TRIMEG_HOST inputs the call returns after the copies are enqueued from the caller's
  * buffers, so those must stay valid until trimeg_sync).  Marker status is reset to 0.
  * Errors: BAD_ARG, BAD_STATE (no mesh), OOM (scratch too small), CUDA. */
@@ -113,10 +113,13 @@ int trimeg_markers_bind(trimeg_ctx* ctx, int64_t n, const double* R, const doubl
 int trimeg_markers_get(trimeg_ctx* ctx, double* R, double* Z, double* phi, double* u, double* w, int32_t* status,
                        int memspace);
 
-/* Re-sort the marker store by cell (triangle x toroidal interval) now / every n-th RK4 step (0 = never again;
- * a sort is always done once after bind before the first push).  Inside trimeg_push_rk4 the sort is fused into
- * the push: every step that precedes a re-sort also writes each marker's new cell key and the cell histogram,
- * the sort proper only builds the permutation, and the next push step reads the markers through it. */
+/* Ordering of the marker store by cell (triangle x toroidal interval).  trimeg_push_rk4 (variant 0) runs every RK4 step
+ * as two phases, each in the cell order of ITS evaluation points; every phase writes the next
+ * phase's cell keys and their histogram, a scan and a scatter turn them into a permutation, and the next phase reads its
+ * markers through it (the sort has no data pass of its own).  set_sort_interval(n): rebuild both orders every n-th step
+ * (default 1 = every step; 0 = only when needed, i.e. once after bind); between re-sorts the phases run in the stale
+ * order and markers that drifted out of their staged block take a slower follow-up path (results do not change).
+ * trimeg_sort: force a rebuild at the next step.  Caller order is never affected. */
 int trimeg_sort(trimeg_ctx* ctx);
 int trimeg_set_sort_interval(trimeg_ctx* ctx, int32_t every_n_steps);
 
@@ -130,21 +133,21 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps);
  * boundary (L89: "time derivatives of R, Z, phi, v_par and the marker weights w").  out [5][n] in `memspace`. */
 int trimeg_rhs(trimeg_ctx* ctx, double* out, int memspace);
 
-/* Select the push kernel: 0 = tiled (cell-coherent gather through shared memory, default),
- * 1 = simple (one thread per marker, coefficients through L1/L2).  Both compute the same thing. */
+/* Select the push kernel: 0 = two-phase warp-specialised kernel (cell-coherent gather through shared memory, default),
+ * 1 = simple (whole RK4 step, one thread per marker, coefficients through L1/L2).  Both compute the same thing. */
 int trimeg_set_push_variant(trimeg_ctx* ctx, int32_t variant);
 
 /* Diagnostics used by the benchmark: achieved FP64 FMA throughput of this device in TFLOP/s
  * (a register-only DFMA loop; the roofline's measured "alu" peak). */
 int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops);
-/* Counters of the last trimeg_push_rk4 call: [0] kernel launches, [1] marker-stage evaluations that took the
- * slow (out-of-tile) gather path in the follow-up kernel, [2] markers that left their staged tile during a step
- * (summed over steps), [3] sorts done. */
+/* Counters of the last trimeg_push_rk4 call: [0] kernel launches, [1] right-hand-side evaluations that took the
+ * slow (out-of-block) path in the follow-up kernel, [2] marker-phases that left their staged block (summed over
+ * phases and steps), [3] permutations built. */
 int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]);
 /* Device time (CUDA events on the context's stream; blocks until they have completed) of the last RK4 step of the
- * last trimeg_push_rk4 call, in milliseconds: [0] sort kernels of that step (keys, scan, permutation; 0 if it did
- * not re-sort), [1] the push kernel proper (the roofline's "dominant kernel"), [2] the follow-up kernels (markers
- * that left their staged tile, markers outside the mesh).  Errors: BAD_ARG, BAD_STATE (nothing pushed yet), CUDA. */
+ * last trimeg_push_rk4 call, in milliseconds: [0] sort kernels of that step (scan, permutation; both phases), [1] the
+ * two launches of the phase kernel (the roofline's "dominant kernel"; divide by 2 for one launch), [2] the follow-up
+ * kernels (markers that left their staged block, markers outside the mesh).  Errors: BAD_ARG, BAD_STATE (nothing pushed yet), CUDA. */
 int trimeg_push_kernel_ms(trimeg_ctx* ctx, double out[3]);
 
 #ifdef __cplusplus
