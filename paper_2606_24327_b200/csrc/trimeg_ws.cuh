@@ -21,7 +21,8 @@ struct ChunkDesc { int m0, end, b, pad; };   // m0 < 0: no more work
 template <class C>
 struct WsLayout {
     static constexpr int K = C::NWARPS;                                  // chunk slots (4 KB each, in the staging area)
-    static constexpr int NCONS = C::NWARPS - 2;
+    static constexpr int NPUB = 2;                                       // publisher warps (tickets of parity pid)
+    static constexpr int NCONS = C::NWARPS - 1 - NPUB;
     static constexpr size_t OFF_DESC = C::OFF_STAGE + C::WSTAGE * C::NWARPS;
     static constexpr size_t OFF_FULL = OFF_DESC + 16 * K;
     static constexpr size_t OFF_EMPTY = OFF_FULL + 8 * K;
@@ -137,8 +138,9 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
             ws_commit<C>(smem, b, tb, w, lane);
             have = ws_fetch<C>(tb, tt, work_counter, lane, w);   // the next entry's global loads overlap the compute warps' work
         }
-    } else if (wid == 1) {
-        // ------------------------------------------------------------------ publisher
+    } else if (wid <= L::NPUB) {
+        // ------------------------------------------------------------------ publishers: warp pid takes the tickets t with t % NPUB == pid
+        const unsigned pid = wid - 1;
         unsigned ticket = 0;
         auto slot_acquire = [&](unsigned t) {   // wait until the previous user of the slot has pulled its records out
             const unsigned s = t % L::K, g = t / L::K;
@@ -151,13 +153,18 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
             const BlockCtrl* ctl = ctl_all + b;
             if (ctl->sc < 0) break;
             const int begin = ctl->begin, end = ctl->end;
+            // the chunks of this entry carry tickets ticket .. ticket + nch - 1; ours are those of parity pid
+            const unsigned t0 = ticket, nch = (unsigned)(end - begin + 31) >> 5;
+            unsigned t = t0 + (pid + L::NPUB - t0 % L::NPUB) % L::NPUB;
+            ticket = t0 + nch;
             int pr_next = 0;
-            if (begin + lane < end) pr_next = perm ? perm[begin + lane] : begin + lane;
-            for (int c0 = begin; c0 < end; c0 += 32, ++ticket) {
+            if (t < t0 + nch) { const int q = begin + 32 * (int)(t - t0) + lane; if (q < end) pr_next = perm ? perm[q] : q; }
+            for (; t < t0 + nch; t += L::NPUB) {
+                const int c0 = begin + 32 * (int)(t - t0);
                 const int pr = pr_next;
-                const int n0 = c0 + 32 + lane;
-                if (n0 < end) pr_next = perm ? perm[n0] : n0;      // next chunk's permutation entries: in flight during this one
-                const int s = slot_acquire(ticket);
+                const int n0 = c0 + 32 * L::NPUB + lane;
+                if (n0 < end) pr_next = perm ? perm[n0] : n0;      // our next chunk's permutation entries: in flight during this one
+                const int s = slot_acquire(t);
                 if (lane == 0) { desc[s].m0 = c0; desc[s].end = end; desc[s].b = b; __threadfence_block(); }
                 __syncwarp();
                 const int nvalid = min(32, end - c0);
@@ -178,6 +185,7 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
         }
         // one end-of-work ticket per compute warp
         for (int q = 0; q < L::NCONS; ++q, ++ticket) {
+            if (ticket % L::NPUB != pid) continue;
             const int s = slot_acquire(ticket);
             if (lane == 0) { desc[s].m0 = -1; __threadfence_block(); }
             __syncwarp();
