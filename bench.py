@@ -144,6 +144,51 @@ def workload_config(cfg, n, args):
             "l2": "inputs_exceed_l2" if n * 104 > 126e6 else "l2_flushed_between_steps"}
 
 
+def run_gather(args, cfg):
+    """BASELINE configs[4]: one field evaluation per point, random order and then the same points sorted by cell.
+    Prints one JSON line ("mode": "gather"); not the headline metric (that is the push)."""
+    import torch
+    from paper_2606_24327_b200.binding import Trimeg
+    n = args.markers if args.markers is not None else cfg.n_markers
+    g = Trimeg(0)
+    setup_case(cfg, g)
+    host, views = make_inputs(cfg, n, 0, pinned=False)
+    pts = {k: host[k].cuda() for k in ("R", "Z", "phi")}
+    out = torch.empty((8, n), dtype=torch.float64, device="cuda")
+    tri = torch.empty(n, dtype=torch.int32, device="cuda")
+
+    def timed(P):
+        for _ in range(args.warmup):
+            g.gather(P["R"], P["Z"], P["phi"], out=out, tri_out=tri)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        ev[0].record()
+        for s in range(args.steps):
+            g.gather(P["R"], P["Z"], P["phi"], out=out, tri_out=tri)
+            ev[s + 1].record()
+        torch.cuda.synchronize()
+        return statistics.mean(ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)) * 1e-3
+
+    t_rand = timed(pts)
+    # cell key = triangle x toroidal interval (caller numbering is enough to make the reads of a cell adjacent)
+    k = torch.clamp((pts["phi"] % cfg.phi_period) / cfg.phi_period * cfg.n_planes, max=cfg.n_planes - 1).to(torch.int64)
+    key = tri.to(torch.int64) * cfg.n_planes + k
+    order = torch.argsort(key)
+    spts = {q: v[order].contiguous() for q, v in pts.items()}
+    del key, order, k
+    t_sort = timed(spts)
+    T, Pn = 2 * cfg.nr * cfg.ntheta, cfg.n_planes
+    table = T * (Pn + 5) * 336
+    algo = n * (24 + 4 + 64) + table          # points in, triangle id + 8 values out, one pass over the coefficient table
+    peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"] if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else 6650.0
+    line = {"mode": "gather", "metric": "field gathers/s (fp64, 1 B200)", "unit": "gathers/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "value": n / t_sort, "value_unsorted": n / t_rand, "ms_sorted": 1e3 * t_sort, "ms_unsorted": 1e3 * t_rand, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {T} triangles x {Pn} planes, {n} points, one evaluation of phi, A_par and gradients per point",
+                       "l2": "inputs_exceed_l2"},
+            "roofline": {"bound": "hbm", "achieved": algo / t_sort / 1e9, "achieved_unsorted": algo / t_rand / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": algo / t_sort / 1e9 / peak, "traffic": None, "kernel": "k_gather", "algorithmic_bytes": algo}}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -159,6 +204,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=400_000, help="markers of the oracle cpu_baseline leg (x 4 steps)")
     ap.add_argument("--ref-markers", type=int, default=200_000, help="markers per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--gather", action="store_true", help="gather-only stress test (use with --config 4), unsorted vs cell-sorted points")
     args = ap.parse_args()
 
     import dataclasses
@@ -169,6 +215,10 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, cfg, rank, world)
+        return
+    if args.gather:
+        if rank == 0:
+            run_gather(args, cfg)
         return
 
     import torch
@@ -260,7 +310,7 @@ def main():
                 "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, n, args), "clocks": clocks,
                 "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 7 * 8 * n, "d2h_bytes_per_step": (5 * 8 + 4) * n, "steps": e2e_steps,
-                        "note": "bind(HOST) includes the first sort by cell; PCIe-bound"},
+                        "note": "every e2e step re-binds from HOST buffers, so it also pays the k1 initialisation of an unsorted store; PCIe-bound"},
                 "gpu_launches": launches,
                 "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
                              "traffic": TRAFFIC_BYTES_PER_LAUNCH if (args.variant == 0 and args.config == 3 and n == cfg.n_markers) else None,

@@ -577,6 +577,9 @@ int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]) {
         CU(cudaSetDevice(ctx->device));
         CU(cudaMemcpyAsync(h, ctx->d_stats, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
+#ifdef TRIMEG_WAITSTATS
+        fprintf(stderr, "waitstats kcycles: compute-warps-for-chunk %llu  stager-for-free-entry %llu  publishers-for-block %llu\n", h[2], h[3], h[0]);
+#endif
         out[1] = (int64_t)(2 * h[1]);   // each follow-up marker-phase is two right-hand-side evaluations
         out[2] = (int64_t)h[1];
     }

@@ -368,68 +368,12 @@ __global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP s
     for (int q = 0; q < 5; ++q) out[(long long)q * n + r.id] = d[q];
 }
 
-// ============================================================================================ tiled phase kernel
+// ============================================================================================ phase kernel: helpers
 // markers that left their staged block during a phase: positions in the cell order, finished by k_phase_global
 struct RetireList {
     int* list;      // [n]
     int* count;     // device counter
 };
-
-// (re)fill ring entry b with the next non-empty super-cell; executed by one whole warp.  The entry's mbarrier completes
-// when the TMA bytes have landed (or at once, with sc = -1, when the work list is exhausted).
-template <class C>
-__device__ __forceinline__ void tile_refill(unsigned char* smem, int b, const DevTables& tb, const TileTables& tt, int* work_counter, int lane) {
-    constexpr unsigned FULL = 0xffffffffu;
-    double* coef = reinterpret_cast<double*>(smem + C::BLOCK_BYTES * b);
-    SlotGeom* sgeom = reinterpret_cast<SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
-    BlockCtrl* ctl = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL) + b;
-    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF) + 2 * b;
-    int sc = 0, begin = 0, end = 0;
-    for (;;) {
-        if (lane == 0) sc = atomicAdd(work_counter, 1);
-        sc = __shfl_sync(FULL, sc, 0);
-        if (sc >= tt.nsc) { sc = -1; break; }
-        begin = tt.offs[(long long)sc * C::CPS]; end = tt.offs[(long long)(sc + 1) * C::CPS];
-        if (begin != end) break;
-    }
-    if (sc < 0) {
-        if (lane == 0) { ctl->sc = -1; ctl->left = 0; __threadfence_block(); asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(mbar)) : "memory"); }
-        return;
-    }
-    const int patch = sc / tt.nwin, k0 = (sc - patch * tt.nwin) * C::WK;
-    const int ns = tt.nslots[patch];
-    const int* pslots = tt.slots + (long long)patch * C::SMAX;
-    if (lane == 0) { ctl->sc = sc; ctl->begin = begin; ctl->end = end; ctl->next = begin; ctl->left = 0; ctl->ns = ns; ctl->patch = patch; ctl->k0 = k0; }
-    int cnt = 0;
-    for (int sl = lane; sl < ns; sl += 32) {
-        int t = pslots[sl];
-        SlotGeom g;
-        if (t >= 0) {
-            const TriGeom tg = tb.geom[t];
-            g.v0x = tg.v0x; g.v0y = tg.v0y; g.a11 = tg.a11; g.a12 = tg.a12; g.a21 = tg.a21; g.a22 = tg.a22;
-            const short* nb = tt.nbr + ((long long)patch * C::SMAX + sl) * 4;
-            g.nbr[0] = nb[0]; g.nbr[1] = nb[1]; g.nbr[2] = nb[2]; g.nbr[3] = -1;
-            cnt++;
-        } else {
-            g.v0x = g.v0y = 1e300; g.a11 = g.a12 = g.a21 = g.a22 = 0.0; g.nbr[0] = g.nbr[1] = g.nbr[2] = g.nbr[3] = -1;
-        }
-        g.tri = t; g.pad = 0;
-        sgeom[sl] = g;
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(FULL, cnt, o);
-    __threadfence_block();
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic accesses of this block vs. the async writes
-    __syncwarp();
-    if (lane == 0) mbar_expect_tx(mbar, (unsigned)(cnt * C::SLOT_DOUBLES * sizeof(double)));
-    __syncwarp();
-    for (int sl = lane; sl < ns; sl += 32) {
-        int t = pslots[sl];
-        if (t >= 0)
-            tma_bulk_g2s(coef + (size_t)sl * C::SLOT_DOUBLES, tb.coef + (long long)t * tb.tri_stride + (long long)k0 * PLANE_STRIDE,
-                         (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
-    }
-}
 
 // slot-space edge walk inside the staged block: returns the slot containing (R, Z) or a negative code: -1 left the staged
 // set (or hop cap), -2 crossed the mesh boundary.  `last` = the last staged slot visited.
@@ -452,192 +396,6 @@ __device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int
 __device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int sl, double R, double Z, double& xi, double& eta) {
     int last;
     return slot_walk(sgeom, sl, R, Z, xi, eta, last);
-}
-
-// One phase of the RK4 step for the markers of one super-cell after another.  Position j of the cell order is record
-// src[perm[j]] (perm null: src[j]) and is written to dst[j].  Persistent: one CTA per SM, every warp runs on its own.
-// Per warp the work is software-pipelined over chunks of 32 markers:
-//   records of the NEXT chunk travel global -> shared by per-lane bulk copies (TMA) while the current chunk is computed,
-//   updated records travel registers -> shared -> global by per-lane bulk stores (no LSU wavefronts for 32 scattered lines).
-struct ChunkRef { int m0, end, b; unsigned it; };
-
-template <class C, int PHASE>
-__global__ void __launch_bounds__(C::NTHREADS, TRIMEG_CTAS_PER_SM)
-k_phase_tiled(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __restrict__ src, Rec* __restrict__ dst, const int* __restrict__ perm,
-              RetireList rq, KeyOut ko, CellMap cm, double dt, int* __restrict__ work_counter) {
-    extern __shared__ __align__(128) unsigned char smem[];
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    BlockCtrl* ctl_all = reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL);
-    unsigned long long* mbar_all = reinterpret_cast<unsigned long long*>(smem + C::OFF_CTRL + 64 * C::NBUF);
-    unsigned char* in_buf = smem + C::OFF_STAGE + (size_t)wid * C::WSTAGE;
-    if (tid == 0) {
-        for (int b = 0; b < C::NBUF; ++b) mbar_init(mbar_all + 2 * b, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    if (wid == 0) {
-        for (int b = 0; b < C::NBUF; ++b) tile_refill<C>(smem, b, tb, tt, work_counter, lane);
-    }
-    const int P = tb.tor.P;
-    constexpr unsigned FULL = 0xffffffffu;
-
-    // ---- ring bookkeeping (all warp-uniform).  acq_it: ring iteration the warp takes chunks from; leave_it: first iteration
-    // it has not left yet.  An entry is left once the warp will take no more chunks from it AND is not computing on it;
-    // the last warp to leave refills it.
-    unsigned acq_it = 0, leave_it = 0;
-    bool exhausted = false;
-    auto leave_upto = [&](unsigned upto) {   // leave every entry with iteration < upto
-        for (; leave_it < upto; ++leave_it) {
-            const int b = leave_it % C::NBUF;
-            BlockCtrl* ctl = ctl_all + b;
-            __syncwarp();
-            int last = 0;
-            if (lane == 0) { __threadfence_block(); last = atomicAdd(&ctl->left, 1) == C::NWARPS - 1; }
-            last = __shfl_sync(FULL, last, 0);
-            if (last) { __threadfence_block(); tile_refill<C>(smem, b, tb, tt, work_counter, lane); }
-        }
-    };
-    // take the next chunk.  hold >= 0: the warp still computes on ring iteration `hold`; it then looks at most NBUF - 1 entries
-    // ahead (an entry further on can only be refilled after this warp has left `hold`) and leaves nothing at or after `hold`.
-    // Returns 1 = got one, 0 = nothing within the look-ahead, -1 = no work left.
-    auto acquire = [&](ChunkRef& c, long long hold) -> int {
-        for (;;) {
-            if (exhausted) return -1;
-            if (hold >= 0 && (long long)acq_it > hold + C::NBUF - 1) return 0;
-            const int b = acq_it % C::NBUF;
-            mbar_wait(mbar_all + 2 * b, (acq_it / C::NBUF) & 1);
-            BlockCtrl* ctl = ctl_all + b;
-            if (ctl->sc < 0) { exhausted = true; return -1; }
-            const int end = ctl->end;
-            int chunk = 0;
-            if (lane == 0) chunk = atomicAdd(&ctl->next, 32);
-            chunk = __shfl_sync(FULL, chunk, 0);
-            if (chunk < end) { c.m0 = chunk; c.end = end; c.b = b; c.it = acq_it; return 1; }
-            ++acq_it;
-            leave_upto(hold >= 0 ? (unsigned)min((long long)acq_it, hold) : acq_it);
-        }
-    };
-    // start the record loads of chunk c into the warp's in-buffer: eight 16-byte cp.async per lane; a group of 8 lanes
-    // copies one whole record per instruction (4 lines per warp instruction instead of 32)
-    auto fetch = [&](const ChunkRef& c) {
-        const int nvalid = min(32, c.end - c.m0);
-        int pr = 0;
-        if (lane < nvalid) { const int m = c.m0 + lane; pr = perm ? perm[m] : m; }
-        const unsigned ib = smem_u32(in_buf);
-        const int ch = lane & 7, g = lane >> 3;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const int R = 4 * k + g;
-            const int ri = __shfl_sync(FULL, pr, R);
-            if (R < nvalid) {
-                const unsigned d = ib + R * 128 + 16 * ((ch ^ (ri & 7)) ^ (R & 7));
-                const char* s = reinterpret_cast<const char*>(src + ri) + 16 * ch;
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(s) : "memory");
-            }
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    };
-    ChunkRef cur, nxt;
-    int have = acquire(cur, -1);
-    if (have == 1) fetch(cur);
-    while (have == 1) {
-        // ---- records of the current chunk: shared -> registers
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncwarp();
-        const int m = cur.m0 + lane;
-        const bool valid = m < cur.end;
-        Rec r;
-        if (valid) {
-            const unsigned a = smem_u32(in_buf) + lane * 128;
-            double* rd = reinterpret_cast<double*>(&r);
-#pragma unroll
-            for (int j = 0; j < 7; ++j) lds128(a + 16 * (j ^ (lane & 7)), rd[2 * j], rd[2 * j + 1]);
-        }
-        __syncwarp();   // every lane has its record in registers before the next chunk's copies may land
-        // ---- next chunk: take it and start its loads (at most one ring entry ahead of the one being computed on)
-        int have_next = acquire(nxt, (long long)cur.it);
-        if (have_next == 1) fetch(nxt);
-
-        // ---- compute
-        const double* coef = reinterpret_cast<const double*>(smem + C::BLOCK_BYTES * cur.b);
-        const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * cur.b + C::COEF_BYTES);
-        const BlockCtrl* ctl = ctl_all + cur.b;
-        const int patch = ctl->patch, k0 = ctl->k0, ns = ctl->ns;
-        if (valid) {
-            const double mu = r.mu, pw = r.p;
-            int st = r.st, slot = -1, tri_last = r.tri;
-            {
-                int sl = tri_last - patch * C::TP;
-                if (sl >= 0 && sl < C::TP) slot = sl;
-                else {   // not sorted since it moved: look for the triangle in the halo
-                    for (int q = C::TP; q < ns; ++q) if (sgeom[q].tri == tri_last) { slot = q; break; }
-                }
-            }
-            auto eval = [&](const double y[5], double d[5]) {
-                double xi = 0.0, eta = 0.0, sf;
-                const int sl = slot_walk(sgeom, slot, y[0], y[1], xi, eta);
-                const int k = toroidal_interval(tb.tor, y[2], sf);
-                int dk = k - k0;
-                if (dk > P / 2) dk -= P; else if (dk < -(P / 2)) dk += P;
-                const int lk = dk + C::HK;
-                if (!(sl >= 0 && lk >= 0 && lk < C::NW)) return false;
-                slot = sl;
-                const SlotGeom& g = sgeom[sl];
-                tri_last = g.tri;
-                double w[4], dw[4], g8[8];
-                bspline_from_s(tb.tor, sf, w, dw);
-                LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
-                gather_cell(ld, xi, eta, w, dw, g8);
-                Fields fo;
-                fo.P = g8[0]; fo.PR = fma(g.a11, g8[1], g.a21 * g8[2]); fo.PZ = fma(g.a12, g8[1], g.a22 * g8[2]); fo.Pp = g8[3];
-                fo.A = g8[4]; fo.AR = fma(g.a11, g8[5], g.a21 * g8[6]); fo.AZ = fma(g.a12, g8[5], g.a22 * g8[6]); fo.Ap = g8[7];
-                rhs_eval(ep, sp, y[0], y[1], y[3], y[4], mu, pw, fo, d);
-                return true;
-            };
-            double next[3];
-#ifdef TRIMEG_EXP_NOEVAL
-            next[0] = r.y[0]; next[1] = r.y[1]; next[2] = r.y[2];
-            if (r.y[0] > -1e300) {
-#else
-            if (phase_step<PHASE>(tb.tor, dt, r, eval, next)) {
-#endif
-                // triangle of the next phase's first evaluation point: staged walk, else the global walk (rare)
-                double xi, eta;
-                const int sl = slot_walk(sgeom, slot, next[0], next[1], xi, eta);
-                const int t = sl >= 0 ? sgeom[sl].tri : locate_walk(tb.bg, tb.geom, tri_last, next[0], next[1]);
-                r.st = st; r.tri = t;
-#ifndef TRIMEG_EXP_NOSTORE
-                rec_store(dst, m, r);
-#else
-                if (r.y[0] == 1.2345e-200) rec_store(dst, m, r);
-#endif
-                if (ko.enabled) {
-                    double sf;
-                    const int k = toroidal_interval(tb.tor, next[2], sf);
-                    const int key = t < 0 ? ko.ncell : cm.cell(t, k);
-                    ko.keys[m] = key;
-                    atomicAdd(ko.hist + key, 1);
-                }
-            } else {
-                // the follow-up kernel redoes this phase through the global tables, reading src again and writing dst[m]
-                rq.list[atomicAdd(rq.count, 1)] = m;
-            }
-        }
-        // ---- done computing on cur.it: leave every entry the warp is through with
-        if (have_next == 1) {
-            leave_upto(nxt.it);
-            cur = nxt;
-            have = 1;
-        } else {
-            leave_upto(cur.it + 1);
-            if (have_next == 0) {   // nothing within the look-ahead limit: look again now that the entry is left
-                have = acquire(cur, -1);
-                if (have == 1) fetch(cur);
-            } else have = -1;
-        }
-    }
-    // leave whatever is still held so that the ring drains for the other warps (entries up to the terminating one)
-    leave_upto(acq_it);
 }
 
 }  // namespace trimeg
@@ -716,6 +474,11 @@ __global__ void __launch_bounds__(256) k_sort_perm(long long n, const int* __res
 // per phase: acc[0] += markers left to the follow-up kernel
 __global__ void k_accumulate_stat(const int* __restrict__ v, unsigned long long* __restrict__ acc) {
     atomicAdd(acc, (unsigned long long)*v);
+#ifdef TRIMEG_WAITSTATS
+    atomicAdd(acc + 1, (unsigned long long)v[1]);   // compute warps waiting for a chunk (kilo-cycles, summed over warps)
+    atomicAdd(acc + 2, (unsigned long long)v[2]);   // stager waiting for a free ring entry
+    atomicAdd(acc - 1, (unsigned long long)v[3]);   // publishers waiting (block landed, slot free)
+#endif
 }
 
 // ============================================================================================ DFMA micro-benchmark

@@ -1,23 +1,13 @@
-// Tiled RK4 push: cell-coherent gather through shared memory.
+// Shared-memory tiling of the phase kernel: layout constants, slot geometry and the PTX helpers
+// (mbarrier, TMA bulk copy, shared-memory vector access).
 //
-// Why: one field evaluation reads 8 x 21 coefficients = 1344 B per marker.  Through L1 with one address per lane
-// that costs >= 1344*32/128 = 336 L1 cycles per warp (measured: 16-32 B/clk/SM delivered when lanes diverge), against
-// 338 DFMA = 169 issue cycles per SM of FP64 work.  Shared memory delivers 256 B/clk/SM when consecutive lanes read
-// the same address (measured), i.e. 168 cycles per warp -- if the lanes of a warp sit in the same few cells.  RK
-// stages 2-4 are evaluated at displaced positions (at dt = 0.05 most markers leave their home triangle), so lanes
-// are re-grouped by cell before every gather:
-//   owner lane (holds the marker's RK state in registers)      gather lane (rank i of the warp in cell order)
-//     locate by edge walk in the staged patch, B-spline cell
-//     warp bitonic sort of (cell, lane) keys           ---->   reads (xi, eta, s) of the i-th marker in cell order,
-//                                                              evaluates 2 fields x 4 planes with near-broadcast LDS.128,
-//     reads 8 field values back, equilibrium + RHS     <----   writes physical-gradient results to the owner's row
-// Everything between two stagings is warp-synchronous (no block barrier): the 16 warps of the CTA run independently
-// and hide each other's latencies.
-// The coefficient blocks of a patch of TP triangles plus a halo (SMAX slots), for a window of WK toroidal intervals
-// plus HK on either side, are staged per super-cell with 1-D TMA bulk copies (cp.async.bulk + mbarrier).
-// A marker whose stage position leaves the staged set RETIRES: it parks (marker index, stage, y_stage, k-sum) in a
-// global queue and a follow-up kernel finishes its step through the global tables, so that no warp ever waits on
-// a divergent slow lane.
+// Why tiles: one field evaluation reads 8 x 21 coefficients = 1344 B per marker.  Through L1 with one address per lane
+// that is >= 336 L1 cycles per warp against 338 DFMA = 169 issue cycles of FP64 work (measured: the L1-path kernel is
+// 2x slower even when every lane of a warp sits in the same cell).  So the coefficient blocks of a patch of TP triangles
+// plus a halo (SMAX slots), for a window of WK toroidal intervals plus HK on either side, are staged per super-cell with
+// 1-D TMA bulk copies (cp.async.bulk + mbarrier), and markers are visited in cell order so that the lanes of a warp read
+// the same few blocks.  A marker whose evaluation point leaves the staged set RETIRES to a list that a follow-up kernel
+// finishes through the global tables, so that no warp waits on a divergent slow lane.
 #pragma once
 #include "trimeg_math.cuh"
 
@@ -43,13 +33,12 @@ struct TileCfg {
     static constexpr size_t COEF_BYTES = sizeof(double) * SMAX * SLOT_DOUBLES;
     static constexpr size_t BLOCK_BYTES = COEF_BYTES + 64 * SMAX;
     static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;
-    static constexpr size_t OFF_WBAR = OFF_CTRL + 64 * NBUF + 16 * NBUF;          // one mbarrier per warp (record loads)
-    // per-warp marker staging: the 32 records of the next chunk (cp.async), 128 B each, XOR-swizzled rows
+    // chunk slots: 32 marker records of 128 B (XOR-swizzled rows), filled by cp.async; NWARPS slots
     static constexpr size_t WSTAGE = 32 * 128;
-    static constexpr size_t OFF_STAGE = (OFF_WBAR + 8 * NWARPS + 127) / 128 * 128;
+    static constexpr size_t OFF_STAGE = (OFF_CTRL + 64 * NBUF + 16 * NBUF + 127) / 128 * 128;
     static constexpr size_t BYTES = OFF_STAGE + WSTAGE * NWARPS;
 };
-struct BlockCtrl {   // 64 B per ring entry
+struct BlockCtrl {   // 64 B per ring entry; left = chunks done, pad[0] = chunks cut from the entry
     int sc, begin, end, next, left, ns, patch, k0;
     int pad[8];
 };
@@ -76,19 +65,9 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigne
                  "r"(smem_u32(bar))
                  : "memory");
 }
-// 16 <= bytes, multiple of 16; completion is tracked by the issuing thread's bulk async-group
-__device__ __forceinline__ void tma_bulk_s2g(void* dst, const void* src, unsigned bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void lds128(unsigned addr, double& a, double& b) {
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "r"(addr));
-}
-__device__ __forceinline__ void sts128(unsigned addr, double a, double b) {
-    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(a), "d"(b) : "memory");
 }
 
 struct LdShared {   // coefficient pair fetch from the staged block

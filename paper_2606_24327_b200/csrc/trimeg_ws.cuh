@@ -91,8 +91,13 @@ __device__ __forceinline__ void ws_commit(unsigned char* smem, int b, const DevT
                      (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
 }
 
+#ifdef TRIMEG_MAXNREG
+#define TRIMEG_WS_BOUNDS __maxnreg__(TRIMEG_MAXNREG)
+#else
+#define TRIMEG_WS_BOUNDS __launch_bounds__(C::NTHREADS, 1)
+#endif
 template <class C, int PHASE>
-__global__ void __launch_bounds__(C::NTHREADS, 1)
+__global__ void TRIMEG_WS_BOUNDS
 k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __restrict__ src, Rec* __restrict__ dst, const int* __restrict__ perm,
            RetireList rq, KeyOut ko, CellMap cm, double dt, int* __restrict__ work_counter) {
     using L = WsLayout<C>;
@@ -123,7 +128,13 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
                 BlockCtrl* ctl = ctl_all + b;
                 if (lane == 0) {
                     const int need = ctl->pad[0];
+#ifdef TRIMEG_WAITSTATS
+                    const long long w0 = clock64();
+#endif
                     while (*reinterpret_cast<volatile int*>(&ctl->left) < need) __nanosleep(64);
+#ifdef TRIMEG_WAITSTATS
+                    atomicAdd(rq.count + 2, (int)((clock64() - w0) >> 10));
+#endif
                 }
                 __syncwarp();
             }
@@ -149,7 +160,13 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
         };
         for (unsigned it = 0;; ++it) {
             const int b = it % C::NBUF;
+#ifdef TRIMEG_WAITSTATS
+            const long long w0 = clock64();
+#endif
             mbar_wait(blk_bar + 2 * b, (it / C::NBUF) & 1);
+#ifdef TRIMEG_WAITSTATS
+            if (lane == 0) atomicAdd(rq.count + 3, (int)((clock64() - w0) >> 10));
+#endif
             const BlockCtrl* ctl = ctl_all + b;
             if (ctl->sc < 0) break;
             const int begin = ctl->begin, end = ctl->end;
@@ -199,7 +216,13 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
         for (;;) {
             const unsigned t = __shfl_sync(FULL, t_next, 0);
             const unsigned s = t % L::K, g = t / L::K;
+#ifdef TRIMEG_WAITSTATS
+            const long long w0 = clock64();
+#endif
             mbar_wait(full_bar + s, g & 1);
+#ifdef TRIMEG_WAITSTATS
+            if (lane == 0) atomicAdd(rq.count + 1, (int)((clock64() - w0) >> 10));
+#endif
             const int m0 = desc[s].m0, end = desc[s].end, b = desc[s].b;
             if (m0 < 0) break;
             const int m = m0 + lane;

@@ -253,6 +253,18 @@ def test_cfg1_full_size_sampled():
     _check_push(o, g, m, cfg, cfg.dt, 10, 0, sample=sample)
 
 
+def test_cfg3_mesh_two_phase_sorted_every_step():
+    """BASELINE configs[3]'s mesh and fields (80 080 triangles, 64 planes, EM) in the configuration bench.py times
+    (variant 0, both phases re-sorted every step), with 2e6 of its markers: the oracle checks a strided 4 000-marker
+    sample of the state after 5 steps, and every marker's status."""
+    cfg = dataclasses.replace(synth.CONFIGS[3], n_markers=2_000_000)
+    RZ, tri, o, g, m = _make(cfg)
+    sample = np.arange(0, cfg.n_markers, 500)
+    res, exp = _check_push(o, g, m, cfg, cfg.dt, 5, 0, sort_every=1, sample=sample)
+    st = g.push_stats()
+    assert st["sorts"] == 10 and st["retired"] < 0.02 * 10 * cfg.n_markers  # two permutations per step; the follow-up path stays rare
+
+
 # ------------------------------------------------------------------------------------------- errors
 def test_error_behaviour():
     import torch
