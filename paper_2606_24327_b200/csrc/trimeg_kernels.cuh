@@ -386,8 +386,9 @@ __device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int
         xi = fma(g.a11, dx, g.a12 * dy);
         eta = fma(g.a21, dx, g.a22 * dy);
         double l0 = 1.0 - xi - eta;
-        if (fmin(fmin(xi, eta), l0) >= INSIDE_TOL) return sl;
-        int e = (eta <= xi && eta <= l0) ? 0 : ((l0 <= xi) ? 1 : 2);
+        // three compares chained on a predicate instead of two fmin (no DMNMX on sm_100: each fmin is a compare + 4 selects)
+        if (xi >= INSIDE_TOL && eta >= INSIDE_TOL && l0 >= INSIDE_TOL) return sl;
+        const int e = (eta <= xi && eta <= l0) ? 0 : ((l0 <= xi) ? 1 : 2);
         sl = g.nbr[e];
         if (sl < 0) return sl;
     }

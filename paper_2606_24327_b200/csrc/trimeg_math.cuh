@@ -46,8 +46,24 @@ struct BoxGrid {
 
 struct Fields { double P, PR, PZ, Pp, A, AR, AZ, Ap; };   // values, d/dR, d/dZ, raw d/dphi
 
-__device__ __forceinline__ double rcp_nr(double x) {   // 1/x: hardware seed + Newton; full double accuracy for normal x
-    return __drcp_rn(x);
+// 1/x and 1/sqrt(x) for normal positive-or-negative x (R, q, B, B*_par, r^2 ...): hardware seed (MUFU, ~2^-20) and two
+// Newton steps in FMA form, without the denormal / infinity side path of the library routines (a branch and a call each).
+__device__ __forceinline__ double rcp_nr(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+__device__ __forceinline__ double rsqrt_nr(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double hx = 0.5 * x;
+    double e = fma(-hx * y, y, 0.5);      // (1 - x y^2) / 2
+    y = fma(y, e, y);
+    e = fma(-hx * y, y, 0.5);
+    return fma(y, e, y);
 }
 
 // ---- toroidal uniform periodic cubic B-spline (L35) -------------------------------------------------
@@ -253,14 +269,14 @@ struct Equil {
 __device__ __forceinline__ void equil_eval(const EquilP& e, double R, double Z, Equil& o) {
     double x = R - e.R0;
     double r2 = fma(x, x, Z * Z);
-    double inv_r = rsqrt(r2), r = r2 * inv_r;
+    double inv_r = rsqrt_nr(r2), r = r2 * inv_r;
     double xa = r * e.inv_a;
     double q = fma(xa, fma(e.q2, xa, e.q1), e.q0);
     double dq = fma(2.0 * e.q2, xa, e.q1) * e.inv_a;
     double qb = q, dqb = dq;
     if (e.qbar_sqrt) {
         double s2 = fma(-r2, e.inv_R0sq, 1.0);
-        double inv_s = rsqrt(s2), s = s2 * inv_s;
+        double inv_s = rsqrt_nr(s2), s = s2 * inv_s;
         double ds = -r * e.inv_R0sq * inv_s;
         qb = q * s;
         dqb = fma(dq, s, q * ds);
@@ -278,7 +294,7 @@ __device__ __forceinline__ void equil_eval(const EquilP& e, double R, double Z, 
     double BZ_R = (pRR - BZ) * iR, BZ_Z = pRZ * iR;
     double Bp_R = -Bp * iR;
     double B2 = fma(BR, BR, fma(BZ, BZ, Bp * Bp));
-    double iB = rsqrt(B2), B = B2 * iB;
+    double iB = rsqrt_nr(B2), B = B2 * iB;
     double gR = fma(BR, BR_R, fma(BZ, BZ_R, Bp * Bp_R)) * iB;
     double gZ = fma(BR, BR_Z, BZ * BZ_Z) * iB;
     double bR = BR * iB, bZ = BZ * iB, bp = Bp * iB;
