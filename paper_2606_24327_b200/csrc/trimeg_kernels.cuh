@@ -197,7 +197,10 @@ __device__ __forceinline__ void gather_at(const DevTables& tb, int t, double R, 
     to_fields(g, acc, f);
 }
 
-__global__ void __launch_bounds__(256) k_gather(DevTables tb, long long n, const double* __restrict__ R, const double* __restrict__ Z,
+#ifndef TRIMEG_GATHER_BLOCKS
+#define TRIMEG_GATHER_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(256, TRIMEG_GATHER_BLOCKS) k_gather(DevTables tb, long long n, const double* __restrict__ R, const double* __restrict__ Z,
                                                 const double* __restrict__ phi, double* __restrict__ out, int* __restrict__ tri_out) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= n) return;
