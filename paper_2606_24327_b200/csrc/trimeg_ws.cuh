@@ -20,10 +20,13 @@ struct ChunkDesc { int m0, end, b, pad; };   // m0 < 0: no more work
 
 template <class C>
 struct WsLayout {
-    static constexpr int K = C::NWARPS;                                  // chunk slots (4 KB each, in the staging area)
+#ifndef TRIMEG_NSLOTS
+#define TRIMEG_NSLOTS 20
+#endif
+    static constexpr int K = TRIMEG_NSLOTS;                              // chunk slots (4 KB each): one per compute warp + look-ahead
     static constexpr int NPUB = 2;                                       // publisher warps (tickets of parity pid)
     static constexpr int NCONS = C::NWARPS - 1 - NPUB;
-    static constexpr size_t OFF_DESC = C::OFF_STAGE + C::WSTAGE * C::NWARPS;
+    static constexpr size_t OFF_DESC = C::OFF_STAGE + C::WSTAGE * K;
     static constexpr size_t OFF_FULL = OFF_DESC + 16 * K;
     static constexpr size_t OFF_EMPTY = OFF_FULL + 8 * K;
     static constexpr size_t OFF_HEAD = OFF_EMPTY + 8 * K;
@@ -234,11 +237,7 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
 #pragma unroll
                 for (int j = 0; j < 7; ++j) lds128(a + 16 * (j ^ (lane & 7)), rd[2 * j], rd[2 * j + 1]);
             }
-            __syncwarp();
-            if (lane == 0) {
-                mbar_arrive(empty_bar + s);                        // the slot may be refilled
-                t_next = (unsigned)atomicAdd(cons_head, 1);        // next ticket: its latency hides behind the arithmetic
-            }
+            if (lane == 0) t_next = (unsigned)atomicAdd(cons_head, 1);   // next ticket: its latency hides behind the arithmetic
 
             const double* coef = reinterpret_cast<const double*>(smem + C::BLOCK_BYTES * b);
             const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
@@ -284,7 +283,6 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
                     const int sl = slot_walk(sgeom, slot, next[0], next[1], xi, eta);
                     const int tn = sl >= 0 ? sgeom[sl].tri : locate_walk(tb.bg, tb.geom, tri_last, next[0], next[1]);
                     r.st = st; r.tri = tn;
-                    rec_store(dst, m, r);
                     if (ko.enabled) {
                         double sf;
                         const int k = toroidal_interval(tb.tor, next[2], sf);
@@ -293,12 +291,27 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
                         atomicAdd(ko.hist + key, 1);
                     }
                 } else {
-                    // the follow-up kernel redoes this phase through the global tables, reading src again and writing dst[m]
+                    // the follow-up kernel redoes this phase through the global tables; r is unchanged and goes to dst[m] as it
+                    // is (when the phase works in place, dst[m] is also what the follow-up kernel reads)
                     rq.list[atomicAdd(rq.count, 1)] = m;
                 }
+                // the record goes back into its row of the chunk slot, now in the swizzle of its position in dst ...
+                const unsigned a = smem_u32(smem + C::OFF_STAGE + (size_t)s * C::WSTAGE) + lane * 128;
+                const double* rs = reinterpret_cast<const double*>(&r);
+#pragma unroll
+                for (int j = 0; j < 7; ++j) sts128(a + 16 * (j ^ (m & 7)), rs[2 * j], rs[2 * j + 1]);
             }
+            // ... and the chunk leaves as ONE bulk copy (32 scattered 128-byte lines would cost 224 LSU wavefronts as STG.128)
+            fence_async_smem();
             __syncwarp();
-            if (lane == 0) { __threadfence_block(); atomicAdd(&ctl->left, 1); }   // one more chunk of this ring entry done
+            if (lane == 0) {
+                tma_bulk_s2g(dst + m0, smem + C::OFF_STAGE + (size_t)s * C::WSTAGE, (unsigned)(min(32, end - m0) * 128));
+                bulk_commit();
+                __threadfence_block();
+                atomicAdd(&ctl->left, 1);        // one more chunk of this ring entry done
+                bulk_wait_read0();               // the copy has read the slot:
+                mbar_arrive(empty_bar + s);      // it may be refilled
+            }
         }
     }
 }
