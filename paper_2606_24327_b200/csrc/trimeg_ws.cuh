@@ -6,11 +6,12 @@
 // is taken off the compute warps:
 //   warp 0  "stager"    : takes super-cells off the work list, waits until a ring entry is free, fills it (slot geometry
 //                         + TMA bulk copies of the coefficient blocks);
-//   warp 1  "publisher" : once an entry has landed, cuts its marker range into chunks of 32 and, for each, copies the
+//   warps 1-2 "publishers": once an entry has landed, cuts its marker range into chunks of 32 and, for each, copies the
 //                         32 records into a free chunk slot (cp.async through the sort permutation; completion is
 //                         signalled on the slot's mbarrier by cp.async.mbarrier.arrive);
-//   warps 2.. "compute" : take chunk slots in ticket order, pull their record into registers, free the slot, evaluate
-//                         the phase, store the record, and count the chunk done on its ring entry.
+//   warps 3.. "compute" : take chunk slots in ticket order, pull their record into registers, evaluate the phase, put
+//                         the record back into its slot row, send the chunk off as one bulk store, free the slot and
+//                         count the chunk done on its ring entry.
 // A ring entry is refilled when all chunks cut from it are done, not when every warp has walked past it.
 #pragma once
 
