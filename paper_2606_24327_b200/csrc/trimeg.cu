@@ -210,7 +210,7 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     const long long tri_stride = (long long)(n_planes + 3 + 2 * PLANE_PAD) * PLANE_STRIDE;
     const size_t coef_bytes = (size_t)T * tri_stride * sizeof(double);
     trimeg_host::HostPatches hp;
-    trimeg_host::build_patches(hm, RZ, n_nodes, T, Tile::TP, Tile::SMAX, axis_p, 3.0, hp);
+    trimeg_host::build_patches(hm, RZ, n_nodes, T, Tile::TP, Tile::SGEOM, axis_p, 3.0, hp);
     const int nwin = (n_planes + Tile::WK - 1) / Tile::WK;
     ctx->cm.P = n_planes; ctx->cm.nwin = nwin;
     ctx->ncell = (long long)hp.npatch * nwin * Tile::CPS;

@@ -35,10 +35,11 @@ struct DevTables {
     long long tri_stride;    // doubles per triangle = (P+3+2*PLANE_PAD)*42
 };
 
-// tiled push configuration: patches of 8 triangles + halo (16 slots), windows of 4 toroidal intervals (+1 each side),
+// tiled push configuration: patches of 8 triangles + halo (15 slots with coefficients, 32 with geometry), windows of 4 toroidal
+// intervals (+1 each side),
 // ring of 3 staged blocks, 16 independent warps per CTA, one CTA per SM
 #ifndef TRIMEG_SMAX
-#define TRIMEG_SMAX 16
+#define TRIMEG_SMAX 15
 #endif
 #ifndef TRIMEG_NWARPS
 #define TRIMEG_NWARPS 16

@@ -31,7 +31,13 @@ struct TileCfg {
     static constexpr int NBUF = NBUF_;               // ring of staged blocks
     // shared memory carve-up (bytes): NBUF x { coefficients, slot geometry }, then the control words
     static constexpr size_t COEF_BYTES = sizeof(double) * SMAX * SLOT_DOUBLES;
-    static constexpr size_t BLOCK_BYTES = COEF_BYTES + 64 * SMAX;
+    // slot GEOMETRY (64 B per slot) is staged for SGEOM slots, coefficients only for the first SMAX of them: the walk that
+    // locates the next phase's first evaluation point needs no coefficients and stays in shared memory further out
+#ifndef TRIMEG_SGEOM
+#define TRIMEG_SGEOM 32
+#endif
+    static constexpr int SGEOM = TRIMEG_SGEOM;
+    static constexpr size_t BLOCK_BYTES = COEF_BYTES + 64 * SGEOM;
     static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;
     // chunk slots: 32 marker records of 128 B (XOR-swizzled rows), filled by cp.async; NWARPS slots
     static constexpr size_t WSTAGE = 32 * 128;

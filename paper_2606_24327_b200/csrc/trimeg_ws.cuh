@@ -27,6 +27,7 @@ struct WsLayout {
     static constexpr int K = TRIMEG_NSLOTS;                              // chunk slots (4 KB each): one per compute warp + look-ahead
     static constexpr int NPUB = 2;                                       // publisher warps (tickets of parity pid)
     static constexpr int NCONS = C::NWARPS - 1 - NPUB;
+    static_assert(K % NPUB == 0, "a chunk slot is always served by the same publisher warp (an odd K hung on the GPU)");
     static constexpr size_t OFF_DESC = C::OFF_STAGE + C::WSTAGE * K;
     static constexpr size_t OFF_FULL = OFF_DESC + 16 * K;
     static constexpr size_t OFF_EMPTY = OFF_FULL + 8 * K;
@@ -42,7 +43,7 @@ __device__ __forceinline__ void mbar_arrive(void* bar) { asm volatile("mbarrier.
 struct StageWork { int sc, begin, end, patch, k0, ns, t; SlotGeom g; };
 template <class C>
 __device__ __forceinline__ bool ws_fetch(const DevTables& tb, const TileTables& tt, int* work_counter, int lane, StageWork& w) {
-    static_assert(C::SMAX <= 32, "one slot per lane");
+    static_assert(C::SMAX <= C::SGEOM && C::SGEOM <= 32, "one slot per lane");
     constexpr unsigned FULL = 0xffffffffu;
     int sc = 0, begin = 0, end = 0;
     for (;;) {
@@ -59,11 +60,11 @@ __device__ __forceinline__ bool ws_fetch(const DevTables& tb, const TileTables& 
     SlotGeom& g = w.g;
     g.v0x = g.v0y = 1e300; g.a11 = g.a12 = g.a21 = g.a22 = 0.0; g.nbr[0] = g.nbr[1] = g.nbr[2] = g.nbr[3] = -1;
     if (lane < w.ns) {
-        w.t = tt.slots[(long long)w.patch * C::SMAX + lane];
+        w.t = tt.slots[(long long)w.patch * C::SGEOM + lane];
         if (w.t >= 0) {
             const TriGeom tg = tb.geom[w.t];
             g.v0x = tg.v0x; g.v0y = tg.v0y; g.a11 = tg.a11; g.a12 = tg.a12; g.a21 = tg.a21; g.a22 = tg.a22;
-            const short* nb = tt.nbr + ((long long)w.patch * C::SMAX + lane) * 4;
+            const short* nb = tt.nbr + ((long long)w.patch * C::SGEOM + lane) * 4;
             g.nbr[0] = nb[0]; g.nbr[1] = nb[1]; g.nbr[2] = nb[2];
         }
     }
@@ -84,13 +85,14 @@ __device__ __forceinline__ void ws_commit(unsigned char* smem, int b, const DevT
         *reinterpret_cast<volatile int*>(&ctl->left) = 0;             // chunks done
     }
     if (lane < w.ns) sgeom[lane] = w.g;
-    const int cnt = __popc(__ballot_sync(FULL, w.t >= 0));
+    const bool has_coef = w.t >= 0 && lane < C::SMAX;
+    const int cnt = __popc(__ballot_sync(FULL, has_coef));
     __threadfence_block();
     fence_async_smem();   // earlier generic accesses of this block vs. the async writes
     __syncwarp();
     if (lane == 0) mbar_expect_tx(mbar, (unsigned)(cnt * C::SLOT_DOUBLES * sizeof(double)));
     __syncwarp();
-    if (w.t >= 0)
+    if (has_coef)
         tma_bulk_g2s(coef + (size_t)lane * C::SLOT_DOUBLES, tb.coef + (long long)w.t * tb.tri_stride + (long long)w.k0 * PLANE_STRIDE,
                      (unsigned)(C::SLOT_DOUBLES * sizeof(double)), mbar);
 }
@@ -261,7 +263,7 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
                     int dk = k - k0;
                     if (dk > P / 2) dk -= P; else if (dk < -(P / 2)) dk += P;
                     const int lk = dk + C::HK;
-                    if (!(sl >= 0 && lk >= 0 && lk < C::NW)) return false;
+                    if (!(sl >= 0 && sl < C::SMAX && lk >= 0 && lk < C::NW)) return false;   // slots >= SMAX carry geometry only
                     slot = sl;
                     const SlotGeom& gg = sgeom[sl];
                     tri_last = gg.tri;
