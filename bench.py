@@ -32,7 +32,7 @@ UNIT = "marker-pushes/s"
 FLOP_PER_PUSH = 3772.0          # 943 flop per RK stage x 4
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
 KEYS = ("R", "Z", "phi", "u", "w", "mu", "p")
-TRAFFIC_BYTES_PER_LAUNCH = 31.97e9   # dram__bytes_read.sum + dram__bytes_write.sum of one k_phase_ws launch (profiles/r01d_summary.md)
+TRAFFIC_BYTES_PER_LAUNCH = 28.68e9   # dram__bytes_read.sum + dram__bytes_write.sum of one k_phase_ws launch (profiles/r01e_summary.md)
 ALGO_BYTES_PER_LAUNCH = 2 * 112 + 8 + 17   # per marker: 112 live record bytes in and out, permutation + key, one pass over the coefficient table
 SORT_EVERY = 1                  # two-phase kernel: both phases re-bin every step (BASELINE configs[2] uses 10)
 
