@@ -240,7 +240,9 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* __res
 #pragma unroll
                 for (int j = 0; j < 7; ++j) lds128(a + 16 * (j ^ (lane & 7)), rd[2 * j], rd[2 * j + 1]);
             }
-            if (lane == 0) t_next = (unsigned)atomicAdd(cons_head, 1);   // next ticket: its latency hides behind the arithmetic
+            // next ticket now, so that its latency hides behind the arithmetic (volatile asm: as a plain atomicAdd the
+            // compiler sinks it to the end of the iteration, next to the other lane-0 work, and its latency is exposed)
+            if (lane == 0) asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(t_next) : "r"(smem_u32(cons_head)) : "memory");
 
             const double* coef = reinterpret_cast<const double*>(smem + C::BLOCK_BYTES * b);
             const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
