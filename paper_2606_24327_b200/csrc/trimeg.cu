@@ -244,6 +244,7 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     ctx->tt.npatch = hp.npatch; ctx->tt.nwin = nwin; ctx->tt.nsc = hp.npatch * nwin;
     CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WsLayout<Tile>::BYTES));
     CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WsLayout<Tile>::BYTES));
+    CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_INIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WsLayout<Tile>::BYTES));
     CU(cudaMemcpyAsync(ctx->d_geom, geom.data(), sizeof(TriGeom) * T, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_tri, hm.tri.data(), sizeof(int) * 3 * T, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_head, hm.head.data(), sizeof(int) * hm.head.size(), cudaMemcpyHostToDevice, ctx->stream));
@@ -474,9 +475,19 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps) {
                 ko.keys = ctx->d_keys; ko.hist = ctx->d_hist; ko.ncell = (int)ctx->ncell; ko.enabled = need_sort ? 1 : 0;
                 CU(cudaMemsetAsync(ctx->d_hist, 0, sizeof(int) * (ctx->ncell + 2), ctx->stream));
                 Rec* recs = ctx->recs[ctx->cur];
-                k_phase_global<PHASE_INIT><<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->cm, ko, recs, recs, nullptr, nullptr, nullptr,
-                                                                                        nullptr, n, dt);
-                KCHECK();
+                if (need_sort) {
+                    // bin by the cell of y_n itself, then let the phase kernel compute k1 in that order (it also writes the
+                    // keys of the half-step points for phase A)
+                    ko.enabled = 1;
+                    k_locate_keys<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, ctx->cm, ko, recs, n);
+                    KCHECK();
+                    int rc = run_phase<PHASE_INIT>(ctx, dt, true, true, nullptr);
+                    if (rc) return rc;
+                } else {
+                    k_phase_global<PHASE_INIT><<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->cm, ko, recs, recs, nullptr, nullptr,
+                                                                                            nullptr, nullptr, n, dt);
+                    KCHECK();
+                }
                 ctx->k1_valid = true; ctx->key_dt = dt; ctx->keys_valid = need_sort;
                 ctx->stats[0] += 1;
             }

@@ -329,6 +329,23 @@ __global__ void __launch_bounds__(128) k_phase_global(DevTables tb, EquilP ep, S
     }
 }
 
+// first step after a bind: triangle and cell key of every marker's CURRENT position (box-grid locate), so that k1 = f(y_n)
+// can be computed by the phase kernel in cell order instead of through the global tables in caller order
+__global__ void __launch_bounds__(256) k_locate_keys(DevTables tb, CellMap cm, KeyOut ko, Rec* __restrict__ recs, long long n) {
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    Rec r;
+    rec_load(recs, i, r);
+    const int t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
+    r.tri = t;
+    reinterpret_cast<double2*>(recs + i)[6 ^ (int)(i & 7)] = reinterpret_cast<const double2*>(&r)[6];   // (tri, st, id, pad0)
+    double sf;
+    const int k = toroidal_interval(tb.tor, r.y[2], sf);
+    const int key = t < 0 ? ko.ncell : cm.cell(t, k);
+    ko.keys[i] = key;
+    atomicAdd(ko.hist + key, 1);
+}
+
 // variant 1: the whole classical RK4 step, one thread per marker, in place, coefficients through L1/L2 (reference for the
 // two-phase path; leaves the records' k stale)
 __global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, SpeciesP sp, Rec* __restrict__ recs, long long n, double dt) {
