@@ -362,15 +362,18 @@ int trimeg_markers_get(trimeg_ctx* ctx, double* R, double* Z, double* phi, doubl
     CU(cudaSetDevice(ctx->device));
     const long long n = ctx->n;
     const Rec* recs = ctx->recs[ctx->cur];
+    // the retire list is free between phases: it holds the caller id -> record position map
+    k_inv_ids<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(recs, n, ctx->d_retired);
+    KCHECK();
     if (memspace == TRIMEG_DEVICE) {
-        k_get<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(recs, n, R, Z, phi, u, w, status);
+        k_get<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(recs, ctx->d_retired, n, R, Z, phi, u, w, status);
         KCHECK();
         return TRIMEG_OK;
     }
     // HOST: un-sort into the inactive record buffer (free between steps), then copy out
     double* st = (double*)ctx->recs[ctx->cur ^ 1];
     int* sti = (int*)(st + 5 * n);
-    k_get<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(recs, n, R ? st : nullptr, Z ? st + n : nullptr, phi ? st + 2 * n : nullptr, u ? st + 3 * n : nullptr,
+    k_get<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(recs, ctx->d_retired, n, R ? st : nullptr, Z ? st + n : nullptr, phi ? st + 2 * n : nullptr, u ? st + 3 * n : nullptr,
                                                         w ? st + 4 * n : nullptr, status ? sti : nullptr);
     KCHECK();
     double* dst[5] = {R, Z, phi, u, w};

@@ -161,13 +161,21 @@ __global__ void k_bind(Rec* __restrict__ recs, long long first, long long cnt, c
     r.pad[0] = r.pad[1] = 0.0;
     rec_store(recs, first + i, r);
 }
-// records -> SoA arrays in the caller's order (any may be null)
-__global__ void k_get(const Rec* __restrict__ recs, long long n, double* R, double* Z, double* phi, double* u, double* w, int* status) {
+// records -> SoA arrays in the caller's order (any may be null), in two steps so that the 8-byte writes are coalesced:
+// inv[caller id] = record position (one scattered 4-byte write per marker), then one thread per caller id reads its
+// record (a whole line) and writes the arrays in order.
+__global__ void k_inv_ids(const Rec* __restrict__ recs, long long n, int* __restrict__ inv) {
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    const int2 v = __ldcs(reinterpret_cast<const int2*>(reinterpret_cast<const double2*>(recs + i) + (6 ^ (int)(i & 7))) + 1);   // (id, pad0)
+    inv[v.x] = (int)i;
+}
+__global__ void k_get(const Rec* __restrict__ recs, const int* __restrict__ inv, long long n, double* R, double* Z, double* phi, double* u, double* w,
+                      int* status) {
+    long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= n) return;
     Rec r;
-    rec_load(recs, i, r);
-    const long long o = r.id;
+    rec_load(recs, inv[o], r);
     if (R) R[o] = r.y[0];
     if (Z) Z[o] = r.y[1];
     if (phi) phi[o] = r.y[2];
