@@ -310,7 +310,7 @@ def main():
                 "ms_per_step": 1e3 * total_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, n, args), "clocks": clocks,
                 "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 7 * 8 * n, "d2h_bytes_per_step": (5 * 8 + 4) * n, "steps": e2e_steps,
-                        "note": "every e2e step re-binds from HOST buffers, so it also pays the k1 initialisation of an unsorted store; PCIe-bound"},
+                        "note": "every e2e step re-binds from HOST buffers, so it also pays the locate + k1 initialisation of a fresh store; PCIe-bound"},
                 "gpu_launches": launches,
                 "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
                              "traffic": TRAFFIC_BYTES_PER_LAUNCH if (args.variant == 0 and args.config == 3 and n == cfg.n_markers) else None,
