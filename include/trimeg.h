@@ -137,6 +137,12 @@ int trimeg_rhs(trimeg_ctx* ctx, double* out, int memspace);
  * 1 = simple (whole RK4 step, one thread per marker, coefficients through L1/L2).  Both compute the same thing. */
 int trimeg_set_push_variant(trimeg_ctx* ctx, int32_t variant);
 
+/* Which push kernel trimeg_push_rk4 will actually run with the loaded mesh: *out = 0 (two-phase kernel) or 1 (simple).
+ * Variant 0 needs n_planes >= 6 (a staged window of 4 toroidal intervals plus one on either side must not alias under
+ * the periodic wrap); with fewer planes variant 1 runs whatever trimeg_set_push_variant selected.
+ * Errors: BAD_ARG, BAD_STATE (no mesh). */
+int trimeg_push_variant_used(trimeg_ctx* ctx, int32_t* out);
+
 /* Diagnostics used by the benchmark: achieved FP64 FMA throughput of this device in TFLOP/s
  * (a register-only DFMA loop; the roofline's measured "alu" peak). */
 int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops);

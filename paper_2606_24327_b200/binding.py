@@ -20,7 +20,7 @@ EXPORTS = [
     "trimeg_create", "trimeg_destroy", "trimeg_sync", "trimeg_last_error", "trimeg_equilibrium_set",
     "trimeg_species_set", "trimeg_mesh_load", "trimeg_fields_set", "trimeg_gather", "trimeg_scratch_bytes",
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
-    "trimeg_rhs", "trimeg_set_push_variant", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
+    "trimeg_rhs", "trimeg_set_push_variant", "trimeg_push_variant_used", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
 ]
 
 
@@ -75,6 +75,7 @@ def load_library():
     lib.trimeg_push_rk4.argtypes = [vp, dbl, i32]
     lib.trimeg_rhs.argtypes = [vp, vp, C.c_int]
     lib.trimeg_set_push_variant.argtypes = [vp, i32]
+    lib.trimeg_push_variant_used.argtypes = [vp, C.POINTER(i32)]
     lib.trimeg_bench_dfma.argtypes = [vp, C.POINTER(dbl)]
     lib.trimeg_push_stats.argtypes = [vp, C.POINTER(i64)]
     lib.trimeg_push_kernel_ms.argtypes = [vp, C.POINTER(dbl)]
@@ -223,6 +224,11 @@ class Trimeg:
 
     def set_push_variant(self, variant):
         self._ck(self._lib.trimeg_set_push_variant(self._h, int(variant)), "trimeg_set_push_variant")
+
+    def push_variant_used(self):
+        v = C.c_int32(-1)
+        self._ck(self._lib.trimeg_push_variant_used(self._h, C.byref(v)), "trimeg_push_variant_used")
+        return v.value
 
     def push_rk4(self, dt, nsteps):
         self._ck(self._lib.trimeg_push_rk4(self._h, float(dt), int(nsteps)), "trimeg_push_rk4")

@@ -28,6 +28,8 @@ struct trimeg_ctx {
     EquilP ep{};
     SpeciesP sp{};
     trimeg_equil eq_in{};
+    trimeg_species sp_in{};
+    int NPP = 0;                 // planes of the padded coefficient table
     // mesh
     int T = 0, P = 0;
     long long n_nodes = 0;
@@ -103,6 +105,19 @@ static void free_mesh(trimeg_ctx* c) {
 // anything the cached k1 / keys depend on has changed
 static void invalidate_step_state(trimeg_ctx* c) { c->k1_valid = false; c->keys_valid = false; }
 
+// device form of the species: Eq.(8) scalars from the raw species and the current equilibrium (a, R0)
+static void derive_species(trimeg_ctx* ctx) {
+    const trimeg_equil& eq = ctx->eq_in;
+    const trimeg_species* s = &ctx->sp_in;
+    SpeciesP& p = ctx->sp;
+    p.qom = s->qom; p.kappa = 1.0 / s->qom;
+    p.kn_R0 = s->kappa_n / eq.R0; p.kT_R0 = s->kappa_T / eq.R0;
+    p.two_inv_wn_a = 2.0 / (s->w_n * eq.a); p.two_inv_wT_a = 2.0 / (s->w_T * eq.a); p.r0 = s->r0;
+    p.cT = s->kappa_T * s->w_T * eq.a / eq.R0;
+    p.same_w = (s->w_n == s->w_T) ? 1 : 0;
+    p.bstar_exact = s->bstar_exact ? 1 : 0; p.weight_mode = s->weight_mode ? 1 : 0;
+}
+
 extern "C" {
 
 int trimeg_create(trimeg_ctx** out, int device, void* cuda_stream) {
@@ -150,9 +165,10 @@ int trimeg_equilibrium_set(trimeg_ctx* ctx, const trimeg_equil* eq) {
         return fail(ctx, TRIMEG_ERR_BAD_ARG, "equilibrium_set: need 0 < a < R0, finite nonzero B0, finite q");
     ctx->eq_in = *eq;
     EquilP& e = ctx->ep;
-    e.R0 = eq->R0; e.B0 = eq->B0; e.F = eq->B0 * eq->R0; e.inv_a = 1.0 / eq->a; e.inv_R0sq = 1.0 / (eq->R0 * eq->R0);
+    e.R0 = eq->R0; e.B0 = eq->B0; e.F = eq->B0 * eq->R0; e.F2 = e.F * e.F; e.inv_a = 1.0 / eq->a; e.inv_R0sq = 1.0 / (eq->R0 * eq->R0);
     e.q0 = eq->q0; e.q1 = eq->q1; e.q2 = eq->q2; e.qbar_sqrt = eq->qbar_sqrt ? 1 : 0;
     ctx->have_eq = true;
+    if (ctx->have_sp) derive_species(ctx);   // the profile scalars of Eq.(8) depend on a and R0
     invalidate_step_state(ctx);
     return TRIMEG_OK;
 }
@@ -162,14 +178,8 @@ int trimeg_species_set(trimeg_ctx* ctx, const trimeg_species* s) {
     if (!ctx->have_eq) return fail(ctx, TRIMEG_ERR_BAD_STATE, "species_set: call trimeg_equilibrium_set first (profiles use a and R0)");
     if (!std::isfinite(s->qom) || s->qom == 0 || !(s->w_n > 0) || !(s->w_T > 0) || !std::isfinite(s->kappa_n + s->kappa_T + s->r0))
         return fail(ctx, TRIMEG_ERR_BAD_ARG, "species_set: need finite nonzero qom, w_n > 0, w_T > 0");
-    const trimeg_equil& eq = ctx->eq_in;
-    SpeciesP& p = ctx->sp;
-    p.qom = s->qom; p.kappa = 1.0 / s->qom;
-    p.kn_R0 = s->kappa_n / eq.R0; p.kT_R0 = s->kappa_T / eq.R0;
-    p.inv_wn_a = 1.0 / (s->w_n * eq.a); p.inv_wT_a = 1.0 / (s->w_T * eq.a); p.r0 = s->r0;
-    p.cT = s->kappa_T * s->w_T * eq.a / eq.R0;
-    p.same_w = (s->w_n == s->w_T) ? 1 : 0;
-    p.bstar_exact = s->bstar_exact ? 1 : 0; p.weight_mode = s->weight_mode ? 1 : 0;
+    ctx->sp_in = *s;
+    derive_species(ctx);
     ctx->have_sp = true;
     invalidate_step_state(ctx);
     return TRIMEG_OK;
@@ -207,15 +217,18 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
         if (!trimeg_host::triangle_K(ec, v, &K[(size_t)t * 18])) return fail(ctx, TRIMEG_ERR_BAD_MESH, "mesh_load: degenerate triangle %d", g.orig);
     }
     ctx->T = T; ctx->P = n_planes; ctx->n_nodes = n_nodes; ctx->period = phi_period;
-    const long long tri_stride = (long long)(n_planes + 3 + 2 * PLANE_PAD) * PLANE_STRIDE;
+    // padded coefficient table: whole windows of Tile::WK intervals, so that the staged plane range of the last window
+    // (which may be partly empty when n_planes is not a multiple of WK) stays inside the triangle's run
+    const int nwin = (n_planes + Tile::WK - 1) / Tile::WK;
+    ctx->NPP = nwin * Tile::WK + 3 + 2 * PLANE_PAD;
+    const long long tri_stride = (long long)ctx->NPP * PLANE_STRIDE;
     const size_t coef_bytes = (size_t)T * tri_stride * sizeof(double);
     trimeg_host::HostPatches hp;
     trimeg_host::build_patches(hm, RZ, n_nodes, T, Tile::TP, Tile::SGEOM, axis_p, 3.0, hp);
-    const int nwin = (n_planes + Tile::WK - 1) / Tile::WK;
     ctx->cm.P = n_planes; ctx->cm.nwin = nwin;
     ctx->ncell = (long long)hp.npatch * nwin * Tile::CPS;
     if ((double)hp.npatch * nwin * Tile::CPS + 2 > 2.0e9) return fail(ctx, TRIMEG_ERR_BAD_ARG, "mesh_load: too many cells for int32 ids");
-    ctx->tiled_ok = (n_planes % Tile::WK == 0) && (n_planes >= Tile::NW);
+    ctx->tiled_ok = n_planes >= Tile::NW;   // fewer planes: the window's wrapped intervals would alias (variant 1 is used instead)
     CU(cudaMalloc(&ctx->d_geom, sizeof(TriGeom) * T));
     CU(cudaMalloc(&ctx->d_tri, sizeof(int) * 3 * T));
     CU(cudaMalloc(&ctx->d_head, sizeof(int) * hm.head.size()));
@@ -242,9 +255,9 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     CU(cudaMemsetAsync(ctx->d_fill, 0, sizeof(int) * ncnt, ctx->stream));
     ctx->tt.slots = ctx->d_pslots; ctx->tt.nbr = ctx->d_pnbr; ctx->tt.nslots = ctx->d_pnslots; ctx->tt.offs = ctx->d_offs;
     ctx->tt.npatch = hp.npatch; ctx->tt.nwin = nwin; ctx->tt.nsc = hp.npatch * nwin;
-    CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WsLayout<Tile>::BYTES));
-    CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WsLayout<Tile>::BYTES));
-    CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_INIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WsLayout<Tile>::BYTES));
+    CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tile::BYTES));
+    CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tile::BYTES));
+    CU(cudaFuncSetAttribute(k_phase_ws<Tile, PHASE_INIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tile::BYTES));
     CU(cudaMemcpyAsync(ctx->d_geom, geom.data(), sizeof(TriGeom) * T, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_tri, hm.tri.data(), sizeof(int) * 3 * T, cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_head, hm.head.data(), sizeof(int) * hm.head.size(), cudaMemcpyHostToDevice, ctx->stream));
@@ -259,6 +272,7 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     tb.bg.nx = hm.nx; tb.bg.ny = hm.ny; tb.bg.head = ctx->d_head; tb.bg.list = ctx->d_list;
     tb.tor.period = phi_period; tb.tor.inv_period = 1.0 / phi_period; tb.tor.P = n_planes;
     tb.tor.inv_dphi = (double)n_planes / phi_period; tb.tor.half_inv_dphi = 0.5 * (double)n_planes / phi_period;
+    tb.tor.m2_inv_dphi = -2.0 * (double)n_planes / phi_period;
     ctx->have_mesh = true;
     invalidate_step_state(ctx);
     ctx->order_valid = false;
@@ -280,7 +294,7 @@ int trimeg_fields_set(trimeg_ctx* ctx, int which, const double* dof, int memspac
         d_dof = tmp;
     }
     long long work = (long long)ctx->T * ctx->P;
-    k_fields_set<<<blocks_for(work, 128), 128, 0, ctx->stream>>>(ctx->T, ctx->P, which, ctx->d_tri, ctx->d_RZ, ctx->d_K, d_dof, ctx->n_nodes, ctx->d_coef);
+    k_fields_set<<<blocks_for(work, 128), 128, 0, ctx->stream>>>(ctx->T, ctx->P, which, ctx->d_tri, ctx->d_RZ, ctx->d_K, d_dof, ctx->n_nodes, ctx->NPP, ctx->d_coef);
     cudaError_t e = cudaGetLastError();
     if (tmp) { cudaStreamSynchronize(ctx->stream); cudaFree(tmp); }
     if (e != cudaSuccess) return fail(ctx, TRIMEG_ERR_CUDA, "fields_set kernel: %s", cudaGetErrorString(e));
@@ -430,14 +444,14 @@ static int run_phase(trimeg_ctx* ctx, double dt, bool sort_now, bool keys_out, c
     }
     KeyOut ko;
     ko.keys = ctx->d_keys; ko.hist = ctx->d_hist; ko.ncell = (int)ctx->ncell; ko.enabled = keys_out ? 1 : 0;
-    RetireList rq{ctx->d_retired, ctx->d_work + 4};
+    RetireList rq{ctx->d_retired, ctx->d_work + 4, (int)ctx->n};
     CU(cudaMemsetAsync(ctx->d_work, 0, 8 * sizeof(int), ctx->stream));
     // a phase that re-sorts moves the records into the other buffer in cell order; otherwise it works in place in the stale order
     const Rec* src = ctx->recs[ctx->cur];
     Rec* dst = ctx->recs[sort_now ? ctx->cur ^ 1 : ctx->cur];
     const int* perm = sort_now ? ctx->d_perm : nullptr;
     if (ev) CU(cudaEventRecord(ev[0], ctx->stream));
-    k_phase_ws<Tile, PHASE><<<ctx->num_sms, Tile::NTHREADS, WsLayout<Tile>::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, src, dst, perm, rq, ko, ctx->cm, dt,
+    k_phase_ws<Tile, PHASE><<<ctx->num_sms, Tile::NTHREADS, Tile::BYTES, ctx->stream>>>(ctx->tb, ctx->tt, ctx->ep, ctx->sp, src, dst, perm, rq, ko, ctx->cm, dt,
                                                                                            ctx->d_work);
     KCHECK();
     if (ev) CU(cudaEventRecord(ev[1], ctx->stream));
@@ -448,11 +462,13 @@ static int run_phase(trimeg_ctx* ctx, double dt, bool sort_now, bool keys_out, c
     k_phase_global<PHASE><<<ctx->num_sms * 2, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->cm, ko, src, dst, perm, nullptr, ctx->d_offs + ctx->ncell,
                                                                       nullptr, ctx->n, dt);
     KCHECK();
+    k_fix_keys<PHASE><<<ctx->num_sms * 2, 128, 0, ctx->stream>>>(ctx->tb, ctx->cm, ko, dst, ctx->d_retired, ctx->d_work + 5, ctx->n, dt);
+    KCHECK();
     if (sort_now) ctx->cur ^= 1;
     k_accumulate_stat<<<1, 1, 0, ctx->stream>>>(ctx->d_work + 4, ctx->d_stats + 1);
     KCHECK();
     if (ev) CU(cudaEventRecord(ev[2], ctx->stream));
-    ctx->stats[0] += 4;
+    ctx->stats[0] += 5;
     return TRIMEG_OK;
 }
 
@@ -515,6 +531,13 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps) {
         }
         if (timed) ctx->ev_valid = true;
     }
+    return TRIMEG_OK;
+}
+
+int trimeg_push_variant_used(trimeg_ctx* ctx, int32_t* out) {
+    if (!ctx || !out) return fail(ctx, TRIMEG_ERR_BAD_ARG, "push_variant_used: null argument");
+    if (!ctx->have_mesh) return fail(ctx, TRIMEG_ERR_BAD_STATE, "push_variant_used: call trimeg_mesh_load first");
+    *out = (ctx->variant == 0 && ctx->tiled_ok) ? 0 : 1;
     return TRIMEG_OK;
 }
 
@@ -591,9 +614,6 @@ int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]) {
         CU(cudaSetDevice(ctx->device));
         CU(cudaMemcpyAsync(h, ctx->d_stats, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
-#ifdef TRIMEG_WAITSTATS
-        fprintf(stderr, "waitstats kcycles: compute-warps-for-chunk %llu  stager-for-free-entry %llu  publishers-for-block %llu\n", h[2], h[3], h[0]);
-#endif
         out[1] = (int64_t)(2 * h[1]);   // each follow-up marker-phase is two right-hand-side evaluations
         out[2] = (int64_t)h[1];
     }

@@ -35,22 +35,22 @@ struct DevTables {
     long long tri_stride;    // doubles per triangle = (P+3+2*PLANE_PAD)*42
 };
 
-// tiled push configuration: patches of 8 triangles + halo (15 slots with coefficients, 32 with geometry), windows of 4 toroidal
-// intervals (+1 each side),
-// ring of 3 staged blocks, 16 independent warps per CTA, one CTA per SM
+// tiled push configuration: patches of 8 triangles + halo (SMAX slots with coefficients, 32 with geometry), windows of 4
+// toroidal intervals (+1 each side), ring of NBUF staged blocks, K chunk slots of 64 records, 4 producer + 4 locator + 8
+// compute warps per CTA, one CTA per SM.  (TRIMEG_* macros: tuning sweeps only; the shipped build uses the defaults.)
 #ifndef TRIMEG_SMAX
-#define TRIMEG_SMAX 15
-#endif
-#ifndef TRIMEG_NWARPS
-#define TRIMEG_NWARPS 16
+#define TRIMEG_SMAX 13
 #endif
 #ifndef TRIMEG_NBUF
-#define TRIMEG_NBUF 3
+#define TRIMEG_NBUF 2
 #endif
-#ifndef TRIMEG_CTAS_PER_SM
-#define TRIMEG_CTAS_PER_SM 1
+#ifndef TRIMEG_NSLOTS
+#define TRIMEG_NSLOTS 16
 #endif
-using Tile = TileCfg<8, TRIMEG_SMAX, 4, TRIMEG_NWARPS, TRIMEG_NBUF>;
+#ifndef TRIMEG_NCOMP
+#define TRIMEG_NCOMP 8
+#endif
+using Tile = TileCfg<8, TRIMEG_SMAX, 4, TRIMEG_NCOMP, TRIMEG_NBUF, TRIMEG_NSLOTS>;
 // cell numbering used by the sort: super-cell (patch, window) major, then triangle within the patch, then interval
 struct CellMap {
     int P, nwin;
@@ -70,20 +70,22 @@ struct KeyOut {
 __constant__ double c_Aplus[21 * 18];
 __constant__ double c_Nul[21 * 3];
 
-// In memory the eight 16-byte chunks of record i are stored XOR-swizzled by (i & 7): logical chunk j sits at chunk
-// position j ^ (i & 7) (a record is only ever handled whole, so the swizzle costs nothing; it lets row-per-lane shared-memory
-// images of records be read and written 16 bytes per lane without bank conflicts).
+// In memory the eight 16-byte chunks of record i are stored XOR-swizzled by rec_swizzle(i) = (i >> 1) & 7: logical chunk j
+// sits at chunk position j ^ rec_swizzle(i) (a record is only ever handled whole, so the swizzle costs nothing).  In the
+// phase kernel lane l reads rows 2l and 2l + 1 of a chunk slot; with this swizzle the eight lanes of a shared-memory
+// wavefront hit eight different 16-byte bank groups.
+__host__ __device__ __forceinline__ int rec_swizzle(long long i) { return (int)(i >> 1) & 7; }
 __device__ __forceinline__ void rec_load(const Rec* __restrict__ base, long long i, Rec& r) {
     const double2* s = reinterpret_cast<const double2*>(base + i);
     double2* d = reinterpret_cast<double2*>(&r);
-    const int sw = (int)(i & 7);
+    const int sw = rec_swizzle(i);
 #pragma unroll
     for (int j = 0; j < 7; ++j) d[j] = __ldcs(s + (j ^ sw));   // 14 doubles are live; the last chunk is padding
 }
 __device__ __forceinline__ void rec_store(Rec* __restrict__ base, long long i, const Rec& r) {
     double2* d = reinterpret_cast<double2*>(base + i);
     const double2* s = reinterpret_cast<const double2*>(&r);
-    const int sw = (int)(i & 7);
+    const int sw = rec_swizzle(i);
 #pragma unroll
     for (int j = 0; j < 7; ++j) d[j ^ sw] = s[j];
 }
@@ -92,7 +94,7 @@ __device__ __forceinline__ void rec_store(Rec* __restrict__ base, long long i, c
 // fields_set: nodal DOFs -> per-triangle reference-frame polynomial coefficients, for one field.
 // One thread per (triangle, plane).  c = c0 - Nul (K c0_5),  c0 = Aplus d_ref,  d_ref = DOFs pulled back with J.
 __global__ void k_fields_set(int T, int P, int which, const int* __restrict__ tri, const double* __restrict__ RZ,
-                             const double* __restrict__ Kmat, const double* __restrict__ dof, long long n_nodes,
+                             const double* __restrict__ Kmat, const double* __restrict__ dof, long long n_nodes, int NPP,
                              double* __restrict__ coef) {
     long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= (long long)T * P) return;
@@ -133,17 +135,15 @@ __global__ void k_fields_set(int T, int P, int which, const int* __restrict__ tr
         for (int m = 0; m < 6; ++m) s = fma(K[r * 6 + m], c[qi[m]], s);
         z[r] = s;
     }
-    const int NPP = P + 3 + 2 * PLANE_PAD;
+    // toroidal plane k sits at every padded index pp = k + 1 + PLANE_PAD (mod P) inside [0, NPP)
     long long tri_stride = (long long)NPP * PLANE_STRIDE;
     double* base = coef + (long long)t * tri_stride;
-    int slots[3];
+    double v[21];
 #pragma unroll
-    for (int s = 0; s < 3; ++s) { int pp = k + 1 + PLANE_PAD + (s - 1) * P; slots[s] = (pp >= 0 && pp < NPP) ? pp : -1; }
+    for (int i = 0; i < 21; ++i) v[i] = c[i] - (c_Nul[i * 3] * z[0] + c_Nul[i * 3 + 1] * z[1] + c_Nul[i * 3 + 2] * z[2]);
+    for (int pp = (k + 1 + PLANE_PAD) % P; pp < NPP; pp += P) {
 #pragma unroll
-    for (int i = 0; i < 21; ++i) {
-        double v = c[i] - (c_Nul[i * 3] * z[0] + c_Nul[i * 3 + 1] * z[1] + c_Nul[i * 3 + 2] * z[2]);
-#pragma unroll
-        for (int s = 0; s < 3; ++s) if (slots[s] >= 0) base[(long long)slots[s] * PLANE_STRIDE + 2 * i + which] = v;
+        for (int i = 0; i < 21; ++i) base[(long long)pp * PLANE_STRIDE + 2 * i + which] = v[i];
     }
 }
 
@@ -167,7 +167,7 @@ __global__ void k_bind(Rec* __restrict__ recs, long long first, long long cnt, c
 __global__ void k_inv_ids(const Rec* __restrict__ recs, long long n, int* __restrict__ inv) {
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const int2 v = __ldcs(reinterpret_cast<const int2*>(reinterpret_cast<const double2*>(recs + i) + (6 ^ (int)(i & 7))) + 1);   // (id, pad0)
+    const int2 v = __ldcs(reinterpret_cast<const int2*>(reinterpret_cast<const double2*>(recs + i) + (6 ^ rec_swizzle(i))) + 1);   // (id, pad0)
     inv[v.x] = (int)i;
 }
 __global__ void k_get(const Rec* __restrict__ recs, const int* __restrict__ inv, long long n, double* R, double* Z, double* phi, double* u, double* w,
@@ -181,7 +181,7 @@ __global__ void k_get(const Rec* __restrict__ recs, const int* __restrict__ inv,
     if (phi) phi[o] = r.y[2];
     if (u) u[o] = r.y[3];
     if (w) w[o] = r.y[4];
-    if (status) status[o] = r.st;
+    if (status) status[o] = r.st & 1;
 }
 
 // ============================================================================================ gather / global path
@@ -202,14 +202,11 @@ __device__ __forceinline__ void gather_at(const DevTables& tb, int t, double R, 
     int kk = bspline_weights(tb.tor, phi, w, dw);
     LdGlobal ld{reinterpret_cast<const double2*>(tb.coef + (long long)t * tb.tri_stride + (long long)(kk + PLANE_PAD) * PLANE_STRIDE)};
     double acc[8];
-    gather_cell(ld, xi, eta, w, dw, acc);
+    gather_cell<true, double>(ld, xi, eta, w, dw, acc);
     to_fields(g, acc, f);
 }
 
-#ifndef TRIMEG_GATHER_BLOCKS
-#define TRIMEG_GATHER_BLOCKS 4
-#endif
-__global__ void __launch_bounds__(256, TRIMEG_GATHER_BLOCKS) k_gather(DevTables tb, long long n, const double* __restrict__ R, const double* __restrict__ Z,
+__global__ void __launch_bounds__(256, 4) k_gather(DevTables tb, long long n, const double* __restrict__ R, const double* __restrict__ Z,
                                                 const double* __restrict__ phi, double* __restrict__ out, int* __restrict__ tri_out) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= n) return;
@@ -228,7 +225,9 @@ __device__ __forceinline__ int stage_simple(const DevTables& tb, const EquilP& e
     t = locate_walk(tb.bg, tb.geom, t, R, Z);
     Fields f;
     gather_at(tb, t, R, Z, phi, f);
-    rhs_eval(ep, sp, R, Z, u, w, mu, p, f, d);
+    FieldsG<double> fg;
+    fields_to_g(f, u, fg);
+    rhs_eval<double>(ep, sp, R, Z, u, w, mu, p, fg, d);
     return t < 0;
 }
 
@@ -292,7 +291,7 @@ __device__ __forceinline__ bool phase_step(const TorP& tor, double dt, Rec& r, E
 }
 
 // final store of one record: the record itself and (if enabled) the sort key of its next evaluation point
-__device__ __forceinline__ void store_rec(const DevTables& tb, const CellMap& cm, const KeyOut& ko, Rec* __restrict__ recs, long long ri,
+__device__ __forceinline__ void store_rec(const DevTables& tb, const CellMap& cm, const KeyOut& ko, Rec* recs, long long ri,
                                           Rec& r, int t, const double next[3]) {
     r.tri = t;
     rec_store(recs, ri, r);
@@ -309,13 +308,21 @@ __device__ __forceinline__ void store_rec(const DevTables& tb, const CellMap& cm
 // left their staged block, markers outside the mesh), the initial k1, and un-sorted operation
 template <int PHASE>
 __device__ __forceinline__ void phase_global(const DevTables& tb, const EquilP& ep, const SpeciesP& sp, const CellMap& cm, const KeyOut& ko,
-                                             const Rec* __restrict__ src, Rec* __restrict__ dst, long long ri, long long m, double dt) {
+                                             const Rec* src, Rec* dst, long long ri, long long m, double dt) {
     Rec r;
     rec_load(src, ri, r);
     int t = r.tri, st = r.st;
     const double mu = r.mu, p = r.p;
+    // status bit 0: some RK stage of a finished or running step was evaluated outside the mesh (sticky); bit 1: the cached
+    // k1 = f(y_n) was.  That evaluation is the first stage of the NEXT step, so it only counts once that step runs:
+    // phase A folds bit 1 into bit 0, markers_get reports bit 0 only (the oracle's and variant 1's rule).
+    if (PHASE == PHASE_A && (st & 2)) st = (st | 1) & ~2;
+    if (PHASE == PHASE_INIT) st &= ~2;
+    int ev = 0;
     auto eval = [&](const double y[5], double d[5]) {
-        st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, d);
+        const int out = stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, d);
+        st |= (PHASE == PHASE_A || (PHASE == PHASE_B && ev == 0)) ? out : 2 * out;
+        ++ev;
         return true;
     };
     double next[3];
@@ -327,8 +334,8 @@ __device__ __forceinline__ void phase_global(const DevTables& tb, const EquilP& 
 // positions m = index[i] (or i if index is null) of the cell order for i in [*first (or 0), *count (or n)):
 // record src[perm[m]] (or src[m] if perm is null) -> dst[m]
 template <int PHASE>
-__global__ void __launch_bounds__(128) k_phase_global(DevTables tb, EquilP ep, SpeciesP sp, CellMap cm, KeyOut ko, const Rec* __restrict__ src,
-                                                      Rec* __restrict__ dst, const int* __restrict__ perm, const int* __restrict__ index,
+__global__ void __launch_bounds__(128) k_phase_global(DevTables tb, EquilP ep, SpeciesP sp, CellMap cm, KeyOut ko, const Rec* src,
+                                                      Rec* dst, const int* __restrict__ perm, const int* __restrict__ index,
                                                       const int* __restrict__ first, const int* __restrict__ count, long long n, double dt) {
     const long long lo = first ? (long long)*first : 0, hi = count ? (long long)*count : n;
     for (long long i = lo + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < hi; i += (long long)gridDim.x * blockDim.x) {
@@ -346,12 +353,39 @@ __global__ void __launch_bounds__(256) k_locate_keys(DevTables tb, CellMap cm, K
     rec_load(recs, i, r);
     const int t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
     r.tri = t;
-    reinterpret_cast<double2*>(recs + i)[6 ^ (int)(i & 7)] = reinterpret_cast<const double2*>(&r)[6];   // (tri, st, id, pad0)
+    reinterpret_cast<double2*>(recs + i)[6 ^ rec_swizzle(i)] = reinterpret_cast<const double2*>(&r)[6];   // (tri, st, id, pad0)
     double sf;
     const int k = toroidal_interval(tb.tor, r.y[2], sf);
     const int key = t < 0 ? ko.ncell : cm.cell(t, k);
     ko.keys[i] = key;
     atomicAdd(ko.hist + key, 1);
+}
+
+// markers whose next evaluation point left the staged geometry of the phase kernel: their records are complete except for
+// the triangle of that point (the record holds a hint) and the sort key.  Next point: after phase A the stage-4 position held
+// in k, otherwise y + dt/2 k.
+template <int PHASE>
+__global__ void __launch_bounds__(128) k_fix_keys(DevTables tb, CellMap cm, KeyOut ko, Rec* recs, const int* __restrict__ list, const int* __restrict__ count,
+                                                  long long n, double dt) {
+    const int cnt = *count;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += gridDim.x * blockDim.x) {
+        const long long m = list[n - 1 - i];
+        Rec r;
+        rec_load(recs, m, r);
+        const double h2 = 0.5 * dt;
+        const double R = PHASE == PHASE_A ? r.k[0] : fma(h2, r.k[0], r.y[0]), Z = PHASE == PHASE_A ? r.k[1] : fma(h2, r.k[1], r.y[1]);
+        const double phi = PHASE == PHASE_A ? r.k[2] : fma(h2, r.k[2], r.y[2]);
+        const int t = locate_walk(tb.bg, tb.geom, r.tri, R, Z);
+        r.tri = t;
+        reinterpret_cast<double2*>(recs + m)[6 ^ rec_swizzle(m)] = reinterpret_cast<const double2*>(&r)[6];   // (tri, st, id, pad0)
+        if (ko.enabled) {
+            double sf;
+            const int k = toroidal_interval(tb.tor, phi, sf);
+            const int key = t < 0 ? ko.ncell : cm.cell(t, k);
+            ko.keys[m] = key;
+            atomicAdd(ko.hist + key, 1);
+        }
+    }
 }
 
 // variant 1: the whole classical RK4 step, one thread per marker, in place, coefficients through L1/L2 (reference for the
@@ -365,7 +399,7 @@ __global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, Sp
 #pragma unroll
     for (int q = 0; q < 5; ++q) y0[q] = r.y[q];
     const double mu = r.mu, p = r.p;
-    int t = r.tri, st = r.st;
+    int t = r.tri, st = r.st & ~2;   // variant 1 keeps no cached k1
     st |= stage_simple(tb, ep, sp, t, y0[0], y0[1], y0[2], y0[3], y0[4], mu, p, k);
 #pragma unroll
     for (int q = 0; q < 5; ++q) { acc[q] = k[q]; y[q] = fma(0.5 * dt, k[q], y0[q]); }
@@ -399,34 +433,13 @@ __global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP s
 
 // ============================================================================================ phase kernel: helpers
 // markers that left their staged block during a phase: positions in the cell order, finished by k_phase_global
+// and markers whose NEXT evaluation point left the staged geometry (record done, triangle and sort key still to be found by
+// k_fix_keys): the same array, filled from its end
 struct RetireList {
     int* list;      // [n]
-    int* count;     // device counter
+    int* count;     // device counters: [0] retired, [1] keys to fix
+    int n;
 };
-
-// slot-space edge walk inside the staged block: returns the slot containing (R, Z) or a negative code: -1 left the staged
-// set (or hop cap), -2 crossed the mesh boundary.  `last` = the last staged slot visited.
-__device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int sl, double R, double Z, double& xi, double& eta, int& last) {
-    if (sl < 0) return -1;
-    for (int hop = 0; hop < 16; ++hop) {
-        const SlotGeom& g = sgeom[sl];
-        last = sl;
-        double dx = R - g.v0x, dy = Z - g.v0y;
-        xi = fma(g.a11, dx, g.a12 * dy);
-        eta = fma(g.a21, dx, g.a22 * dy);
-        double l0 = 1.0 - xi - eta;
-        // three compares chained on a predicate instead of two fmin (no DMNMX on sm_100: each fmin is a compare + 4 selects)
-        if (xi >= INSIDE_TOL && eta >= INSIDE_TOL && l0 >= INSIDE_TOL) return sl;
-        const int e = (eta <= xi && eta <= l0) ? 0 : ((l0 <= xi) ? 1 : 2);
-        sl = g.nbr[e];
-        if (sl < 0) return sl;
-    }
-    return -1;
-}
-__device__ __forceinline__ int slot_walk(const SlotGeom* __restrict__ sgeom, int sl, double R, double Z, double& xi, double& eta) {
-    int last;
-    return slot_walk(sgeom, sl, R, Z, xi, eta, last);
-}
 
 }  // namespace trimeg
 #include "trimeg_ws.cuh"
@@ -502,14 +515,7 @@ __global__ void __launch_bounds__(256) k_sort_perm(long long n, const int* __res
     perm[pos] = (int)m;
 }
 // per phase: acc[0] += markers left to the follow-up kernel
-__global__ void k_accumulate_stat(const int* __restrict__ v, unsigned long long* __restrict__ acc) {
-    atomicAdd(acc, (unsigned long long)*v);
-#ifdef TRIMEG_WAITSTATS
-    atomicAdd(acc + 1, (unsigned long long)v[1]);   // compute warps waiting for a chunk (kilo-cycles, summed over warps)
-    atomicAdd(acc + 2, (unsigned long long)v[2]);   // stager waiting for a free ring entry
-    atomicAdd(acc - 1, (unsigned long long)v[3]);   // publishers waiting (block landed, slot free)
-#endif
-}
+__global__ void k_accumulate_stat(const int* __restrict__ v, unsigned long long* __restrict__ acc) { atomicAdd(acc, (unsigned long long)*v); }
 
 // ============================================================================================ DFMA micro-benchmark
 __global__ void __launch_bounds__(512) k_dfma(double* out, int iters, double a, double b) {

@@ -2,8 +2,12 @@
 // analytic equilibrium, guiding-centre and weight right-hand sides.  fp64 throughout.
 // Passages: /root/reference/PAPER.md L35 (C1 element x cubic B-spline), Eq.(2)-(6) L45-55, B*_par L61,
 // Eq.(7), Eq.(8) L314.  Formulation notes (what differs from a literal transcription) are in DESIGN.md
-// "Kernel arithmetic": reciprocals are shared, sqrt/div go through rsqrt/rcp + FMA, curl b comes from the
-// identity curl b = (curl B + b x grad B)/B, everything else is written in FMA form.
+// section 6 "Kernel arithmetic".
+//
+// Every routine is a template over the scalar type T: `double` (one marker per thread: gather, rhs, follow-up and
+// simple-push kernels) or `D2` (two markers per lane, the phase kernel: the two markers of a lane sit in the same
+// cell, so one shared-memory coefficient load feeds both Horner chains and the FP64 pipe sees two independent
+// dependency chains per warp).
 #pragma once
 #include <cstdint>
 
@@ -11,24 +15,41 @@ namespace trimeg {
 
 constexpr int NCOEF = 21;                 // quintic monomials xi^i eta^j, i + j <= 5
 constexpr int PLANE_STRIDE = NCOEF * 2;   // doubles per (triangle, plane): [21][field]
-constexpr int PLANE_PAD = 1;              // extra toroidal planes on each side of the padded coefficient table
-// padded table: plane index pp in [0, P + 3 + 2 PLANE_PAD) holds toroidal plane (pp - 1 - PLANE_PAD) mod P, so the four planes
-// k-1..k+2 of interval k are pp = k + PLANE_PAD .. k + PLANE_PAD + 3, contiguous for every k (no wrap in the kernels)
+constexpr int PLANE_PAD = 1;              // extra toroidal planes in front of the padded coefficient table
+// padded table: plane index pp in [0, NPP) holds toroidal plane (pp - 1 - PLANE_PAD) mod P, so the four planes
+// k-1..k+2 of interval k are pp = k + PLANE_PAD .. k + PLANE_PAD + 3, contiguous for every k (no wrap in the kernels);
+// NPP = (number of 4-interval windows) * 4 + 3 + 2 PLANE_PAD (see trimeg_mesh_load)
 constexpr double INSIDE_TOL = -1e-12;
 
+#define TRIMEG_DI __device__ __forceinline__
+
+// ---- two markers per lane ---------------------------------------------------------------------------
+struct D2 {
+    double a, b;
+    TRIMEG_DI D2() {}
+    TRIMEG_DI D2(double x) : a(x), b(x) {}
+    TRIMEG_DI D2(double x, double y) : a(x), b(y) {}
+};
+TRIMEG_DI D2 operator+(D2 x, D2 y) { return D2(x.a + y.a, x.b + y.b); }
+TRIMEG_DI D2 operator-(D2 x, D2 y) { return D2(x.a - y.a, x.b - y.b); }
+TRIMEG_DI D2 operator*(D2 x, D2 y) { return D2(x.a * y.a, x.b * y.b); }
+TRIMEG_DI D2 operator-(D2 x) { return D2(-x.a, -x.b); }
+TRIMEG_DI D2 fma(D2 x, D2 y, D2 z) { return D2(::fma(x.a, y.a, z.a), ::fma(x.b, y.b, z.b)); }
+using ::fma;
+
 struct EquilP {
-    double R0, B0, F, inv_a, inv_R0sq, q0, q1, q2;
+    double R0, B0, F, F2, inv_a, inv_R0sq, q0, q1, q2;   // F = B0 R0, F2 = F^2
     int qbar_sqrt;
 };
 struct SpeciesP {
     double qom, kappa;                 // q/m and m/q
     double kn_R0, kT_R0;               // kappa_n / R0, kappa_T / R0   (d ln H/dr = -(kappa_H/R0) sech^2)
-    double inv_wn_a, inv_wT_a, r0;     // 1/(w_n a), 1/(w_T a)
-    double cT;                         // kappa_T w_T a / R0 : T = exp(-cT tanh)
+    double two_inv_wn_a, two_inv_wT_a, r0;     // 2/(w_n a), 2/(w_T a): tanh x = 1 - 2/(exp(2x) + 1)
+    double cT;                         // kappa_T w_T a / R0 : 1/T = exp(cT tanh)
     int same_w, bstar_exact, weight_mode;
 };
 struct TorP {
-    double period, inv_period, inv_dphi, half_inv_dphi;   // 1/dphi, 1/(2 dphi)
+    double period, inv_period, inv_dphi, half_inv_dphi, m2_inv_dphi;   // 1/dphi, 1/(2 dphi), -2/dphi
     int P;
 };
 // per-triangle geometry, 64 B: reference coordinates xi = a11 (R - v0x) + a12 (Z - v0y), eta = a21 (..) + a22 (..)
@@ -46,53 +67,48 @@ struct BoxGrid {
 
 struct Fields { double P, PR, PZ, Pp, A, AR, AZ, Ap; };   // values, d/dR, d/dZ, raw d/dphi
 
-// 1/x and 1/sqrt(x) for normal positive-or-negative x (R, q, B, B*_par, r^2 ...): hardware seed (MUFU, ~2^-20) and two
-// Newton steps in FMA form, without the denormal / infinity side path of the library routines (a branch and a call each).
-__device__ __forceinline__ double rcp_nr(double x) {
+// ---- reciprocal, reciprocal square root, exp ---------------------------------------------------------
+// 1/x and 1/sqrt(x) for normal x (R, q, B, B*_par, r^2 ...): hardware seed (MUFU on the upper 32 bits of x: relative
+// error e ~ 2^-20) and ONE third-order correction in FMA form, without the denormal / infinity side path of the library
+// routines:  1/x = y0 / (1 - e) = y0 (1 + e + e^2 + O(e^3)),  x^-1/2 = y0 (1 - e)^-1/2 = y0 (1 + e/2 + 3 e^2/8 + O(e^3)),
+// truncation <= e^3 ~ 1e-18 relative, below the rounding of the final FMA.
+TRIMEG_DI double rcp_nr(double x) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double e = fma(-x, y, 1.0);
-    y = fma(y, e, y);
-    e = fma(-x, y, 1.0);
-    return fma(y, e, y);
+    const double e = fma(-x, y, 1.0);
+    return fma(y, fma(e, e, e), y);
 }
-__device__ __forceinline__ double rsqrt_nr(double x) {
+TRIMEG_DI double rsqrt_nr(double x) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double hx = 0.5 * x;
-    double e = fma(-hx * y, y, 0.5);      // (1 - x y^2) / 2
-    y = fma(y, e, y);
-    e = fma(-hx * y, y, 0.5);
-    return fma(y, e, y);
+    const double e = fma(-x * y, y, 1.0);
+    return fma(y * e, fma(e, 0.375, 0.5), y);
 }
-
-// exp and tanh for the profile terms of Eq.(7)/(8) (arguments of order one).  exp: x = n ln2 + r, |r| <= ln2/2, Taylor
-// polynomial of degree 13 in r (truncation 0.347^14/14! = 4e-18), 2^n through the exponent field; the coefficients sit in
-// constant memory so that every DFMA takes its constant as an operand (the library routines materialise theirs with two
-// UMOV each: 110 of the phase kernel's 2 970 instructions per chunk).  tanh x = 1 - 2/(e^{2x} + 1): absolute error ~1e-16,
-// which is what sech^2 = 1 - tanh^2 and T = exp(-c tanh) need.
+// exp for the profile terms of Eq.(7)/(8): x = n ln2 + r, |r| <= ln2/2, Taylor polynomial of degree 13 in r (truncation
+// 0.347^14/14! = 4e-18), times 2^n built in the exponent field (n clamped to +-1000 so that huge arguments saturate to
+// inf / ~0 through an ordinary multiplication instead of wrapping the exponent).  The coefficients sit in constant memory
+// so that every DFMA takes its constant as an operand.
 __constant__ double c_expk[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320, 1.0 / 362880,
                                   1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0};
 __constant__ double c_expr[4] = {1.4426950408889634, 6755399441055744.0, 6.93147180369123816490e-01, 1.90821492927058770002e-10};
-__device__ __forceinline__ double exp_nr(double x) {
+TRIMEG_DI double exp_nr(double x) {
     const double t = fma(x, c_expr[0], c_expr[1]);     // round(x / ln2) in the low mantissa bits
-    const int n = __double2loint(t);
-    const double fn = t - c_expr[1];
+    const int n = max(-1000, min(1000, __double2loint(t)));
+    const double fn = (double)n;
     double r = fma(-fn, c_expr[2], x);
     r = fma(-fn, c_expr[3], r);
     double p = c_expk[13];
 #pragma unroll
     for (int k = 12; k >= 0; --k) p = fma(p, r, c_expk[k]);
-    return __hiloint2double(__double2hiint(p) + n * 1048576, __double2loint(p));
+    return p * __hiloint2double((n + 1023) << 20, 0);
 }
-__device__ __forceinline__ double tanh_nr(double x) {
-    const double E = exp_nr(x + x);
-    return fma(-2.0, rcp_nr(E + 1.0), 1.0);
-}
+TRIMEG_DI D2 rcp_nr(D2 x) { return D2(rcp_nr(x.a), rcp_nr(x.b)); }
+TRIMEG_DI D2 rsqrt_nr(D2 x) { return D2(rsqrt_nr(x.a), rsqrt_nr(x.b)); }
+TRIMEG_DI D2 exp_nr(D2 x) { return D2(exp_nr(x.a), exp_nr(x.b)); }
 
 // ---- toroidal uniform periodic cubic B-spline (L35) -------------------------------------------------
 // interval index k in [0, P) and fraction s in [0, 1] of phi (any real)
-__device__ __forceinline__ int toroidal_interval(const TorP& tp, double phi, double& s) {
+TRIMEG_DI int toroidal_interval(const TorP& tp, double phi, double& s) {
     double pm = fma(-tp.period, floor(phi * tp.inv_period), phi);
     if (pm < 0.0) pm += tp.period;
     if (pm >= tp.period) pm -= tp.period;
@@ -102,54 +118,58 @@ __device__ __forceinline__ int toroidal_interval(const TorP& tp, double phi, dou
     s = u - (double)k;
     return k;
 }
-__device__ __forceinline__ void bspline_from_s(const TorP& tp, double s, double w[4], double dw[4]) {
-    double t = 1.0 - s;
-    const double sixth = 1.0 / 6.0;
-    double s2 = s * s, t2 = t * t;
-    w[0] = t2 * t * sixth;
-    w[3] = s2 * s * sixth;
-    w[1] = fma(s2, fma(3.0, s, -6.0), 4.0) * sixth;
-    w[2] = fma(t2, fma(3.0, t, -6.0), 4.0) * sixth;
-    dw[0] = -t2 * tp.half_inv_dphi;
-    dw[3] = s2 * tp.half_inv_dphi;
-    dw[1] = s * fma(3.0, s, -4.0) * tp.half_inv_dphi;
-    dw[2] = -t * fma(3.0, t, -4.0) * tp.half_inv_dphi;
+// w = [(1-s)^3, 3 s^3 - 6 s^2 + 4, 3 t^3 - 6 t^2 + 4, s^3] / 6 with t = 1 - s;  dw = d w / d phi
+template <class T>
+TRIMEG_DI void bspline_from_s(const TorP& tp, T s, T w[4], T dw[4]) {
+    const T t = T(1.0) - s;
+    const T s2 = s * s, t2 = t * t;
+    const T s2h = s2 * T(tp.half_inv_dphi), t2h = t2 * T(tp.half_inv_dphi);
+    w[0] = t2 * t * T(1.0 / 6.0);
+    w[3] = s2 * s * T(1.0 / 6.0);
+    w[1] = fma(s2, fma(T(0.5), s, T(-1.0)), T(2.0 / 3.0));
+    w[2] = fma(t2, fma(T(0.5), t, T(-1.0)), T(2.0 / 3.0));
+    dw[0] = -t2h;
+    dw[3] = s2h;
+    dw[1] = fma(T(3.0), s2h, T(tp.m2_inv_dphi) * s);
+    dw[2] = -fma(T(3.0), t2h, T(tp.m2_inv_dphi) * t);
 }
 // returns the interval k; the four planes are padded-table planes k + PLANE_PAD .. k + PLANE_PAD + 3
-__device__ __forceinline__ int bspline_weights(const TorP& tp, double phi, double w[4], double dw[4]) {
+TRIMEG_DI int bspline_weights(const TorP& tp, double phi, double w[4], double dw[4]) {
     double s;
     int k = toroidal_interval(tp, phi, s);
-    bspline_from_s(tp, s, w, dw);
+    bspline_from_s<double>(tp, s, w, dw);
     return k;
 }
 
 // ---- reduced quintic in reference coordinates --------------------------------------------------------
 // Coefficients j-major: a_j(xi) = sum_{i<=5-j} c[off_j + i] xi^i, p = sum_j eta^j a_j(xi).
 // Two fields interleaved: c[2*idx + f].  38 FMA per field: value, d/dxi, d/deta.
-template <int N, typename Ld>
-__device__ __forceinline__ void horner2(Ld ld, int off, double x, double& v0, double& d0, double& v1, double& d1) {
-    // both fields in lock-step; ld(idx, a, b) fetches coefficient idx of field 0 and 1
+// ld(idx, c0, c1) fetches coefficient idx of field 0 and 1 as doubles; the Horner state is T, so with T = D2 one fetch
+// serves both markers of the lane.
+template <int N, class T, class Ld>
+TRIMEG_DI void horner2(Ld ld, int off, T x, T& v0, T& d0, T& v1, T& d1) {
     double c0, c1;
     ld(off + N, c0, c1);
-    if (N == 0) { v0 = c0; v1 = c1; d0 = 0.0; d1 = 0.0; return; }
+    if (N == 0) { v0 = T(c0); v1 = T(c1); d0 = T(0.0); d1 = T(0.0); return; }
     double e0, e1;
     ld(off + N - 1, e0, e1);
-    v0 = fma(c0, x, e0); v1 = fma(c1, x, e1);
-    d0 = c0; d1 = c1;
+    v0 = fma(T(c0), x, T(e0)); v1 = fma(T(c1), x, T(e1));
+    d0 = T(c0); d1 = T(c1);
 #pragma unroll
     for (int i = N - 2; i >= 0; --i) {
         ld(off + i, e0, e1);
         d0 = fma(d0, x, v0); d1 = fma(d1, x, v1);
-        v0 = fma(v0, x, e0); v1 = fma(v1, x, e1);
+        v0 = fma(v0, x, T(e0)); v1 = fma(v1, x, T(e1));
     }
 }
 
-// acc[0..3] += (w p, w p_xi, w p_eta, dw p) for field 0, acc[4..7] likewise for field 1.
+// One plane: acc[0..3] += (w p, w p_xi, w p_eta, dw p) for field 0, acc[4..7] likewise for field 1; the value of field 0
+// (acc[0]) only if WITH_P (the right-hand sides never use Phi itself, only its gradient).
 // Outer Horner in eta runs j = 5 -> 0 and consumes each a_j(xi), a_j'(xi) as soon as the inner Horner produced it,
 // so only the three running sums per field stay live.
-template <typename Ld>
-__device__ __forceinline__ void quintic_pair_accum(Ld ld, double xi, double eta, double w, double dw, double acc[8]) {
-    double p0, p1, py0, py1, px0, px1, a0, a1, b0, b1;
+template <bool WITH_P, class T, class Ld>
+TRIMEG_DI void quintic_pair_accum(Ld ld, T xi, T eta, T w, T dw, T acc[8]) {
+    T p0, p1, py0, py1, px0, px1, a0, a1, b0, b1;
     horner2<0>(ld, 20, xi, p0, b0, p1, b1);          // a_5 (constant)
     horner2<1>(ld, 18, xi, a0, px0, a1, px1);        // a_4, a_4'
     py0 = p0; py1 = p1;
@@ -162,84 +182,69 @@ __device__ __forceinline__ void quintic_pair_accum(Ld ld, double xi, double eta,
     py0 = fma(py0, eta, p0); py1 = fma(py1, eta, p1); p0 = fma(p0, eta, a0); p1 = fma(p1, eta, a1); px0 = fma(px0, eta, b0); px1 = fma(px1, eta, b1);
     horner2<5>(ld, 0, xi, a0, b0, a1, b1);
     py0 = fma(py0, eta, p0); py1 = fma(py1, eta, p1); p0 = fma(p0, eta, a0); p1 = fma(p1, eta, a1); px0 = fma(px0, eta, b0); px1 = fma(px1, eta, b1);
-    acc[0] = fma(w, p0, acc[0]); acc[1] = fma(w, px0, acc[1]); acc[2] = fma(w, py0, acc[2]); acc[3] = fma(dw, p0, acc[3]);
+    if (WITH_P) acc[0] = fma(w, p0, acc[0]);
+    acc[1] = fma(w, px0, acc[1]); acc[2] = fma(w, py0, acc[2]); acc[3] = fma(dw, p0, acc[3]);
     acc[4] = fma(w, p1, acc[4]); acc[5] = fma(w, px1, acc[5]); acc[6] = fma(w, py1, acc[6]); acc[7] = fma(dw, p1, acc[7]);
 }
 
-// two planes at once: four independent Horner chains (2 planes x 2 fields) for instruction-level parallelism
-template <int N, typename LdA, typename LdB>
-__device__ __forceinline__ void horner4(LdA lda, LdB ldb, int off, double x, double v[4], double d[4]) {
-    double c[4], e[4];
-    lda(off + N, c[0], c[1]); ldb(off + N, c[2], c[3]);
-    if (N == 0) {
-#pragma unroll
-        for (int q = 0; q < 4; ++q) { v[q] = c[q]; d[q] = 0.0; }
-        return;
-    }
-    lda(off + N - 1, e[0], e[1]); ldb(off + N - 1, e[2], e[3]);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) { v[q] = fma(c[q], x, e[q]); d[q] = c[q]; }
-#pragma unroll
-    for (int i = N - 2; i >= 0; --i) {
-        lda(off + i, e[0], e[1]); ldb(off + i, e[2], e[3]);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) { d[q] = fma(d[q], x, v[q]); v[q] = fma(v[q], x, e[q]); }
-    }
-}
-template <typename LdA, typename LdB>
-__device__ __forceinline__ void quintic_quad_accum(LdA lda, LdB ldb, double xi, double eta, double wa, double dwa, double wb, double dwb, double acc[8]) {
-    double p[4], py[4], px[4], a[4], b[4];
-    horner4<0>(lda, ldb, 20, xi, p, b);
-    horner4<1>(lda, ldb, 18, xi, a, px);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) { py[q] = p[q]; p[q] = fma(p[q], eta, a[q]); }
-    horner4<2>(lda, ldb, 15, xi, a, b);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) { py[q] = fma(py[q], eta, p[q]); p[q] = fma(p[q], eta, a[q]); px[q] = fma(px[q], eta, b[q]); }
-    horner4<3>(lda, ldb, 11, xi, a, b);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) { py[q] = fma(py[q], eta, p[q]); p[q] = fma(p[q], eta, a[q]); px[q] = fma(px[q], eta, b[q]); }
-    horner4<4>(lda, ldb, 6, xi, a, b);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) { py[q] = fma(py[q], eta, p[q]); p[q] = fma(p[q], eta, a[q]); px[q] = fma(px[q], eta, b[q]); }
-    horner4<5>(lda, ldb, 0, xi, a, b);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) { py[q] = fma(py[q], eta, p[q]); p[q] = fma(p[q], eta, a[q]); px[q] = fma(px[q], eta, b[q]); }
-    // q = 0,1: plane A fields 0,1 ; q = 2,3: plane B fields 0,1
-    acc[0] = fma(wa, p[0], acc[0]); acc[1] = fma(wa, px[0], acc[1]); acc[2] = fma(wa, py[0], acc[2]); acc[3] = fma(dwa, p[0], acc[3]);
-    acc[4] = fma(wa, p[1], acc[4]); acc[5] = fma(wa, px[1], acc[5]); acc[6] = fma(wa, py[1], acc[6]); acc[7] = fma(dwa, p[1], acc[7]);
-    acc[0] = fma(wb, p[2], acc[0]); acc[1] = fma(wb, px[2], acc[1]); acc[2] = fma(wb, py[2], acc[2]); acc[3] = fma(dwb, p[2], acc[3]);
-    acc[4] = fma(wb, p[3], acc[4]); acc[5] = fma(wb, px[3], acc[5]); acc[6] = fma(wb, py[3], acc[6]); acc[7] = fma(dwb, p[3], acc[7]);
-}
-
 // all four planes; ldp(idx, a, b) fetches pair idx of [4][21] (16-byte aligned pairs); result in reference-gradient form
-template <typename LdPlane>
-__device__ __forceinline__ void gather_cell(LdPlane ldp, double xi, double eta, const double w[4], const double dw[4], double acc[8]) {
+template <bool WITH_P, class T, class LdPlane>
+TRIMEG_DI void gather_cell(LdPlane ldp, T xi, T eta, const T w[4], const T dw[4], T acc[8]) {
 #pragma unroll
-    for (int q = 0; q < 8; ++q) acc[q] = 0.0;
-#ifdef TRIMEG_GATHER_PAIRWISE
-#pragma unroll
-    for (int j = 0; j < 4; j += 2) {
-        auto lda = [&](int idx, double& a, double& b) { ldp(j * NCOEF + idx, a, b); };
-        auto ldb = [&](int idx, double& a, double& b) { ldp((j + 1) * NCOEF + idx, a, b); };
-        quintic_quad_accum(lda, ldb, xi, eta, w[j], dw[j], w[j + 1], dw[j + 1], acc);
-    }
-#else
+    for (int q = 0; q < 8; ++q) acc[q] = T(0.0);
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         auto ld = [&](int idx, double& a, double& b) { ldp(j * NCOEF + idx, a, b); };
-        quintic_pair_accum(ld, xi, eta, w[j], dw[j], acc);
+        quintic_pair_accum<WITH_P>(ld, xi, eta, w[j], dw[j], acc);
     }
-#endif
 }
+// The same with the plane loop ROLLED (one copy of the 168-FMA plane body: the phase kernel's hot loop has to fit the
+// 32 KB instruction cache) and the B-spline weights formed inside the loop from their polynomials in s,
+//   w_j(s) = sum_i c_bw[j][i] s^i,   d w_j / d s = sum_i c_bd[j][i] s^i   (j = plane k-1+j of interval k, L35),
+// whose coefficients sit in constant memory and are indexed by the (warp-uniform) loop counter.  The phi-derivative sums
+// acc[3], acc[7] are scaled by 1/dphi at the end.  base = shared-space byte address of the cell's first plane.
+__constant__ double c_bw[4][4] = {{1.0 / 6, -0.5, 0.5, -1.0 / 6}, {2.0 / 3, 0.0, -1.0, 0.5}, {1.0 / 6, 0.5, 0.5, -0.5}, {0.0, 0.0, 0.0, 1.0 / 6}};
+__constant__ double c_bd[4][3] = {{-0.5, 1.0, -0.5}, {0.0, -2.0, 1.5}, {0.5, 1.0, -1.5}, {0.0, 0.0, 0.5}};
+template <bool WITH_P, class T, class LdBase>
+TRIMEG_DI void gather_cell_rolled(unsigned base, T xi, T eta, T s, double inv_dphi, T acc[8]) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) acc[q] = T(0.0);
+#pragma unroll 1
+    for (int j = 0; j < 4; ++j) {
+        const T w = fma(fma(fma(T(c_bw[j][3]), s, T(c_bw[j][2])), s, T(c_bw[j][1])), s, T(c_bw[j][0]));
+        const T dw = fma(fma(T(c_bd[j][2]), s, T(c_bd[j][1])), s, T(c_bd[j][0]));
+        LdBase ld{base + (unsigned)(j * PLANE_STRIDE * sizeof(double))};
+        quintic_pair_accum<WITH_P>(ld, xi, eta, w, dw, acc);
+    }
+    acc[3] = acc[3] * T(inv_dphi);
+    acc[7] = acc[7] * T(inv_dphi);
+}
+
 // reference gradient -> physical gradient (grad_phys = J^-T grad_ref)
-__device__ __forceinline__ void to_fields(const TriGeom& g, const double acc[8], Fields& f) {
+TRIMEG_DI void to_fields(const TriGeom& g, const double acc[8], Fields& f) {
     f.P = acc[0]; f.PR = fma(g.a11, acc[1], g.a21 * acc[2]); f.PZ = fma(g.a12, acc[1], g.a22 * acc[2]); f.Pp = acc[3];
     f.A = acc[4]; f.AR = fma(g.a11, acc[5], g.a21 * acc[6]); f.AZ = fma(g.a12, acc[5], g.a22 * acc[6]); f.Ap = acc[7];
 }
 
+// What the right-hand sides need of the perturbed fields: g = grad(Phi - u A) at fixed u, as (d_R, raw d_phi, d_Z), and A
+// itself.  From the gathered reference-frame sums acc[] (quintic_pair_accum) and the triangle's J^-1 = (a11 a12; a21 a22):
+// the combination with u is done on the two reference components before the 2x2 transform (7 FMA instead of 11).
+template <class T>
+struct FieldsG { T gR, gZ, gp, A; };
+template <class T>
+TRIMEG_DI void to_fields_g(T a11, T a12, T a21, T a22, const T acc[8], T u, FieldsG<T>& f) {
+    const T gx = fma(-u, acc[5], acc[1]), gy = fma(-u, acc[6], acc[2]);
+    f.gR = fma(a11, gx, a21 * gy);
+    f.gZ = fma(a12, gx, a22 * gy);
+    f.gp = fma(-u, acc[7], acc[3]);
+    f.A = acc[4];
+}
+TRIMEG_DI void fields_to_g(const Fields& f, double u, FieldsG<double>& g) {
+    g.gR = fma(-u, f.AR, f.PR); g.gZ = fma(-u, f.AZ, f.PZ); g.gp = fma(-u, f.Ap, f.Pp); g.A = f.A;
+}
+
 // ---- locate -------------------------------------------------------------------------------------------
-__device__ __forceinline__ void ref_coords(const TriGeom& g, double R, double Z, double& xi, double& eta) {
+TRIMEG_DI void ref_coords(const TriGeom& g, double R, double Z, double& xi, double& eta) {
     double dx = R - g.v0x, dy = Z - g.v0y;
     xi = fma(g.a11, dx, g.a12 * dy);
     eta = fma(g.a21, dx, g.a22 * dy);
@@ -287,93 +292,92 @@ __device__ inline int locate_walk(const BoxGrid& bg, const TriGeom* __restrict__
 }
 
 // ---- equilibrium (L89) + Eq.(2)-(7) ----------------------------------------------------------------------
+// Analytic concentric-circular tokamak, psi'(r) = B0 r / qbar(r) (trimeg.h).  With P = psi', H = sqrt(P^2 + F^2):
+//   B = H / R,  b = (-P s, F, P c) / H  in (R, phi, Z)  (c, s = cos, sin of the poloidal angle),
+//   grad B = (H' c / R - B / R, 0, H' s / R),  H' = P P' / H,
+//   curl B = J e_phi,  J = [P c / R - (P' + P / r)] / R,
+//   curl b = (curl B + b x grad B) / B  =>  b . curl b = b_phi J / B.
+// (The oracle differentiates the components of b directly; this route is independent of it.)
+template <class T>
 struct Equil {
-    double B, invB, bR, bp, bZ, gBR, gBZ, cbR, cbp, cbZ, r, cth, sth;
+    T B, iB, iR, bR, bp, bZ, gBR, gBZ, J, r, c, s;
 };
-__device__ __forceinline__ void equil_eval(const EquilP& e, double R, double Z, Equil& o) {
-    double x = R - e.R0;
-    double r2 = fma(x, x, Z * Z);
-    double inv_r = rsqrt_nr(r2), r = r2 * inv_r;
-    double xa = r * e.inv_a;
-    double q = fma(xa, fma(e.q2, xa, e.q1), e.q0);
-    double dq = fma(2.0 * e.q2, xa, e.q1) * e.inv_a;
-    double qb = q, dqb = dq;
-    if (e.qbar_sqrt) {
-        double s2 = fma(-r2, e.inv_R0sq, 1.0);
-        double inv_s = rsqrt_nr(s2), s = s2 * inv_s;
-        double ds = -r * e.inv_R0sq * inv_s;
-        qb = q * s;
-        dqb = fma(dq, s, q * ds);
+template <class T>
+TRIMEG_DI void equil_eval(const EquilP& e, T R, T Z, Equil<T>& o) {
+    const T x = R - T(e.R0);
+    const T r2 = fma(x, x, Z * Z);
+    const T ir = rsqrt_nr(r2), r = r2 * ir;
+    const T c = x * ir, s = Z * ir;
+    const T xa = r * T(e.inv_a);
+    const T q = fma(xa, fma(T(e.q2), xa, T(e.q1)), T(e.q0));
+    const T dq = fma(T(2.0 * e.q2), xa, T(e.q1)) * T(e.inv_a);
+    T qb = q, dqb = dq;
+    if (e.qbar_sqrt) {   // qbar = q sqrt(1 - r^2/R0^2)
+        const T s2 = fma(-r2, T(e.inv_R0sq), T(1.0));
+        const T is = rsqrt_nr(s2), sq = s2 * is;
+        qb = q * sq;
+        dqb = fma(dq, sq, -(q * r) * (T(e.inv_R0sq) * is));
     }
-    double inv_qb = rcp_nr(qb);
-    double p1 = e.B0 * r * inv_qb;                 // psi'
-    double p2 = fma(-p1, dqb, e.B0) * inv_qb;      // psi''
-    double c = x * inv_r, s_ = Z * inv_r;
-    double p1r = p1 * inv_r, D = p2 - p1r;
-    double pR = p1 * c, pZ = p1 * s_;
-    double pRR = fma(D * c, c, p1r), pRZ = D * c * s_, pZZ = fma(D * s_, s_, p1r);
-    double iR = rcp_nr(R);
-    double BR = -pZ * iR, BZ = pR * iR, Bp = e.F * iR;
-    double BR_R = -(pRZ + BR) * iR, BR_Z = -pZZ * iR;
-    double BZ_R = (pRR - BZ) * iR, BZ_Z = pRZ * iR;
-    double Bp_R = -Bp * iR;
-    double B2 = fma(BR, BR, fma(BZ, BZ, Bp * Bp));
-    double iB = rsqrt_nr(B2), B = B2 * iB;
-    double gR = fma(BR, BR_R, fma(BZ, BZ_R, Bp * Bp_R)) * iB;
-    double gZ = fma(BR, BR_Z, BZ * BZ_Z) * iB;
-    double bR = BR * iB, bZ = BZ * iB, bp = Bp * iB;
-    double cBp = BR_Z - BZ_R;
-    o.B = B; o.invB = iB; o.bR = bR; o.bp = bp; o.bZ = bZ; o.gBR = gR; o.gBZ = gZ;
-    o.cbR = bp * gZ * iB;
-    o.cbp = (cBp + fma(bZ, gR, -bR * gZ)) * iB;
-    o.cbZ = -bp * gR * iB;
-    o.r = r; o.cth = c; o.sth = s_;
+    const T iqb = rcp_nr(qb);
+    const T P = T(e.B0) * r * iqb;                   // psi'
+    const T P1 = fma(-P, dqb, T(e.B0)) * iqb;        // psi''
+    const T iH = rsqrt_nr(fma(P, P, T(e.F2)));
+    const T iR = rcp_nr(R);
+    const T H = fma(P, P, T(e.F2)) * iH;
+    const T B = H * iR;
+    const T bt = P * iH;                             // poloidal component of b
+    const T t = (P * P1) * (iH * iR);                // H' / R
+    o.B = B; o.iB = R * iH; o.iR = iR;
+    o.bR = -(bt * s); o.bZ = bt * c; o.bp = T(e.F) * iH;
+    o.gBR = fma(t, c, -(B * iR)); o.gBZ = t * s;
+    o.J = fma(P * c, iR, -fma(P, ir, P1)) * iR;
+    o.r = r; o.c = c; o.s = s;
 }
 
-// time derivatives of (R, Z, phi, u, w) at one phase-space point (gyro-average off, L320; dA^s = 0: p_par form)
-__device__ __forceinline__ void rhs_eval(const EquilP& ep, const SpeciesP& sp, double R, double Z, double u, double w,
-                                         double mu, double p, const Fields& f, double d[5]) {
-    Equil e;
+// time derivatives of (R, Z, phi, u, w) at one phase-space point (gyro-average off, L320; dA^s = 0: p_par form).
+//   B*_par = B + kappa u b.curl b  (L61),  S = beta b + kappa u curl b with beta = B (b* = B*/B*_par, reading R7) or
+//   beta = B*_par (the literal expression printed at L53), so that in both cases b* = S / B*_par and every product with
+//   b* is formed with S and scaled by 1/B*_par once at the end.
+template <class T>
+TRIMEG_DI void rhs_eval(const EquilP& ep, const SpeciesP& sp, T R, T Z, T u, T w, T mu, T p, const FieldsG<T>& f, T d[5]) {
+    Equil<T> e;
     equil_eval(ep, R, Z, e);
-    double iR = rcp_nr(R);
-    double ku = sp.kappa * u;
-    double Bss = fma(ku, fma(e.bR, e.cbR, fma(e.bp, e.cbp, e.bZ * e.cbZ)), e.B);   // L61
-    double iBss = rcp_nr(Bss);
-    double bsR, bsp, bsZ;
-    if (sp.bstar_exact) {
-        bsR = fma(ku, e.cbR, e.B * e.bR) * iBss; bsp = fma(ku, e.cbp, e.B * e.bp) * iBss; bsZ = fma(ku, e.cbZ, e.B * e.bZ) * iBss;
-    } else {
-        double k2 = ku * iBss;
-        bsR = fma(k2, e.cbR, e.bR); bsp = fma(k2, e.cbp, e.bp); bsZ = fma(k2, e.cbZ, e.bZ);
-    }
+    const T ku = T(sp.kappa) * u, km = T(sp.kappa) * mu;
+    const T kub = ku * e.iB;
+    const T Bss = fma(kub * e.bp, e.J, e.B);                                       // L61
+    const T iBss = rcp_nr(Bss);
+    const T beta = sp.bstar_exact ? e.B : Bss;
+    // B curl b = (b_phi gB_Z, J + b_Z gB_R - b_R gB_Z, -b_phi gB_R)
+    const T SR = fma(kub, e.bp * e.gBZ, beta * e.bR);
+    const T Sp = fma(kub, fma(e.bZ, e.gBR, fma(-e.bR, e.gBZ, e.J)), beta * e.bp);
+    const T SZ = fma(-kub, e.bp * e.gBR, beta * e.bZ);
     // g = grad(Phi - u A), grad = (d_R, (1/R) d_phi, d_Z)
-    double gR = fma(-u, f.AR, f.PR), gp = fma(-u, f.Ap, f.Pp) * iR, gZ = fma(-u, f.AZ, f.PZ);
-    double km = sp.kappa * mu;
-    double GR = fma(km, e.gBR, gR), Gp = gp, GZ = fma(km, e.gBZ, gZ);
+    const T gR = f.gR, gZ = f.gZ, gp = f.gp * e.iR;
+    const T GR = fma(km, e.gBR, gR), GZ = fma(km, e.gBZ, gZ);                      // G = kappa mu grad B + g
     // b x G, right-handed (R, phi, Z)
-    double cR = fma(e.bp, GZ, -e.bZ * Gp), cp = fma(e.bZ, GR, -e.bR * GZ), cZ = fma(e.bR, Gp, -e.bp * GR);
-    double vpar = fma(-sp.qom, f.A, u);
-    double XR = fma(vpar, bsR, cR * iBss), Xp = fma(vpar, bsp, cp * iBss), XZ = fma(vpar, bsZ, cZ * iBss);   // Eq.(2)+(4)
-    double bs_g = fma(bsR, gR, fma(bsp, gp, bsZ * gZ));
-    double bs_gB = fma(bsR, e.gBR, bsZ * e.gBZ);
-    d[0] = XR; d[1] = XZ; d[2] = Xp * iR;
-    d[3] = -fma(mu, bs_gB, sp.qom * bs_g);                                                                  // Eq.(3)+(5)
+    const T cR = fma(e.bp, GZ, -(e.bZ * gp)), cp = fma(e.bZ, GR, -(e.bR * GZ)), cZ = fma(e.bR, gp, -(e.bp * GR));
+    const T vpar = fma(T(-sp.qom), f.A, u);
+    d[0] = fma(vpar, SR, cR) * iBss;                                               // Eq.(2)+(4)
+    d[1] = fma(vpar, SZ, cZ) * iBss;
+    d[2] = fma(vpar, Sp, cp) * (iBss * e.iR);
+    const T qgR = T(sp.qom) * gR, qgp = T(sp.qom) * gp, qgZ = T(sp.qom) * gZ;
+    const T Sqg = fma(SR, qgR, fma(Sp, qgp, SZ * qgZ));                            // qom S.g
+    d[3] = -(fma(mu, fma(SR, e.gBR, SZ * e.gBZ), Sqg) * iBss);                     // Eq.(3)+(5)
     // Eq.(7): delta-parts of the motion against grad ln f0, f0 Maxwellian with Eq.(8) profiles
-    double hR = fma(e.bp, gZ, -e.bZ * gp), hZ = fma(e.bR, gp, -e.bp * gR);    // (b x g)_R, (b x g)_Z
-    double qA = sp.qom * f.A;
-    double dXR = fma(hR, iBss, -qA * bsR), dXZ = fma(hZ, iBss, -qA * bsZ);
-    double ddu = -sp.qom * bs_g;
-    double dr = e.r - sp.r0;
-    double thT = tanh_nr(dr * sp.inv_wT_a);
-    double thn = sp.same_w ? thT : tanh_nr(dr * sp.inv_wn_a);
-    double dlnT = -sp.kT_R0 * fma(-thT, thT, 1.0), dlnn = -sp.kn_R0 * fma(-thn, thn, 1.0);
-    double iT = exp_nr(sp.cT * thT);                          // 1/T(r), Eq.(8)
-    double En = fma(0.5 * u, u, mu * e.B);
-    double cr = fma(dlnT, fma(En, iT, -1.5), dlnn);
-    double muT = mu * iT;
-    double glR = fma(cr, e.cth, -muT * e.gBR), glZ = fma(cr, e.sth, -muT * e.gBZ);
-    double pw = sp.weight_mode ? (p - w) : p;
-    d[4] = -pw * fma(dXR, glR, fma(dXZ, glZ, -ddu * u * iT));
+    const T hR = fma(e.bp, gZ, -(e.bZ * gp)), hZ = fma(e.bR, gp, -(e.bp * gR));    // (b x g)_R, (b x g)_Z
+    const T qA = T(sp.qom) * f.A;
+    const T eR = fma(-qA, SR, hR), eZ = fma(-qA, SZ, hZ);                          // Bss * delta Xdot
+    const T dr = e.r - T(sp.r0);
+    const T thT = fma(T(-2.0), rcp_nr(exp_nr(dr * T(sp.two_inv_wT_a)) + T(1.0)), T(1.0));
+    const T thn = sp.same_w ? thT : fma(T(-2.0), rcp_nr(exp_nr(dr * T(sp.two_inv_wn_a)) + T(1.0)), T(1.0));
+    const T dlnT = T(-sp.kT_R0) * fma(-thT, thT, T(1.0)), dlnn = T(-sp.kn_R0) * fma(-thn, thn, T(1.0));
+    const T iT = exp_nr(T(sp.cT) * thT);                                           // 1/T(r), Eq.(8)
+    const T En = fma(T(0.5) * u, u, mu * e.B);
+    const T cr = fma(dlnT, fma(En, iT, T(-1.5)), dlnn);
+    const T muT = mu * iT;
+    const T glR = fma(cr, e.c, -(muT * e.gBR)), glZ = fma(cr, e.s, -(muT * e.gBZ));
+    const T pw = sp.weight_mode ? (p - w) : p;
+    d[4] = -((pw * iBss) * fma(eR, glR, fma(eZ, glZ, Sqg * (u * iT))));
 }
 
 }  // namespace trimeg

@@ -1,93 +1,132 @@
 // Shared-memory tiling of the phase kernel: layout constants, slot geometry and the PTX helpers
-// (mbarrier, TMA bulk copy, shared-memory vector access).
+// (mbarrier, TMA bulk copy, shared-memory vector access, register re-allocation).
 //
 // Why tiles: one field evaluation reads 8 x 21 coefficients = 1344 B per marker.  Through L1 with one address per lane
-// that is >= 336 L1 cycles per warp against 338 DFMA = 169 issue cycles of FP64 work (measured: the L1-path kernel is
-// 2x slower even when every lane of a warp sits in the same cell).  So the coefficient blocks of a patch of TP triangles
-// plus a halo (SMAX slots), for a window of WK toroidal intervals plus HK on either side, are staged per super-cell with
-// 1-D TMA bulk copies (cp.async.bulk + mbarrier), and markers are visited in cell order so that the lanes of a warp read
-// the same few blocks.  A marker whose evaluation point leaves the staged set RETIRES to a list that a follow-up kernel
-// finishes through the global tables, so that no warp waits on a divergent slow lane.
+// that is >= 336 L1 cycles per warp against 338 DFMA = 169 issue cycles of FP64 work.  So the coefficient blocks of a
+// patch of TP triangles plus a halo (SMAX slots), for a window of WK toroidal intervals plus HK on either side, are
+// staged per super-cell with 1-D TMA bulk copies (cp.async.bulk + mbarrier), and markers are visited in cell order, two
+// markers of the same cell per lane, so that one LDS.128 feeds two fields x two markers.  A marker whose evaluation point
+// leaves the staged set RETIRES to a list that a follow-up kernel finishes through the global tables, so that no warp
+// waits on a divergent slow lane.
 #pragma once
 #include "trimeg_math.cuh"
 
 namespace trimeg {
 
 struct TileTables {
-    const int* slots;        // [npatch][SMAX] global triangle per slot, -1 unused
-    const short* nbr;        // [npatch][SMAX][4] slot across edge e, -1 = not staged / boundary
+    const int* slots;        // [npatch][SGEOM] global triangle per slot, -1 unused
+    const short* nbr;        // [npatch][SGEOM][4] slot across edge e, -1 = not staged, -2 = mesh boundary
     const int* nslots;       // [npatch]
     const int* offs;         // [ncell + 1] exclusive offsets of the cell-sorted marker store
     int npatch, nwin, nsc;   // super-cells = npatch * nwin
 };
 
-template <int TP_, int SMAX_, int WK_, int NWARPS_, int NBUF_>
+template <int TP_, int SMAX_, int WK_, int NCOMP_, int NBUF_, int K_>
 struct TileCfg {
-    static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD, NWARPS = NWARPS_, NTHREADS = 32 * NWARPS_;
+    static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD;
+    static constexpr int NPROD = 4;                  // producer warp-group: stager, two publishers, one spare
+    static constexpr int NPUB = 2;                   // publisher warps (tickets of parity pid)
+    static constexpr int NLOC = 4;                   // locator warp-group (tickets t % NLOC)
+    static constexpr int NCOMP = NCOMP_;             // compute warps (two warp-groups)
+    static_assert(NCOMP == 8, "register hand-over below assumes 16 warps");
+    static constexpr int NWARPS = NPROD + NLOC + NCOMP, NTHREADS = 32 * NWARPS;
+    // register hand-over (setmaxnreg): 16 warps launch with 128 registers; the 8 light warps drop to 40, the 8 compute
+    // warps take the 8 x 88 freed ones: 216
+    static constexpr int REG_PROD = 40, REG_COMP = 216;
     static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
     static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
     static constexpr int CPS = TP * WK;              // cells per super-cell
+    static_assert(CPS == 32, "one lane per cell of a super-cell (pair layout of the publishers)");
     static constexpr int SLOT_DOUBLES = NPL * PLANE_STRIDE;
     static constexpr int NBUF = NBUF_;               // ring of staged blocks
-    // shared memory carve-up (bytes): NBUF x { coefficients, slot geometry }, then the control words
-    static constexpr size_t COEF_BYTES = sizeof(double) * SMAX * SLOT_DOUBLES;
+    static constexpr int K = K_;                     // chunk slots
+    static_assert(K % NPUB == 0, "a chunk slot is always served by the same publisher warp");
     // slot GEOMETRY (64 B per slot) is staged for SGEOM slots, coefficients only for the first SMAX of them: the walk that
     // locates the next phase's first evaluation point needs no coefficients and stays in shared memory further out
-#ifndef TRIMEG_SGEOM
-#define TRIMEG_SGEOM 32
-#endif
-    static constexpr int SGEOM = TRIMEG_SGEOM;
-    static constexpr size_t BLOCK_BYTES = COEF_BYTES + 64 * SGEOM;
+    static constexpr int SGEOM = 32;
+    static_assert(SMAX <= SGEOM, "one slot per lane of the stager");
+    // shared memory carve-up (bytes): NBUF x { coefficients, slot geometry }, control, chunk slots
+    static constexpr size_t COEF_BYTES = sizeof(double) * SMAX * SLOT_DOUBLES;
+    static constexpr size_t GEOM_BYTES = 96 * SGEOM;                          // SlotGeom per slot
+    static constexpr size_t BLOCK_BYTES = COEF_BYTES + GEOM_BYTES + 4 * SGEOM; // + triangle id per slot
+    static constexpr size_t CTRL_BYTES = 320;        // BlockCtrl per ring entry
     static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;
-    // chunk slots: 32 marker records of 128 B (XOR-swizzled rows), filled by cp.async; NWARPS slots
-    static constexpr size_t WSTAGE = 32 * 128;
-    static constexpr size_t OFF_STAGE = (OFF_CTRL + 64 * NBUF + 16 * NBUF + 127) / 128 * 128;
-    static constexpr size_t BYTES = OFF_STAGE + WSTAGE * NWARPS;
+    static constexpr size_t OFF_BAR = OFF_CTRL + CTRL_BYTES * NBUF;          // per ring entry: full, seen (8 B each)
+    static constexpr size_t OFF_DESC = OFF_BAR + 16 * NBUF;                  // per chunk slot: ChunkDesc (16 B)
+    static constexpr size_t OFF_LTAB = OFF_DESC + 16 * K;                    // per chunk slot: 32 lane bytes
+    static constexpr size_t OFF_LFLAG = OFF_LTAB + 32 * K;                   // per chunk slot: 32 lane bytes written by the compute warp
+    static constexpr size_t OFF_CBAR = OFF_LFLAG + 32 * K;                   // per chunk slot: full, computed, empty (8 B each)
+    static constexpr size_t OFF_HEAD = OFF_CBAR + 24 * K;                    // ticket counter
+    static constexpr int CHUNK = 64;                                         // marker records per chunk slot (two per lane)
+    static constexpr size_t WSTAGE = CHUNK * 128;
+    static constexpr size_t OFF_STAGE = (OFF_HEAD + 16 + 127) / 128 * 128;
+    static constexpr size_t BYTES = OFF_STAGE + WSTAGE * K;
+    static_assert(BYTES <= 227 * 1024, "shared memory per CTA");
 };
-struct BlockCtrl {   // 64 B per ring entry; left = chunks done, pad[0] = chunks cut from the entry
-    int sc, begin, end, next, left, ns, patch, k0;
-    int pad[8];
+// one ring entry = one super-cell.  Cells of the super-cell are numbered 0..31 (triangle-in-patch major, interval minor);
+// the markers of a cell are paired up (an odd cell leaves one half-empty pair) so that both markers of a lane share
+// their coefficient block.
+struct BlockCtrl {
+    int sc, patch, k0, ns;
+    int nchunks;           // chunks that will be cut from this entry
+    int done;              // chunks finished (compute warps count up)
+    int npairs, pad;
+    int cell_off[33];      // first marker position of each cell (cell order), [32] = end
+    int pair_incl[32];     // inclusive prefix sum of pairs per cell
 };
+static_assert(sizeof(BlockCtrl) <= 320, "BlockCtrl fits its slot");
+struct ChunkDesc { int m_first, nrec, b, pad; };   // m_first < 0: no more work
 
-struct __align__(16) SlotGeom {   // 64 B
-    double v0x, v0y, a11, a12, a21, a22;
-    short nbr[4];
-    int tri, pad;
+// Geometry of one staged slot, 96 B.  The edge walk tests the three barycentrics in the form l = a R + b Z + c (two
+// dependent FMAs each; their rounding, ~1e-13, only matters within the walk's 1e-12 tolerance band, where either
+// neighbour is a correct answer); the coordinates handed to the polynomial evaluation are recomputed once, for the
+// triangle found, in the cancellation-free form a (R - v0x) + b (Z - v0y).
+struct __align__(16) SlotGeom {
+    double a11, a12, a21, a22;    // J^-1: xi = a11 (R - v0x) + a12 (Z - v0y), eta = a21 (..) + a22 (..)
+    double c1, c2;                // xi = a11 R + a12 Z + c1, eta = a21 R + a22 Z + c2
+    double l0a, l0b, l0c;         // 1 - xi - eta = l0a R + l0b Z + l0c
+    short nbr[4];                 // slot across edge 0 (eta = 0), 1 (1 - xi - eta = 0), 2 (xi = 0): -1 not staged, -2 mesh boundary
+    double v0x, v0y;
 };
+static_assert(sizeof(SlotGeom) == 96, "SlotGeom");
 
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(void* bar, int count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count)); }
-__device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes) {
+TRIMEG_DI unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+TRIMEG_DI void mbar_init(void* bar, int count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count)); }
+TRIMEG_DI void mbar_expect_tx(void* bar, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
+TRIMEG_DI void mbar_arrive(void* bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory"); }
+TRIMEG_DI void mbar_wait(void* bar, unsigned parity) {
     asm volatile(
         "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n" ::"r"(smem_u32(bar)),
         "r"(parity)
         : "memory");
 }
-__device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, unsigned bytes, void* bar) {
+TRIMEG_DI void tma_bulk_g2s(void* dst, const void* src, unsigned bytes, void* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src), "r"(bytes),
                  "r"(smem_u32(bar))
                  : "memory");
 }
 // shared -> global bulk copy (bytes: multiple of 16); completion is tracked by the issuing thread's bulk async-group
-__device__ __forceinline__ void tma_bulk_s2g(void* dst, const void* src, unsigned bytes) {
+TRIMEG_DI void tma_bulk_s2g(void* dst, const void* src, unsigned bytes) {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void sts128(unsigned addr, double a, double b) {
+TRIMEG_DI void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+TRIMEG_DI void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+TRIMEG_DI void sts128(unsigned addr, double a, double b) {
     asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(a), "d"(b) : "memory");
 }
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void lds128(unsigned addr, double& a, double& b) {
+TRIMEG_DI void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+TRIMEG_DI void lds128(unsigned addr, double& a, double& b) {
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "r"(addr));
 }
+// warp-group register re-allocation (sm_90a+): the producer group gives registers up, the compute groups take them
+template <int N> TRIMEG_DI void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> TRIMEG_DI void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 
 struct LdShared {   // coefficient pair fetch from the staged block
     unsigned base;  // shared-space byte address of the cell's first plane
-    __device__ __forceinline__ void operator()(int idx, double& a, double& b) const {
+    TRIMEG_DI void operator()(int idx, double& a, double& b) const {
         asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "r"(base + 16u * (unsigned)idx));
     }
 };
