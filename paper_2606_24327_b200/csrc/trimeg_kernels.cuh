@@ -36,19 +36,19 @@ struct DevTables {
 };
 
 // tiled push configuration: patches of 8 triangles + halo (SMAX slots with coefficients, 32 with geometry), windows of 4
-// toroidal intervals (+1 each side), ring of NBUF staged blocks, K chunk slots of 64 records, 4 producer + 4 locator + 8
+// toroidal intervals (+1 each side), ring of NBUF staged blocks, K chunk slots of 64 records, 4 light (stager, publisher, 2 locators) + 12
 // compute warps per CTA, one CTA per SM.  (TRIMEG_* macros: tuning sweeps only; the shipped build uses the defaults.)
 #ifndef TRIMEG_SMAX
-#define TRIMEG_SMAX 13
+#define TRIMEG_SMAX 12
 #endif
 #ifndef TRIMEG_NBUF
 #define TRIMEG_NBUF 2
 #endif
 #ifndef TRIMEG_NSLOTS
-#define TRIMEG_NSLOTS 16
+#define TRIMEG_NSLOTS 18
 #endif
 #ifndef TRIMEG_NCOMP
-#define TRIMEG_NCOMP 8
+#define TRIMEG_NCOMP 12
 #endif
 using Tile = TileCfg<8, TRIMEG_SMAX, 4, TRIMEG_NCOMP, TRIMEG_NBUF, TRIMEG_NSLOTS>;
 // cell numbering used by the sort: super-cell (patch, window) major, then triangle within the patch, then interval

@@ -24,15 +24,14 @@ struct TileTables {
 template <int TP_, int SMAX_, int WK_, int NCOMP_, int NBUF_, int K_>
 struct TileCfg {
     static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD;
-    static constexpr int NPROD = 4;                  // producer warp-group: stager, two publishers, one spare
-    static constexpr int NPUB = 2;                   // publisher warps (tickets of parity pid)
-    static constexpr int NLOC = 4;                   // locator warp-group (tickets t % NLOC)
-    static constexpr int NCOMP = NCOMP_;             // compute warps (two warp-groups)
-    static_assert(NCOMP == 8, "register hand-over below assumes 16 warps");
-    static constexpr int NWARPS = NPROD + NLOC + NCOMP, NTHREADS = 32 * NWARPS;
-    // register hand-over (setmaxnreg): 16 warps launch with 128 registers; the 8 light warps drop to 40, the 8 compute
-    // warps take the 8 x 88 freed ones: 216
-    static constexpr int REG_PROD = 40, REG_COMP = 216;
+    // one light warp-group: stager, publisher, two locators; three compute warp-groups
+    static constexpr int NLIGHT = 4, NLOC = 2;
+    static constexpr int NCOMP = NCOMP_;
+    static_assert(NCOMP == 12, "register hand-over below assumes 16 warps");
+    static constexpr int NWARPS = NLIGHT + NCOMP, NTHREADS = 32 * NWARPS;
+    // register hand-over (setmaxnreg): 16 warps launch with 128 registers; the light warps drop to 40, the compute warps
+    // take 24 more each (12 x 24 <= 4 x 88)
+    static constexpr int REG_LIGHT = 40, REG_COMP = 152;
     static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
     static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
     static constexpr int CPS = TP * WK;              // cells per super-cell
@@ -40,7 +39,6 @@ struct TileCfg {
     static constexpr int SLOT_DOUBLES = NPL * PLANE_STRIDE;
     static constexpr int NBUF = NBUF_;               // ring of staged blocks
     static constexpr int K = K_;                     // chunk slots
-    static_assert(K % NPUB == 0, "a chunk slot is always served by the same publisher warp");
     // slot GEOMETRY (64 B per slot) is staged for SGEOM slots, coefficients only for the first SMAX of them: the walk that
     // locates the next phase's first evaluation point needs no coefficients and stays in shared memory further out
     static constexpr int SGEOM = 32;

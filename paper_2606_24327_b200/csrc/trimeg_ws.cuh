@@ -161,15 +161,15 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
     constexpr unsigned FULL = 0xffffffffu;
     auto ctl_of = [&](int b) { return reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL + C::CTRL_BYTES * b); };
     if (tid == 0) {
-        for (int b = 0; b < C::NBUF; ++b) { mbar_init(blk_bar + 2 * b, 1); mbar_init(blk_bar + 2 * b + 1, C::NPUB); }
+        for (int b = 0; b < C::NBUF; ++b) { mbar_init(blk_bar + 2 * b, 1); mbar_init(blk_bar + 2 * b + 1, 1); }
         for (int s = 0; s < C::K; ++s) { mbar_init(chunk_bar + 3 * s, 32); mbar_init(chunk_bar + 3 * s + 1, 1); mbar_init(chunk_bar + 3 * s + 2, 1); }
         *cons_head = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    if (wid < C::NPROD) {
-        reg_dealloc<C::REG_PROD>();
+    if (wid < C::NLIGHT) {
+        reg_dealloc<C::REG_LIGHT>();
         if (wid == 0) {
             // ------------------------------------------------------------------ stager
             StageWork w;
@@ -177,7 +177,7 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
             for (unsigned it = 0;; ++it) {
                 const int b = it % C::NBUF;
                 if (it >= (unsigned)C::NBUF) {
-                    // previous occupant: both publishers have read its control block, and all chunks cut from it are done
+                    // previous occupant: the publisher has read its control block, and all chunks cut from it have left
                     mbar_wait(blk_bar + 2 * b + 1, (it / C::NBUF - 1) & 1);
                     BlockCtrl* ctl = ctl_of(b);
                     if (lane == 0) {
@@ -197,17 +197,45 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                 ws_commit<C>(smem, b, tb, w, lane);
                 have = ws_fetch<C>(tb, tt, work_counter, lane, w);   // the next entry's global loads overlap the compute warps' work
             }
-        } else if (wid <= C::NPUB) {
-            // ------------------------------------------------------------------ publishers: warp pid takes the tickets t with t % NPUB == pid
-            const unsigned pid = wid - 1;
+        } else if (wid == 1) {
+            // ------------------------------------------------------------------ publisher: chunks in ticket order.  The layout and the
+            // permutation entries of chunk i + 1 are fetched before chunk i is copied in, so that their latency is hidden.
             unsigned ticket = 0;
             auto slot_acquire = [&](unsigned t) {   // wait until the previous user of the slot has been copied out
                 const unsigned s = t % C::K, g = t / C::K;
                 if (g >= 1) mbar_wait(chunk_bar + 3 * s + 2, (g - 1) & 1);
                 return (int)s;
             };
+            // a chunk whose layout is known and whose permutation entries are in flight
+            int p_have = 0, p_mfirst = 0, p_nrec = 0, p_b = 0, p_pr0 = 0, p_pr1 = 0;
+            unsigned char p_lt = 0;
+            unsigned p_t = 0;
+            auto emit = [&]() {
+                const int s = slot_acquire(p_t);
+                if (lane == 0) { desc[s].m_first = p_mfirst; desc[s].nrec = p_nrec; desc[s].b = p_b; }
+                ltab[s * 32 + lane] = p_lt;
+                __threadfence_block();
+                __syncwarp();
+                const unsigned ib = smem_u32(smem + C::OFF_STAGE + (size_t)s * C::WSTAGE);
+                const int ch = lane & 7, q = lane >> 3;
+#pragma unroll
+                for (int k = 0; k < 16; ++k) {
+                    const int r = 4 * k + q;                                   // row of the chunk slot = record m_first + r of dst
+                    const int ri = __shfl_sync(FULL, k < 8 ? p_pr0 : p_pr1, r & 31);
+                    if (r < p_nrec) {
+                        // logical 16-byte chunk j of a record sits at position j ^ rec_swizzle(index): source position ch
+                        const int j = ch ^ rec_swizzle(ri);
+                        const unsigned d = ib + r * 128 + 16 * (j ^ rec_swizzle(p_mfirst + r));
+                        const char* gp = reinterpret_cast<const char*>(src + ri) + 16 * ch;
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gp) : "memory");
+                    }
+                }
+                asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(chunk_bar + 3 * s)) : "memory");
+                p_have = 0;
+            };
             for (unsigned it = 0;; ++it) {
                 const int b = it % C::NBUF;
+                if (p_have) emit();   // never hold a chunk back while waiting for the next ring entry
                 mbar_wait(blk_bar + 2 * b, (it / C::NBUF) & 1);
                 const BlockCtrl* ctl = ctl_of(b);
                 const int sc = ctl->sc;
@@ -216,10 +244,9 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                 __syncwarp();
                 if (lane == 0) mbar_arrive(blk_bar + 2 * b + 1);   // control block read: the stager may refill once the chunks are done
                 if (sc < 0) break;
-                // the chunks of this entry carry tickets ticket .. ticket + nch - 1; ours are those of parity pid
                 const unsigned t0 = ticket, nch = (unsigned)(npairs + 31) >> 5;
                 ticket = t0 + nch;
-                for (unsigned t = t0 + (pid + C::NPUB - t0 % C::NPUB) % C::NPUB; t < t0 + nch; t += C::NPUB) {
+                for (unsigned t = t0; t < t0 + nch; ++t) {
                     // pair g of the entry -> cell (binary search in the inclusive prefix sums held one per lane) -> marker positions
                     const int g = 32 * (int)(t - t0) + lane;
                     const bool valid = g < npairs;
@@ -237,99 +264,80 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                     // source records of rows lane and lane + 32
                     int pr0 = m_first + lane, pr1 = m_first + 32 + lane;
                     if (perm) { if (lane < nrec) pr0 = perm[pr0]; if (lane + 32 < nrec) pr1 = perm[pr1]; }
-                    const int s = slot_acquire(t);
-                    if (lane == 0) { desc[s].m_first = m_first; desc[s].nrec = nrec; desc[s].b = b; }
-                    ltab[s * 32 + lane] = valid ? (unsigned char)(0x80 | (hasB << 6) | (mA - m_first)) : (unsigned char)0;
-                    __threadfence_block();
-                    __syncwarp();
-                    const unsigned ib = smem_u32(smem + C::OFF_STAGE + (size_t)s * C::WSTAGE);
-                    const int ch = lane & 7, q = lane >> 3;
-#pragma unroll
-                    for (int k = 0; k < 16; ++k) {
-                        const int r = 4 * k + q;                                   // row of the chunk slot = record m_first + r of dst
-                        const int ri = __shfl_sync(FULL, k < 8 ? pr0 : pr1, r & 31);
-                        if (r < nrec) {
-                            // logical 16-byte chunk j of a record sits at position j ^ rec_swizzle(index): source position ch
-                            const int j = ch ^ rec_swizzle(ri);
-                            const unsigned d = ib + r * 128 + 16 * (j ^ rec_swizzle(m_first + r));
-                            const char* gp = reinterpret_cast<const char*>(src + ri) + 16 * ch;
-                            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gp) : "memory");
-                        }
-                    }
-                    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(chunk_bar + 3 * s)) : "memory");
+                    if (p_have) emit();   // the previous chunk goes in while this one's permutation entries are in flight
+                    p_have = 1; p_t = t; p_mfirst = m_first; p_nrec = nrec; p_b = b; p_pr0 = pr0; p_pr1 = pr1;
+                    p_lt = valid ? (unsigned char)(0x80 | (hasB << 6) | (mA - m_first)) : (unsigned char)0;
                 }
             }
             // one end-of-work ticket per compute warp
             for (int q = 0; q < C::NCOMP; ++q, ++ticket) {
-                if (ticket % C::NPUB != pid) continue;
                 const int s = slot_acquire(ticket);
                 if (lane == 0) { desc[s].m_first = -1; __threadfence_block(); }
                 __syncwarp();
                 mbar_arrive(chunk_bar + 3 * s);
             }
-        }
-    } else if (wid < C::NPROD + C::NLOC) {
-        reg_dealloc<C::REG_PROD>();
-        // ------------------------------------------------------------------ locators: warp j takes the tickets t with t % NLOC == j
-        const double h2 = 0.5 * dt;
-        for (unsigned t = wid - C::NPROD;; t += C::NLOC) {
-            const unsigned s = t % C::K, gen = t / C::K;
-            mbar_wait(chunk_bar + 3 * s + 1, gen & 1);
-            const int m_first = desc[s].m_first, nrec = desc[s].nrec, b = desc[s].b;
-            if (m_first < 0) break;
-            const int lt = ltab[s * 32 + lane], lf = lflag[s * 32 + lane];
-            const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
-            const int* stri = reinterpret_cast<const int*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES + C::GEOM_BYTES);
-            const BlockCtrl* ctl = ctl_of(b);
-            const int patch = ctl->patch, ns = ctl->ns;
-            const unsigned slot_base = smem_u32(smem + C::OFF_STAGE + (size_t)s * C::WSTAGE);
-#pragma unroll 1
-            for (int x = 0; x < 2; ++x) {                         // the lane's first, then its second marker (one copy of the code)
-                if (!((lf >> x) & 1)) continue;                   // nothing to locate: no marker, or retired
-                const int row = (lt & 63) + x, m = m_first + row;
-                const unsigned ad = slot_base + row * 128;
-                const int sw = rec_swizzle(m);
-                // next evaluation point: after phase A the stage-4 position held in k, otherwise y + dt/2 k
-                double R, Z, phi, y4, k0, k1, k2, ti, ii;
-                lds128(ad + 16 * (2 ^ sw), y4, k0); lds128(ad + 16 * (3 ^ sw), k1, k2); lds128(ad + 16 * (6 ^ sw), ti, ii);
-                if (PHASE == PHASE_A) { R = k0; Z = k1; phi = k2; }
-                else {
-                    double y0, y1, y2, y3;
-                    lds128(ad + 16 * (0 ^ sw), y0, y1); lds128(ad + 16 * (1 ^ sw), y2, y3);
-                    R = fma(h2, k0, y0); Z = fma(h2, k1, y1); phi = fma(h2, k2, y2);
-                }
-                const int tri0 = __double2loint(ti);              // triangle of the last evaluation point (written by the compute warp)
-                int sl = tri0 - patch * C::TP;
-                if (sl < 0 || sl >= C::TP) {
-                    sl = -1;
-                    for (int q = C::TP; q < ns; ++q) if (stri[q] == tri0) { sl = q; break; }
-                }
-                sl = slot_walk1(sgeom, sl, R, Z);
-                int tn = tri0;
-                if (sl < 0) {   // the point left the staged geometry: k_fix_keys locates it through the global tables (hint: last triangle)
-                    rq.list[rq.n - 1 - atomicAdd(rq.count + 1, 1)] = m;
-                } else {
-                    tn = stri[sl];
-                    if (ko.enabled) {
-                        double sf;
-                        const int k = toroidal_interval(tb.tor, phi, sf);
-                        const int key = cm.cell(tn, k);
-                        ko.keys[m] = key;
-                        atomicAdd(ko.hist + key, 1);
+        } else {
+            // ------------------------------------------------------------------ locators: warp j takes the tickets t with t % NLOC == j
+            const double h2 = 0.5 * dt;
+            for (unsigned t = wid - 2;; t += C::NLOC) {
+                const unsigned s = t % C::K, gen = t / C::K;
+                mbar_wait(chunk_bar + 3 * s + 1, gen & 1);
+                const int m_first = desc[s].m_first, nrec = desc[s].nrec, b = desc[s].b;
+                if (m_first < 0) break;
+                const int lt = ltab[s * 32 + lane], lf = lflag[s * 32 + lane];
+                const SlotGeom* sgeom = reinterpret_cast<const SlotGeom*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES);
+                const int* stri = reinterpret_cast<const int*>(smem + C::BLOCK_BYTES * b + C::COEF_BYTES + C::GEOM_BYTES);
+                const BlockCtrl* ctl = ctl_of(b);
+                const int patch = ctl->patch, ns = ctl->ns;
+                const unsigned slot_base = smem_u32(smem + C::OFF_STAGE + (size_t)s * C::WSTAGE);
+    #pragma unroll 1
+                for (int x = 0; x < 2; ++x) {                         // the lane's first, then its second marker (one copy of the code)
+                    if (!((lf >> x) & 1)) continue;                   // nothing to locate: no marker, or retired
+                    const int row = (lt & 63) + x, m = m_first + row;
+                    const unsigned ad = slot_base + row * 128;
+                    const int sw = rec_swizzle(m);
+                    // next evaluation point: after phase A the stage-4 position held in k, otherwise y + dt/2 k
+                    double R, Z, phi, y4, k0, k1, k2, ti, ii;
+                    lds128(ad + 16 * (2 ^ sw), y4, k0); lds128(ad + 16 * (3 ^ sw), k1, k2); lds128(ad + 16 * (6 ^ sw), ti, ii);
+                    if (PHASE == PHASE_A) { R = k0; Z = k1; phi = k2; }
+                    else {
+                        double y0, y1, y2, y3;
+                        lds128(ad + 16 * (0 ^ sw), y0, y1); lds128(ad + 16 * (1 ^ sw), y2, y3);
+                        R = fma(h2, k0, y0); Z = fma(h2, k1, y1); phi = fma(h2, k2, y2);
                     }
-                    sts128(ad + 16 * (6 ^ sw), __hiloint2double(__double2hiint(ti), tn), ii);
+                    const int tri0 = __double2loint(ti);              // triangle of the last evaluation point (written by the compute warp)
+                    int sl = tri0 - patch * C::TP;
+                    if (sl < 0 || sl >= C::TP) {
+                        sl = -1;
+                        for (int q = C::TP; q < ns; ++q) if (stri[q] == tri0) { sl = q; break; }
+                    }
+                    sl = slot_walk1(sgeom, sl, R, Z);
+                    int tn = tri0;
+                    if (sl < 0) {   // the point left the staged geometry: k_fix_keys locates it through the global tables (hint: last triangle)
+                        rq.list[rq.n - 1 - atomicAdd(rq.count + 1, 1)] = m;
+                    } else {
+                        tn = stri[sl];
+                        if (ko.enabled) {
+                            double sf;
+                            const int k = toroidal_interval(tb.tor, phi, sf);
+                            const int key = cm.cell(tn, k);
+                            ko.keys[m] = key;
+                            atomicAdd(ko.hist + key, 1);
+                        }
+                        sts128(ad + 16 * (6 ^ sw), __hiloint2double(__double2hiint(ti), tn), ii);
+                    }
                 }
-            }
-            // the chunk leaves as ONE bulk copy
-            fence_async_smem();
-            __syncwarp();
-            if (lane == 0) {
-                tma_bulk_s2g(dst + m_first, smem + C::OFF_STAGE + (size_t)s * C::WSTAGE, (unsigned)(nrec * 128));
-                bulk_commit();
-                __threadfence_block();
-                atomicAdd(&ctl_of(b)->done, 1);      // one more chunk of this ring entry done
-                bulk_wait_read0();                   // the copy has read the slot:
-                mbar_arrive(chunk_bar + 3 * s + 2);  // it may be refilled
+                // the chunk leaves as ONE bulk copy
+                fence_async_smem();
+                __syncwarp();
+                if (lane == 0) {
+                    tma_bulk_s2g(dst + m_first, smem + C::OFF_STAGE + (size_t)s * C::WSTAGE, (unsigned)(nrec * 128));
+                    bulk_commit();
+                    __threadfence_block();
+                    atomicAdd(&ctl_of(b)->done, 1);      // one more chunk of this ring entry done
+                    bulk_wait_read0();                   // the copy has read the slot:
+                    mbar_arrive(chunk_bar + 3 * s + 2);  // it may be refilled
+                }
             }
         }
     } else {
@@ -431,7 +439,18 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                 const SlotGeom& gB = sgeom[slB];
                 FieldsG<D2> f;
                 to_fields_g<D2>(D2(gA.a11, gB.a11), D2(gA.a12, gB.a12), D2(gA.a21, gB.a21), D2(gA.a22, gB.a22), acc, yy[3], f);
-                rhs_eval<D2>(ep, sp, yy[0], yy[1], yy[3], yy[4], mu, pw, f, d);
+                // equilibrium and right-hand sides: one marker at a time through ONE copy of the code (registers and
+                // instruction cache; three warps per scheduler supply the FP64 pipe's parallelism here)
+#pragma unroll 1
+                for (int x = 0; x < 2; ++x) {
+                    FieldsG<double> fx;
+                    fx.gR = x ? f.gR.b : f.gR.a; fx.gZ = x ? f.gZ.b : f.gZ.a; fx.gp = x ? f.gp.b : f.gp.a; fx.A = x ? f.A.b : f.A.a;
+                    double dx[5];
+                    rhs_eval<double>(ep, sp, x ? yy[0].b : yy[0].a, x ? yy[1].b : yy[1].a, x ? yy[3].b : yy[3].a, x ? yy[4].b : yy[4].a,
+                                     x ? mu.b : mu.a, x ? pw.b : pw.a, fx, dx);
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) { if (x) d[q].b = dx[q]; else d[q].a = dx[q]; }
+                }
             };
 
             D2 d[5], S[5];
