@@ -36,21 +36,18 @@ struct DevTables {
 };
 
 // tiled push configuration: patches of 8 triangles + halo (SMAX slots with coefficients, 32 with geometry), windows of 4
-// toroidal intervals (+1 each side), ring of NBUF staged blocks, K chunk slots of 64 records, 4 light (stager, publisher, 2 locators) + 12
-// compute warps per CTA, one CTA per SM.  (TRIMEG_* macros: tuning sweeps only; the shipped build uses the defaults.)
+// toroidal intervals (+1 each side), ring of NBUF staged blocks, K chunk slots of 32 records, 4 light + 12 compute warps
+// per CTA, one CTA per SM.  (TRIMEG_* macros: tuning sweeps only; the shipped build uses the defaults.)
 #ifndef TRIMEG_SMAX
-#define TRIMEG_SMAX 12
+#define TRIMEG_SMAX 15
 #endif
 #ifndef TRIMEG_NBUF
-#define TRIMEG_NBUF 2
+#define TRIMEG_NBUF 3
 #endif
 #ifndef TRIMEG_NSLOTS
-#define TRIMEG_NSLOTS 18
+#define TRIMEG_NSLOTS 20
 #endif
-#ifndef TRIMEG_NCOMP
-#define TRIMEG_NCOMP 12
-#endif
-using Tile = TileCfg<8, TRIMEG_SMAX, 4, TRIMEG_NCOMP, TRIMEG_NBUF, TRIMEG_NSLOTS>;
+using Tile = TileCfg<8, TRIMEG_SMAX, 4, TRIMEG_NBUF, TRIMEG_NSLOTS>;
 // cell numbering used by the sort: super-cell (patch, window) major, then triangle within the patch, then interval
 struct CellMap {
     int P, nwin;
@@ -70,11 +67,10 @@ struct KeyOut {
 __constant__ double c_Aplus[21 * 18];
 __constant__ double c_Nul[21 * 3];
 
-// In memory the eight 16-byte chunks of record i are stored XOR-swizzled by rec_swizzle(i) = (i >> 1) & 7: logical chunk j
-// sits at chunk position j ^ rec_swizzle(i) (a record is only ever handled whole, so the swizzle costs nothing).  In the
-// phase kernel lane l reads rows 2l and 2l + 1 of a chunk slot; with this swizzle the eight lanes of a shared-memory
-// wavefront hit eight different 16-byte bank groups.
-__host__ __device__ __forceinline__ int rec_swizzle(long long i) { return (int)(i >> 1) & 7; }
+// In memory the eight 16-byte chunks of record i are stored XOR-swizzled by rec_swizzle(i) = i & 7: logical chunk j sits
+// at chunk position j ^ rec_swizzle(i) (a record is only ever handled whole, so the swizzle costs nothing; it lets
+// row-per-lane shared-memory images of records be read and written 16 bytes per lane without bank conflicts).
+__host__ __device__ __forceinline__ int rec_swizzle(long long i) { return (int)i & 7; }
 __device__ __forceinline__ void rec_load(const Rec* __restrict__ base, long long i, Rec& r) {
     const double2* s = reinterpret_cast<const double2*>(base + i);
     double2* d = reinterpret_cast<double2*>(&r);

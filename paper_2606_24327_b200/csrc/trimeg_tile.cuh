@@ -4,10 +4,9 @@
 // Why tiles: one field evaluation reads 8 x 21 coefficients = 1344 B per marker.  Through L1 with one address per lane
 // that is >= 336 L1 cycles per warp against 338 DFMA = 169 issue cycles of FP64 work.  So the coefficient blocks of a
 // patch of TP triangles plus a halo (SMAX slots), for a window of WK toroidal intervals plus HK on either side, are
-// staged per super-cell with 1-D TMA bulk copies (cp.async.bulk + mbarrier), and markers are visited in cell order, two
-// markers of the same cell per lane, so that one LDS.128 feeds two fields x two markers.  A marker whose evaluation point
-// leaves the staged set RETIRES to a list that a follow-up kernel finishes through the global tables, so that no warp
-// waits on a divergent slow lane.
+// staged per super-cell with 1-D TMA bulk copies (cp.async.bulk + mbarrier), and markers are visited in cell order so
+// that the lanes of a warp read the same few blocks.  A marker whose evaluation point leaves the staged set RETIRES to a
+// list that a follow-up kernel finishes through the global tables, so that no warp waits on a divergent slow lane.
 #pragma once
 #include "trimeg_math.cuh"
 
@@ -21,13 +20,11 @@ struct TileTables {
     int npatch, nwin, nsc;   // super-cells = npatch * nwin
 };
 
-template <int TP_, int SMAX_, int WK_, int NCOMP_, int NBUF_, int K_>
+template <int TP_, int SMAX_, int WK_, int NBUF_, int K_>
 struct TileCfg {
     static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD;
-    // one light warp-group: stager, publisher, two locators; three compute warp-groups
-    static constexpr int NLIGHT = 4, NLOC = 2;
-    static constexpr int NCOMP = NCOMP_;
-    static_assert(NCOMP == 12, "register hand-over below assumes 16 warps");
+    // 16 warps: one light warp-group (stager, two publishers, one spare) and three compute warp-groups
+    static constexpr int NLIGHT = 4, NPUB = 2, NCOMP = 12;
     static constexpr int NWARPS = NLIGHT + NCOMP, NTHREADS = 32 * NWARPS;
     // register hand-over (setmaxnreg): 16 warps launch with 128 registers; the light warps drop to 40, the compute warps
     // take 24 more each (12 x 24 <= 4 x 88)
@@ -35,45 +32,36 @@ struct TileCfg {
     static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
     static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
     static constexpr int CPS = TP * WK;              // cells per super-cell
-    static_assert(CPS == 32, "one lane per cell of a super-cell (pair layout of the publishers)");
     static constexpr int SLOT_DOUBLES = NPL * PLANE_STRIDE;
     static constexpr int NBUF = NBUF_;               // ring of staged blocks
-    static constexpr int K = K_;                     // chunk slots
-    // slot GEOMETRY (64 B per slot) is staged for SGEOM slots, coefficients only for the first SMAX of them: the walk that
+    static constexpr int K = K_;                     // chunk slots: one per compute warp + look-ahead
+    static_assert(K % NPUB == 0, "a chunk slot is always served by the same publisher warp (an odd K hung on the GPU)");
+    // slot GEOMETRY (96 B per slot) is staged for SGEOM slots, coefficients only for the first SMAX of them: the walk that
     // locates the next phase's first evaluation point needs no coefficients and stays in shared memory further out
     static constexpr int SGEOM = 32;
     static_assert(SMAX <= SGEOM, "one slot per lane of the stager");
-    // shared memory carve-up (bytes): NBUF x { coefficients, slot geometry }, control, chunk slots
+    // shared memory carve-up (bytes): NBUF x { coefficients, slot geometry, slot triangles }, control, chunk slots
     static constexpr size_t COEF_BYTES = sizeof(double) * SMAX * SLOT_DOUBLES;
-    static constexpr size_t GEOM_BYTES = 96 * SGEOM;                          // SlotGeom per slot
-    static constexpr size_t BLOCK_BYTES = COEF_BYTES + GEOM_BYTES + 4 * SGEOM; // + triangle id per slot
-    static constexpr size_t CTRL_BYTES = 320;        // BlockCtrl per ring entry
-    static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;
-    static constexpr size_t OFF_BAR = OFF_CTRL + CTRL_BYTES * NBUF;          // per ring entry: full, seen (8 B each)
+    static constexpr size_t GEOM_BYTES = 96 * SGEOM;
+    static constexpr size_t BLOCK_BYTES = COEF_BYTES + GEOM_BYTES + 4 * SGEOM;
+    static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;                   // BlockCtrl (64 B) per ring entry
+    static constexpr size_t OFF_BAR = OFF_CTRL + 64 * NBUF;                  // per ring entry: full, seen (8 B each)
     static constexpr size_t OFF_DESC = OFF_BAR + 16 * NBUF;                  // per chunk slot: ChunkDesc (16 B)
-    static constexpr size_t OFF_LTAB = OFF_DESC + 16 * K;                    // per chunk slot: 32 lane bytes
-    static constexpr size_t OFF_LFLAG = OFF_LTAB + 32 * K;                   // per chunk slot: 32 lane bytes written by the compute warp
-    static constexpr size_t OFF_CBAR = OFF_LFLAG + 32 * K;                   // per chunk slot: full, computed, empty (8 B each)
-    static constexpr size_t OFF_HEAD = OFF_CBAR + 24 * K;                    // ticket counter
-    static constexpr int CHUNK = 64;                                         // marker records per chunk slot (two per lane)
+    static constexpr size_t OFF_CBAR = OFF_DESC + 16 * K;                    // per chunk slot: full, empty (8 B each)
+    static constexpr size_t OFF_HEAD = OFF_CBAR + 16 * K;                    // ticket counter
+    static constexpr int CHUNK = 32;                                         // marker records per chunk slot (one per lane)
     static constexpr size_t WSTAGE = CHUNK * 128;
     static constexpr size_t OFF_STAGE = (OFF_HEAD + 16 + 127) / 128 * 128;
     static constexpr size_t BYTES = OFF_STAGE + WSTAGE * K;
     static_assert(BYTES <= 227 * 1024, "shared memory per CTA");
 };
-// one ring entry = one super-cell.  Cells of the super-cell are numbered 0..31 (triangle-in-patch major, interval minor);
-// the markers of a cell are paired up (an odd cell leaves one half-empty pair) so that both markers of a lane share
-// their coefficient block.
-struct BlockCtrl {
-    int sc, patch, k0, ns;
-    int nchunks;           // chunks that will be cut from this entry
-    int done;              // chunks finished (compute warps count up)
-    int npairs, pad;
-    int cell_off[33];      // first marker position of each cell (cell order), [32] = end
-    int pair_incl[32];     // inclusive prefix sum of pairs per cell
+struct BlockCtrl {   // 64 B per ring entry
+    int sc, begin, end, patch, k0, ns;
+    int nchunks;     // chunks that will be cut from this entry
+    int done;        // chunks finished (compute warps count up)
+    int pad[8];
 };
-static_assert(sizeof(BlockCtrl) <= 320, "BlockCtrl fits its slot");
-struct ChunkDesc { int m_first, nrec, b, pad; };   // m_first < 0: no more work
+struct ChunkDesc { int m0, end, b, pad; };   // m0 < 0: no more work
 
 // Geometry of one staged slot, 96 B.  The edge walk tests the three barycentrics in the form l = a R + b Z + c (two
 // dependent FMAs each; their rounding, ~1e-13, only matters within the walk's 1e-12 tolerance band, where either
