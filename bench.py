@@ -25,16 +25,35 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2606_24327_b200 import shard, synth  # noqa: E402
+from paper_2606_24327_b200 import flopcount, shard, synth  # noqa: E402
 
 METRIC = "marker RK4 pushes/sec incl. field gather (fp64, 1 B200), % of roofline"
 UNIT = "marker-pushes/s"
-FLOP_PER_PUSH = 3772.0          # 943 flop per RK stage x 4
+# Algorithmic work: SURVEY.md 8(d)'s per-unit figure (943 flop per right-hand-side evaluation x 4 stages) is what the
+# roofline uses; the count regenerated from this repo's own minimal formulation (paper_2606_24327_b200/flopcount.py,
+# `python -m paper_2606_24327_b200.flopcount`) is printed beside it.
+FLOP_PER_PUSH = 4.0 * flopcount.SURVEY_FLOP_PER_EVAL
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SM x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
 KEYS = ("R", "Z", "phi", "u", "w", "mu", "p")
-TRAFFIC_BYTES_PER_LAUNCH = 28.68e9   # dram__bytes_read.sum + dram__bytes_write.sum of one k_phase_ws launch (profiles/r01e_summary.md)
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "traffic.csv")   # dram bytes per launch of the dominant kernel, from a tracked ncu capture
 ALGO_BYTES_PER_LAUNCH = 2 * 112 + 8 + 17   # per marker: 112 live record bytes in and out, permutation + key, one pass over the coefficient table
-SORT_EVERY = 1                  # two-phase kernel: both phases re-bin every step (BASELINE configs[2] uses 10)
+SORT_EVERY = 1                  # both phases re-bin every step (DESIGN.md section 6 "Sort interval": faster than BASELINE configs[2]'s every 10)
+PARITY_TOL_10 = 1e-10           # north_star: marker state after 10 RK4 steps
+
+
+def measured_traffic(cfg_name, n, variant):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, read from the tracked ncu summary
+    profiles/traffic.csv (rows written from `ncu --set full` captures; each names the commit and the workload it was taken
+    on; the last matching row wins).  None when no row is for this workload."""
+    import csv
+    best = (None, None)
+    try:
+        for r in csv.DictReader(open(TRAFFIC_FILE)):
+            if r["workload"] == cfg_name and int(r["markers"]) == n and int(r["variant"]) == variant:
+                best = (float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]), {k: r[k] for k in ("kernel", "commit", "source")})
+    except Exception:
+        pass
+    return best
 
 
 def make_inputs(cfg, n, start, pinned):
@@ -42,12 +61,17 @@ def make_inputs(cfg, n, start, pinned):
     import torch
     host = {k: (torch.empty(n, dtype=torch.float64, pin_memory=True) if pinned else torch.empty(n, dtype=torch.float64)) for k in KEYS}
     views = {k: v.numpy() for k, v in host.items()}
-    chunk = 5_000_000
-    for s in range(0, n, chunk):
+    chunk = 2_000_000
+
+    def fill(s):
         e = min(n, s + chunk)
-        m = synth.make_markers(cfg, e - s, start + s)
+        m = synth.make_markers(cfg, e - s, start + s)   # counter-based generator: any slice, any order
         for k in KEYS:
             views[k][s:e] = m[k]
+
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=min(32, os.cpu_count() or 8)) as ex:
+        list(ex.map(fill, range(0, n, chunk)))
     return host, views
 
 
@@ -98,11 +122,13 @@ def setup_case(cfg, backend):
     return RZ, tri, (dphi, dap)
 
 
-def time_oracle(cfg, n_sample, steps, start=0):
+def time_oracle(cfg, n_sample, steps, start=0, oracle=None):
     """The oracle as it stands on the host cores: pushes/s on n_sample markers x steps RK4 steps."""
     from oracle import Oracle, oracle_threads
-    o = Oracle()
-    setup_case(cfg, o)
+    o = oracle
+    if o is None:
+        o = Oracle()
+        setup_case(cfg, o)
     m = synth.make_markers(cfg, n_sample, start)
     args = [m[k] for k in KEYS]
     t0 = time.perf_counter()
@@ -204,6 +230,8 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=400_000, help="markers of the oracle cpu_baseline leg (x 4 steps)")
     ap.add_argument("--ref-markers", type=int, default=200_000, help="markers per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-parity", action="store_true", help="skip the sampled oracle check of the timed run")
+    ap.add_argument("--parity-sample", type=int, default=10_000, help="markers of the timed run compared with the oracle")
     ap.add_argument("--gather", action="store_true", help="gather-only stress test (use with --config 4), unsorted vs cell-sorted points")
     args = ap.parse_args()
 
@@ -251,35 +279,55 @@ def main():
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    launches, slow, retired, kms = 0, 0, 0, []
-    ev[0].record()
-    for s in range(args.steps):
-        g.push_rk4(cfg.dt, 1)
-        ev[s + 1].record()
-        st = g.push_stats()          # reads device counters: synchronises the stream after the step's last kernel
-        kms.append(g.push_kernel_ms())   # CUDA events recorded by the library on its stream around each kernel group
-        launches += st["launches"]
-        slow += st["slow_path"]
-        retired += st["retired"]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    g.push_rk4(cfg.dt, args.steps)     # EXACTLY K steps, nothing else between the two events (no host round trip)
+    ev1.record()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     clocks = sampler.stop() if rank == 0 else None
-    step_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
-    total_s = shard.reduce_max_seconds(sum(step_ms) * 1e-3, dist if world > 1 else None)
+    # counters and per-kernel times are read AFTER the timed region: launches, follow-up evaluations and retired markers of
+    # the K steps; CUDA events recorded by the library on its own stream around each kernel group, mean over the K steps
+    st = g.push_stats()
+    km = g.push_kernel_ms()
+    launches, slow, retired = st["launches"], st["slow_path"], st["retired"]
+    total_s = shard.reduce_max_seconds(ev0.elapsed_time(ev1) * 1e-3, dist if world > 1 else None)
     value = shard.job_rate(n * args.steps, world, total_s)
     # dominant kernel: the phase kernel k_phase_ws, launched twice per step (phase A: k2, k3; phase B: k4, next k1).
     # Algorithmic flops per launch = 943 flop x the right-hand-side evaluations it performed (2 n minus those left to the
     # follow-up kernel), over its average launch duration from the library's CUDA events (sum of the two launches / 2).
     launches_per_step = 2 if args.variant == 0 else 1
-    kern_s = statistics.mean(k["push"] for k in kms) * 1e-3 / launches_per_step
-    sort_ms = statistics.mean(k["sort"] for k in kms)
-    finish_ms = statistics.mean(k["finish"] for k in kms)
+    kern_s = km["push"] * 1e-3 / launches_per_step
+    sort_ms, finish_ms = km["sort"], km["finish"]
     stage_evals = (4.0 * n - slow / args.steps) / launches_per_step
     achieved = (FLOP_PER_PUSH / 4.0) * stage_evals / kern_s / 1e12
-    step_achieved = FLOP_PER_PUSH * n * args.steps / (sum(step_ms) * 1e-3) / 1e12
+    step_achieved = FLOP_PER_PUSH * n / (total_s / args.steps) / 1e12
+
+    # ---- parity of THIS run: a strided sample of the markers just pushed (W + K steps) against the oracle on the same inputs
+    parity, oracle_obj = None, None
+    if not args.no_parity:
+        from oracle import Oracle
+        oracle_obj = Oracle()
+        setup_case(cfg, oracle_obj)
+        nst = args.warmup + args.steps
+        idx = np.unique(np.concatenate([np.arange(0, n, max(1, n // args.parity_sample)), [n - 1]]))
+        got = g.markers_get()
+        tidx = torch.from_numpy(idx).cuda()
+        got = {k: v[tidx].cpu().numpy() for k, v in got.items()}
+        exp = oracle_obj.push_rk4(*[views[k][idx] for k in KEYS], cfg.dt, nst)
+        tol = PARITY_TOL_10 * max(1.0, (nst / 10.0) ** 2)   # rounding-level differences grow at most quadratically over a few steps
+        errs = {}
+        for q, k in enumerate(("R", "Z", "phi", "u", "w")):
+            dlt = np.abs(got[k] - exp[q])
+            if k == "phi":
+                dlt = np.minimum(dlt, np.abs(dlt - cfg.phi_period))
+            errs["max_rel_" + k] = float(dlt.max() / max(np.abs(exp[q]).max(), 1e-300))
+        lost_equal = bool(((got["status"] != 0) == (exp[5] != 0)).all())
+        parity = {"n": int(idx.shape[0]), "steps": nst, "tol": tol, **errs, "lost_set_equal": lost_equal, "lost": int((exp[5] != 0).sum()),
+                  "ok": bool(lost_equal and max(errs.values()) < tol), "against": "oracle/ (CPU, fp64) on the same seeded inputs"}
+        del got, tidx
 
     # ---- end to end through the C-ABI with HOST buffers (pinned): H2D marker arrays, push, D2H result
     pinned_out = {k: torch.empty(n, dtype=torch.float64, pin_memory=True).numpy() for k in ("R", "Z", "phi", "u", "w")}
@@ -303,7 +351,8 @@ def main():
     torch.cuda.synchronize()
     e2e_s = shard.reduce_max_seconds(a.elapsed_time(b) * 1e-3, dist if world > 1 else None)
     e2e_val = shard.job_rate(n * e2e_steps, world, e2e_s)
-    checksum = float(pinned_out["w"][: min(n, 1000)].sum())
+    traffic, traffic_src = measured_traffic(cfg.name, n, args.variant)
+    own = flopcount.count()
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -313,24 +362,33 @@ def main():
                         "note": "every e2e step re-binds from HOST buffers, so it also pays the locate + k1 initialisation of a fresh store; PCIe-bound"},
                 "gpu_launches": launches,
                 "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
-                             "traffic": TRAFFIC_BYTES_PER_LAUNCH if (args.variant == 0 and args.config == 3 and n == cfg.n_markers) else None,
+                             "traffic": traffic, "traffic_source": traffic_src,
                              "kernel": "k_phase_ws" if args.variant == 0 else "k_push_simple", "kernel_ms": 1e3 * kern_s,
                              "kernel_launches_per_step": launches_per_step,
                              "flop_per_push": FLOP_PER_PUSH, "stage_evals_per_launch": stage_evals,
+                             "flop_count": {"used": "SURVEY.md 8(d): 943 flop per right-hand-side evaluation x 4",
+                                            "regenerated_per_eval": own["total"]["flop"],
+                                            "regenerated_parts": {k: v["flop"] for k, v in own.items() if k != "total"},
+                                            "regenerated_ops": {k: own["total"][k] for k in ("add", "mul", "div", "sqrt", "exp")},
+                                            "frac_with_regenerated_count": achieved / FP64_PEAK_TFLOPS * own["total"]["flop"] / flopcount.SURVEY_FLOP_PER_EVAL,
+                                            "source": "python -m paper_2606_24327_b200.flopcount"},
                              "peak_kind": "nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (derived, DESIGN.md)",
                              "measured_dfma_tflops": dfma, "frac_of_measured_dfma": achieved / dfma,
                              "whole_step_frac": step_achieved / FP64_PEAK_TFLOPS,
                              "hbm_algorithmic_GBps": ALGO_BYTES_PER_LAUNCH * n / kern_s / 1e9},
                 "step_breakdown_ms": {"sort": sort_ms, "push": 1e3 * kern_s * launches_per_step, "finish": finish_ms},
-                "slow_path_evals": slow, "retired_markers": retired, "e2e_checksum": checksum}
+                "slow_path_evals": slow, "retired_markers": retired, "parity": parity}
         if not args.no_cpu_baseline:
             cpu_n = min(n, args.cpu_sample)
-            v, cores, secs = time_oracle(cfg, cpu_n, 4)
+            v, cores, secs = time_oracle(cfg, cpu_n, 4, oracle=oracle_obj)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
                                     "sample": f"first {cpu_n} markers of the same workload x 4 RK4 steps"}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+    if parity is not None and not parity["ok"]:
+        print(f"bench.py: parity against the oracle FAILED on rank {rank}: {parity}", file=sys.stderr)
+        sys.exit(1)
 
 
 if __name__ == "__main__":

@@ -95,7 +95,9 @@ int trimeg_fields_set(trimeg_ctx* ctx, int which, const double* dof, int memspac
 int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi, double* out,
                   int32_t* tri_out, int memspace);
 
-/* Bytes of DEVICE scratch trimeg_markers_bind needs for n markers (0 on error). */
+/* Bytes of DEVICE scratch trimeg_markers_bind needs for n markers (0 on error): 268 bytes per marker (two buffers of
+ * 128-byte records for the re-sorting phases + sort key, permutation and follow-up list, 4 bytes each): 26.8 GB at 1e8
+ * markers.  This is twice the structure-of-arrays budget of SURVEY.md 8(a) (a1); DESIGN.md section 5 says why. */
 size_t trimeg_scratch_bytes(const trimeg_ctx* ctx, int64_t n);
 
 /* Hand n markers to the library (L89: R, Z, phi, v_par, w per marker; mu and p are constants of the motion).
@@ -150,8 +152,8 @@ int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops);
  * slow (out-of-block) path in the follow-up kernel, [2] marker-phases that left their staged block (summed over
  * phases and steps), [3] permutations built. */
 int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]);
-/* Device time (CUDA events on the context's stream; blocks until they have completed) of the last RK4 step of the
- * last trimeg_push_rk4 call, in milliseconds: [0] sort kernels of that step (scan, permutation; both phases), [1] the
+/* Device time (CUDA events on the context's stream; blocks until they have completed) per RK4 step, averaged over the
+ * (up to 32) last steps of the last trimeg_push_rk4 call, in milliseconds: [0] sort kernels of a step (scan, permutation; both phases), [1] the
  * two launches of the phase kernel (the roofline's "dominant kernel"; divide by 2 for one launch), [2] the follow-up
  * kernels (markers that left their staged block, markers outside the mesh).  Errors: BAD_ARG, BAD_STATE (nothing pushed yet), CUDA. */
 int trimeg_push_kernel_ms(trimeg_ctx* ctx, double out[3]);

@@ -55,9 +55,10 @@ struct trimeg_ctx {
     long long steps_since_sort = 0;
     int variant = 0;
     long long stats[4] = {0, 0, 0, 0};
-    // per-kernel timing of the last step of trimeg_push_rk4 (events on the context's stream)
-    cudaEvent_t ev[8] = {};
-    bool ev_valid = false;
+    // per-kernel timing of the last (up to EV_STEPS) steps of the last trimeg_push_rk4 call (events on the context's stream)
+    static constexpr int EV_STEPS = 32;
+    cudaEvent_t ev[EV_STEPS][8] = {};
+    int ev_steps = 0;            // steps of the last call that carry events
     // tiled kernel tables
     int *d_pslots = nullptr, *d_pnslots = nullptr, *d_work = nullptr;
     short* d_pnbr = nullptr;
@@ -136,7 +137,7 @@ int trimeg_create(trimeg_ctx** out, int device, void* cuda_stream) {
         delete c;
         return TRIMEG_ERR_CUDA;
     }
-    for (auto& e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
+    for (auto& st : c->ev) for (auto& e : st) if (cudaEventCreate(&e) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
     *out = c;
     return TRIMEG_OK;
 }
@@ -145,7 +146,7 @@ int trimeg_destroy(trimeg_ctx* ctx) {
     if (!ctx) return TRIMEG_ERR_BAD_ARG;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    for (auto& e : ctx->ev) if (e) cudaEventDestroy(e);
+    for (auto& st : ctx->ev) for (auto& e : st) if (e) cudaEventDestroy(e);
     free_mesh(ctx);
     delete ctx;
     return TRIMEG_OK;
@@ -482,9 +483,10 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps) {
     ctx->stats[0] = ctx->stats[1] = ctx->stats[2] = ctx->stats[3] = 0;
     CU(cudaMemsetAsync(ctx->d_stats, 0, sizeof(unsigned long long) * 4, ctx->stream));
     const long long n = ctx->n;
-    ctx->ev_valid = false;
+    ctx->ev_steps = 0;
     for (int s = 0; s < nsteps; ++s) {
-        const bool timed = (s == nsteps - 1);
+        const bool timed = (nsteps - s <= trimeg_ctx::EV_STEPS);
+        cudaEvent_t* const sev = ctx->ev[timed ? ctx->ev_steps : 0];
         if (ctx->variant == 0 && ctx->tiled_ok) {
             const bool need_sort = ctx->force_sort || !ctx->order_valid || (ctx->sort_every > 0 && ctx->steps_since_sort >= ctx->sort_every);
             if (!ctx->k1_valid || ctx->key_dt != dt || (need_sort && !ctx->keys_valid)) {
@@ -512,24 +514,24 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps) {
             }
             const long long next_since = need_sort ? 1 : ctx->steps_since_sort + 1;
             const bool next_sorts = ctx->sort_every > 0 && next_since >= ctx->sort_every;
-            if (timed) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
-            int rc = run_phase<PHASE_A>(ctx, dt, need_sort, need_sort, timed ? ctx->ev + 1 : nullptr);
+            if (timed) CU(cudaEventRecord(sev[0], ctx->stream));
+            int rc = run_phase<PHASE_A>(ctx, dt, need_sort, need_sort, timed ? sev + 1 : nullptr);
             if (rc) return rc;
-            if (timed) CU(cudaEventRecord(ctx->ev[4], ctx->stream));
-            rc = run_phase<PHASE_B>(ctx, dt, need_sort, next_sorts, timed ? ctx->ev + 5 : nullptr);
+            if (timed) CU(cudaEventRecord(sev[4], ctx->stream));
+            rc = run_phase<PHASE_B>(ctx, dt, need_sort, next_sorts, timed ? sev + 5 : nullptr);
             if (rc) return rc;
             ctx->keys_valid = next_sorts;
             ctx->steps_since_sort = next_since;
             ctx->force_sort = false;
         } else {
-            if (timed) { CU(cudaEventRecord(ctx->ev[0], ctx->stream)); CU(cudaEventRecord(ctx->ev[1], ctx->stream)); }
+            if (timed) { CU(cudaEventRecord(sev[0], ctx->stream)); CU(cudaEventRecord(sev[1], ctx->stream)); }
             k_push_simple<<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->recs[ctx->cur], n, dt);
             KCHECK();
-            if (timed) for (int q = 2; q < 8; ++q) CU(cudaEventRecord(ctx->ev[q], ctx->stream));
+            if (timed) for (int q = 2; q < 8; ++q) CU(cudaEventRecord(sev[q], ctx->stream));
             invalidate_step_state(ctx);
             ctx->stats[0] += 1;
         }
-        if (timed) ctx->ev_valid = true;
+        if (timed) ++ctx->ev_steps;
     }
     return TRIMEG_OK;
 }
@@ -543,19 +545,20 @@ int trimeg_push_variant_used(trimeg_ctx* ctx, int32_t* out) {
 
 int trimeg_push_kernel_ms(trimeg_ctx* ctx, double out[3]) {
     if (!ctx || !out) return fail(ctx, TRIMEG_ERR_BAD_ARG, "push_kernel_ms: null argument");
-    if (!ctx->ev_valid) return fail(ctx, TRIMEG_ERR_BAD_STATE, "push_kernel_ms: no step has been pushed");
+    if (ctx->ev_steps <= 0) return fail(ctx, TRIMEG_ERR_BAD_STATE, "push_kernel_ms: no step has been pushed");
     CU(cudaSetDevice(ctx->device));
-    CU(cudaEventSynchronize(ctx->ev[7]));
+    CU(cudaEventSynchronize(ctx->ev[ctx->ev_steps - 1][7]));
     // events: 0 step start | 1 A tiled start, 2 A tiled end, 3 A follow-ups end | 4 B start | 5 B tiled start, 6 B tiled end, 7 B follow-ups end
     const int span[3][2][2] = {{{0, 1}, {4, 5}}, {{1, 2}, {5, 6}}, {{2, 3}, {6, 7}}};
     for (int i = 0; i < 3; ++i) {
         double tot = 0;
-        for (int h = 0; h < 2; ++h) {
-            float ms = 0;
-            CU(cudaEventElapsedTime(&ms, ctx->ev[span[i][h][0]], ctx->ev[span[i][h][1]]));
-            tot += ms;
-        }
-        out[i] = tot;
+        for (int st = 0; st < ctx->ev_steps; ++st)
+            for (int h = 0; h < 2; ++h) {
+                float ms = 0;
+                CU(cudaEventElapsedTime(&ms, ctx->ev[st][span[i][h][0]], ctx->ev[st][span[i][h][1]]));
+                tot += ms;
+            }
+        out[i] = tot / ctx->ev_steps;   // mean per step over the timed steps of the last call
     }
     return TRIMEG_OK;
 }

@@ -12,6 +12,7 @@ normals by Box-Muller.  Same numbers on every platform, any order of generation.
 """
 from __future__ import annotations
 
+import dataclasses
 from dataclasses import dataclass, field
 
 import numpy as np
@@ -217,7 +218,12 @@ def field_dofs(modes, RZ, n_planes, R0, a, phi_period=2 * np.pi, deconvolve=True
     out = np.zeros((n_planes, RZ.shape[0], 6))
     for md in modes:
         sym = (2.0 + np.cos(md.n * dphi)) / 3.0 if deconvolve else 1.0
-        out += mode_field([md], RZ[None, :, 0], RZ[None, :, 1], phik[:, None], R0, a) / sym
+        # cos(m theta + phase - n phi) = cos(m theta + phase) cos(n phi) + sin(m theta + phase) sin(n phi): the poloidal
+        # factors (and their R, Z derivatives) are evaluated once per node, not once per node and plane
+        C = mode_field([md], RZ[:, 0], RZ[:, 1], 0.0, R0, a) / sym
+        S = mode_field([dataclasses.replace(md, phase=md.phase - 0.5 * np.pi)], RZ[:, 0], RZ[:, 1], 0.0, R0, a) / sym
+        for k in range(n_planes):
+            out[k] += np.cos(md.n * phik[k]) * C + np.sin(md.n * phik[k]) * S
     return out
 
 

@@ -1,0 +1,201 @@
+"""GPU parity on BASELINE configs 2 and 4 as stated, and on the code paths the config tests do not reach
+(ragged patch, few planes, Morton numbering, equilibrium re-set, lost-marker rule of both push variants, C-ABI errors).
+
+Same norm and tolerances as tests/test_gpu_parity.py (reading R18): 1e-12 per gathered quantity,
+1e-10 per state quantity after 10 RK4 steps.  After 20 steps the bound is 4e-10: the two sides differ by rounding
+only, and on these orbits a rounding-level difference grows at most quadratically in the step count over a few
+steps (a difference in u shears phi linearly in time, which feeds back through the phi-dependent fields), so
+(20 / 10)^2 = 4 times the 10-step bound.
+"""
+import ctypes as C
+import dataclasses
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2606_24327_b200 import synth  # noqa: E402
+from test_gpu_parity import GATHER_TOL, KEYS, STATE_TOL, _check_push, _dev, _make, _rel  # noqa: E402
+
+
+def _compare_state(res, exp, idx, period, tol, what):
+    st_gpu, st_ref = res["status"][idx] != 0, exp[5] != 0
+    assert (st_gpu == st_ref).all(), f"{what}: lost-marker sets differ at {np.flatnonzero(st_gpu != st_ref)[:10]}"
+    errs = {}
+    for q, k in enumerate(("R", "Z", "phi", "u", "w")):
+        errs[k] = _rel(res[k][idx], exp[q], period if k == "phi" else None)
+    assert max(errs.values()) < tol, (what, errs)
+    return errs
+
+
+def test_cfg2_as_stated_profile_loading_sort_every_10():
+    """BASELINE configs[2]: 20 020 triangles x 32 planes, EM fields, markers loaded with the Eq.(8) density and
+    temperature profiles, re-sorted every 10 steps.  1e6 of its 1e7 markers, 20 steps: both stale decades and the
+    re-sort between them are crossed; a strided 10 000-marker sample (including the last marker) against the oracle
+    after 10 steps (1e-10) and after 20 steps (4e-10, see the module docstring), all statuses of the sample."""
+    cfg = dataclasses.replace(synth.CONFIGS[2], n_markers=1_000_000)
+    assert cfg.loading == "profile" and cfg.sort_every == 10 and cfg.n_planes == 32 and 2 * cfg.nr * cfg.ntheta == 20_020
+    RZ, tri, o, g, m = _make(cfg)
+    sample = np.unique(np.concatenate([np.arange(0, cfg.n_markers, 100), [cfg.n_markers - 1]]))
+    d = _dev(m)
+    g.set_push_variant(0)
+    g.set_sort_interval(cfg.sort_every)
+    g.markers_bind(*[d[k] for k in KEYS])
+    g.push_rk4(cfg.dt, 10)
+    st10 = g.push_stats()
+    res10 = g.markers_get(host=True)
+    g.push_rk4(cfg.dt, 10)
+    st20 = g.push_stats()
+    res20 = g.markers_get(host=True)
+    ins = [m[k][sample] for k in KEYS]
+    e10 = _compare_state(res10, o.push_rk4(*ins, cfg.dt, 10), sample, cfg.phi_period, STATE_TOL, "10 steps")
+    e20 = _compare_state(res20, o.push_rk4(*ins, cfg.dt, 20), sample, cfg.phi_period, 4 * STATE_TOL, "20 steps")
+    print("cfg2 parity", e10, e20, st10, st20)
+    # first call: one order for k1 and one for each phase of step 1, then stale; second call: one re-sort (two orders)
+    assert st10["sorts"] == 3 and st20["sorts"] == 2
+    assert g.push_variant_used() == 0
+
+
+def test_cfg4_mesh_gather_random_and_sorted_host_and_device():
+    """BASELINE configs[4]'s mesh and fields (299 904 triangles x 64 planes: a 6.95 GB coefficient table, the only case
+    whose table offsets exceed 2^32 bytes).  2e6 of its points; the oracle checks a strided 1e5-point sample (including
+    the last point) in random order and in cell-sorted order, through DEVICE and HOST buffers."""
+    import torch
+    cfg = dataclasses.replace(synth.CONFIGS[4], n_markers=2_000_000)
+    assert 2 * cfg.nr * cfg.ntheta == 299_904 and cfg.n_planes == 64
+    RZ, tri, o, g, m = _make(cfg)
+    n = cfg.n_markers
+    sample = np.unique(np.concatenate([np.arange(0, n, 20), [n - 1]]))
+    ref, tref = o.gather(m["R"][sample], m["Z"][sample], m["phi"][sample])
+    # the sample touches the far end of the table
+    assert tref.max() > 0.99 * tri.shape[0]
+
+    def check(out, tout, idx, what):
+        assert ((tout[idx] < 0) == (tref < 0)).all(), what
+        for q in range(8):
+            e = _rel(out[q][idx], ref[q])
+            assert e < GATHER_TOL, (what, q, e)
+
+    d = _dev({k: m[k] for k in ("R", "Z", "phi")})
+    out, tout = g.gather(d["R"], d["Z"], d["phi"])
+    out, tout = out.cpu().numpy(), tout.cpu().numpy()
+    check(out, tout, sample, "device, random order")
+    # cell-sorted order (caller's triangle ids x toroidal interval), HOST buffers
+    k = np.minimum((np.mod(m["phi"], cfg.phi_period) / cfg.phi_period * cfg.n_planes).astype(np.int64), cfg.n_planes - 1)
+    order = np.argsort(tout.astype(np.int64) * cfg.n_planes + k, kind="stable")
+    inv = np.empty_like(order)
+    inv[order] = np.arange(n)
+    outs, touts = g.gather(np.ascontiguousarray(m["R"][order]), np.ascontiguousarray(m["Z"][order]), np.ascontiguousarray(m["phi"][order]))
+    check(outs, touts, inv[sample], "host, cell-sorted order")
+    assert np.array_equal(outs[:, inv], out) and np.array_equal(touts[inv], tout)   # the order of the points changes nothing
+    del d
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("nr,ntheta,n_planes,expect_variant", [(7, 9, 6, 0), (7, 9, 10, 0), (9, 11, 7, 0), (6, 11, 5, 1), (6, 11, 4, 1)])
+def test_push_ragged_patch_and_few_planes(nr, ntheta, n_planes, expect_variant):
+    """Triangle counts that are not multiples of the patch size (the last patch is padded with unused slots), plane counts
+    that are not multiples of the window (n_planes = 6, 7, 10) and plane counts below the tiled kernel's minimum (4, 5:
+    the library then runs variant 1 and says so through trimeg_push_variant_used)."""
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, nr=nr, ntheta=ntheta, n_planes=n_planes, n_markers=6007)
+    assert (2 * nr * ntheta) % 8 != 0
+    RZ, tri, o, g, m = _make(cfg)
+    _check_push(o, g, m, cfg, 0.05, 10, 0, sort_every=1)
+    assert g.push_variant_used() == expect_variant
+    _check_push(o, g, m, cfg, 0.05, 10, 0, sort_every=4)
+
+
+def test_mesh_before_equilibrium_and_equilibrium_reset_after_species():
+    """mesh_load before any equilibrium is known (Morton numbering of the triangles instead of flux-surface numbering), and
+    an equilibrium that is replaced AFTER the species was set: the Eq.(8) scalars that depend on a and R0 must follow."""
+    from oracle import Oracle
+    from paper_2606_24327_b200.binding import Trimeg
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, nr=12, ntheta=40, n_planes=8, n_markers=9001)
+    RZ, tri = synth.make_mesh(cfg)
+    dphi, dap = synth.make_fields(cfg, RZ)
+    m = synth.make_markers(cfg)
+    o, g = Oracle(), Trimeg(0)
+    g.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)          # no equilibrium yet
+    wrong = dict(synth.equilibrium_args(cfg), R0=cfg.R0 * 1.3, a=cfg.a * 0.8)
+    g.equilibrium_set(**wrong)
+    g.species_set(**synth.species_args(cfg))
+    g.equilibrium_set(**synth.equilibrium_args(cfg))             # replaces R0 and a after the species
+    o.equilibrium_set(**synth.equilibrium_args(cfg))
+    o.species_set(**synth.species_args(cfg))
+    o.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+    for x in (o, g):
+        x.fields_set(0, dphi)
+        x.fields_set(1, dap)
+    _check_push(o, g, m, cfg, 0.05, 10, 0, sort_every=1)
+    d = _dev(m)
+    g.markers_bind(*[d[k] for k in KEYS])
+    out = g.rhs(host=True)
+    ref, _ = o.rhs(*[m[k] for k in KEYS])
+    assert _rel(out[4], ref[4]) < 1e-11
+
+
+def test_lost_marker_rule_identical_in_both_variants_near_the_boundary():
+    """Markers loaded in a thin shell at the outer boundary (many leave, some end a step just outside without any stage of
+    that step outside): both push variants and the oracle must report the same lost set after every step count."""
+    cfg = dataclasses.replace(synth.CONFIGS[0], n_markers=4000)
+    RZ, tri, o, g, m = _make(cfg)
+    r = cfg.a * (0.985 + 0.0149 * synth.uniform(77, 1, cfg.n_markers))
+    th = 2 * np.pi * synth.uniform(77, 2, cfg.n_markers)
+    m["R"], m["Z"] = cfg.R0 + r * np.cos(th), r * np.sin(th)
+    lost = []
+    for nsteps in (1, 2, 3, 7):
+        per_variant = []
+        for variant in (0, 1):
+            res, exp = _check_push(o, g, m, cfg, 0.05, nsteps, variant, sort_every=1)
+            per_variant.append(res["status"] != 0)
+        assert np.array_equal(per_variant[0], per_variant[1])
+        lost.append(int(per_variant[0].sum()))
+    assert lost[-1] > lost[0] > 0 and lost[-1] < cfg.n_markers
+
+
+def test_abi_null_pointers_and_bad_memspace():
+    """Errors the header promises (include/trimeg.h): null pointers and an unknown memspace return TRIMEG_ERR_BAD_ARG (-1)
+    through the raw C-ABI, and leave the context usable."""
+    import torch
+    from paper_2606_24327_b200.binding import Trimeg, load_library
+    lib = load_library()
+    cfg = synth.CONFIGS[0]
+    RZ, tri = synth.make_mesh(cfg)
+    g = Trimeg(0)
+    h = g._h
+    assert lib.trimeg_create(None, 0, None) == -1
+    assert lib.trimeg_equilibrium_set(h, None) == -1
+    assert lib.trimeg_species_set(h, None) == -1
+    assert lib.trimeg_mesh_load(h, RZ.shape[0], None, tri.shape[0], tri.ctypes.data, 8, 6.28) == -1
+    assert lib.trimeg_mesh_load(h, RZ.shape[0], RZ.ctypes.data, tri.shape[0], None, 8, 6.28) == -1
+    g.equilibrium_set(**synth.equilibrium_args(cfg))
+    g.species_set(**synth.species_args(cfg))
+    g.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+    dof = np.zeros((cfg.n_planes, RZ.shape[0], 6))
+    assert lib.trimeg_fields_set(h, 0, None, 0) == -1
+    assert lib.trimeg_fields_set(h, 2, dof.ctypes.data, 0) == -1
+    assert lib.trimeg_fields_set(h, 0, dof.ctypes.data, 7) == -1
+    x = torch.zeros(16, dtype=torch.float64, device="cuda")
+    out = torch.zeros((8, 16), dtype=torch.float64, device="cuda")
+    p = x.data_ptr()
+    assert lib.trimeg_gather(h, 16, None, p, p, out.data_ptr(), None, 1) == -1
+    assert lib.trimeg_gather(h, 16, p, p, p, None, None, 1) == -1
+    assert lib.trimeg_gather(h, 16, p, p, p, out.data_ptr(), None, 5) == -1
+    assert lib.trimeg_gather(h, -1, p, p, p, out.data_ptr(), None, 1) == -1
+    scratch = torch.empty(g.scratch_bytes(16), dtype=torch.uint8, device="cuda")
+    args = [p] * 7
+    assert lib.trimeg_markers_bind(h, 16, *args, 1, None, scratch.numel()) == -1
+    assert lib.trimeg_markers_bind(h, 16, None, *args[1:], 1, scratch.data_ptr(), scratch.numel()) == -1
+    assert lib.trimeg_markers_bind(h, 16, *args, 3, scratch.data_ptr(), scratch.numel()) == -1
+    assert lib.trimeg_markers_bind(h, 16, *args, 1, scratch.data_ptr(), 10) == -5           # scratch too small: OOM code
+    assert lib.trimeg_markers_get(h, None, None, None, None, None, None, 9) == -1
+    assert lib.trimeg_rhs(h, None, 1) == -1
+    assert lib.trimeg_push_stats(h, None) == -1
+    assert lib.trimeg_push_variant_used(h, None) == -1
+    assert b"" != lib.trimeg_last_error(h)
+    # still usable
+    mk = _dev(synth.make_markers(cfg, 64))
+    g.markers_bind(*[mk[k] for k in KEYS])
+    g.push_rk4(0.05, 1)
+    g.sync()

@@ -306,3 +306,29 @@ def test_lost_marker_status_and_zero_field_outside(cfg0_oracle):
         assert out[5][0] != 0
     d, outside = o.rhs(np.array([cfg.R0 + 1.5 * cfg.a]), np.array([0.0]), phi[:1], u[:1], w[:1], mu[:1], p[:1])
     assert outside[0] == 1 and np.isfinite(d).all() and d[4, 0] == 0.0
+    # unconditional form: markers that START outside (beyond the outer boundary; inside the hole of the annulus) are
+    # flagged by the very first stage, whatever happens afterwards, while a marker well inside is not; the flag is
+    # sticky (a status passed back in is kept, also for a marker that never leaves); and outside the mesh the motion
+    # is exactly the equilibrium motion, i.e. what the same oracle gives with both perturbed fields set to zero
+    Ro = np.array([cfg.R0 + 1.02 * cfg.a, cfg.R0 + 0.02 * cfg.a, cfg.R0 + 0.5 * cfg.a, cfg.R0 + 1.3 * cfg.a])
+    Zo, pho = np.zeros(4), np.full(4, 0.3)
+    uo, muo, wo, po = np.full(4, 0.4), np.full(4, 0.2), np.zeros(4), np.ones(4)
+    one = o.push_rk4(Ro, Zo, pho, uo, wo, muo, po, 0.05, 1)
+    assert list(one[5] != 0) == [True, True, False, True]
+    more = o.push_rk4(*one[:5], muo, po, 0.05, 3, status=one[5])
+    assert list(more[5] != 0) == [True, True, False, True]
+    kept = o.push_rk4(Ro[2:3], Zo[2:3], pho[2:3], uo[2:3], wo[2:3], muo[2:3], po[2:3], 0.05, 2, status=np.array([1], dtype=np.int32))
+    assert kept[5][0] != 0
+    from oracle import Oracle
+    z = Oracle()
+    z.equilibrium_set(**synth.equilibrium_args(cfg))
+    z.species_set(**synth.species_args(cfg))
+    z.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+    zero = np.zeros((cfg.n_planes, RZ.shape[0], 6))
+    z.fields_set(0, zero)
+    z.fields_set(1, zero)
+    far = o.push_rk4(Ro[3:], Zo[3:], pho[3:], uo[3:], wo[3:], muo[3:], po[3:], 0.05, 5)
+    ref = z.push_rk4(Ro[3:], Zo[3:], pho[3:], uo[3:], wo[3:], muo[3:], po[3:], 0.05, 5)
+    for q in range(5):
+        assert far[q][0] == ref[q][0]
+    assert far[4][0] == 0.0  # w stays 0: no perturbed field, no weight drive
