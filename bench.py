@@ -227,7 +227,7 @@ def main():
     ap.add_argument("--variant", type=int, default=0, help="0 two-phase warp-specialised push, 1 simple")
     ap.add_argument("--sort-every", type=int, default=SORT_EVERY, help="re-sort the marker store every n RK4 steps (inside the timed region)")
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--cpu-sample", type=int, default=400_000, help="markers of the oracle cpu_baseline leg (x 4 steps)")
+    ap.add_argument("--cpu-sample", type=int, default=4_000_000, help="markers of the oracle cpu_baseline leg (x 4 steps)")
     ap.add_argument("--ref-markers", type=int, default=200_000, help="markers per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parity", action="store_true", help="skip the sampled oracle check of the timed run")

@@ -624,3 +624,21 @@ int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]) {
 }
 
 }  // extern "C"
+
+#ifdef TRIMEG_WAITSTATS
+extern "C" int trimeg_debug_wait(unsigned long long out[16], int reset) {
+    if (cudaDeviceSynchronize() != cudaSuccess) return -4;
+    if (cudaMemcpyFromSymbol(out, trimeg::g_wait, sizeof(unsigned long long) * 16) != cudaSuccess) return -4;
+    if (reset) { unsigned long long z[16] = {}; cudaMemcpyToSymbol(trimeg::g_wait, z, sizeof z); }
+    return 0;
+}
+extern "C" int trimeg_debug_cnt(unsigned* out, int block) {
+    cudaDeviceSynchronize();
+    return cudaMemcpyFromSymbol(out, trimeg::g_cnt, sizeof(unsigned) * 4 * 32, sizeof(unsigned) * 4 * 32 * block) == cudaSuccess ? 0 : -4;
+}
+extern "C" int trimeg_debug_dbg(unsigned long long out[64]) {
+    cudaError_t e = cudaDeviceSynchronize();
+    if (cudaMemcpyFromSymbol(out, trimeg::g_dbg, sizeof(unsigned long long) * 64) != cudaSuccess) return -4;
+    return e == cudaSuccess ? 0 : -4;
+}
+#endif

@@ -338,10 +338,31 @@ TRIMEG_DI void equil_eval(const EquilP& e, T R, T Z, Equil<T>& o) {
 //   B*_par = B + kappa u b.curl b  (L61),  S = beta b + kappa u curl b with beta = B (b* = B*/B*_par, reading R7) or
 //   beta = B*_par (the literal expression printed at L53), so that in both cases b* = S / B*_par and every product with
 //   b* is formed with S and scaled by 1/B*_par once at the end.
+// The part of a right-hand-side evaluation that depends on the position only (not on the gathered fields): equilibrium
+// and the Eq.(8) profile terms.  Kept separate so that a kernel can issue these long dependent chains (rsqrt, rcp, two
+// exponentials) BEFORE the gather and let them overlap with the gather's loads and Horner chains.
 template <class T>
-TRIMEG_DI void rhs_eval(const EquilP& ep, const SpeciesP& sp, T R, T Z, T u, T w, T mu, T p, const FieldsG<T>& f, T d[5]) {
+struct RhsPre {
     Equil<T> e;
-    equil_eval(ep, R, Z, e);
+    T dlnT, dlnn, iT;     // d ln T / dr, d ln n / dr, 1 / T(r)
+};
+template <class T>
+TRIMEG_DI void rhs_pre(const EquilP& ep, const SpeciesP& sp, T R, T Z, RhsPre<T>& o) {
+    equil_eval(ep, R, Z, o.e);
+    const T dr = o.e.r - T(sp.r0);
+    const T thT = fma(T(-2.0), rcp_nr(exp_nr(dr * T(sp.two_inv_wT_a)) + T(1.0)), T(1.0));
+    const T thn = sp.same_w ? thT : fma(T(-2.0), rcp_nr(exp_nr(dr * T(sp.two_inv_wn_a)) + T(1.0)), T(1.0));
+    o.dlnT = T(-sp.kT_R0) * fma(-thT, thT, T(1.0));
+    o.dlnn = T(-sp.kn_R0) * fma(-thn, thn, T(1.0));
+    o.iT = exp_nr(T(sp.cT) * thT);                                                 // 1/T(r), Eq.(8)
+}
+// time derivatives of (R, Z, phi, u, w) at one phase-space point (gyro-average off, L320; dA^s = 0: p_par form).
+//   B*_par = B + kappa u b.curl b  (L61),  S = beta b + kappa u curl b with beta = B (b* = B*/B*_par, reading R7) or
+//   beta = B*_par (the literal expression printed at L53), so that in both cases b* = S / B*_par and every product with
+//   b* is formed with S and scaled by 1/B*_par once at the end.
+template <class T>
+TRIMEG_DI void rhs_post(const SpeciesP& sp, const RhsPre<T>& pre, T u, T w, T mu, T p, const FieldsG<T>& f, T d[5]) {
+    const Equil<T>& e = pre.e;
     const T ku = T(sp.kappa) * u, km = T(sp.kappa) * mu;
     const T kub = ku * e.iB;
     const T Bss = fma(kub * e.bp, e.J, e.B);                                       // L61
@@ -367,17 +388,18 @@ TRIMEG_DI void rhs_eval(const EquilP& ep, const SpeciesP& sp, T R, T Z, T u, T w
     const T hR = fma(e.bp, gZ, -(e.bZ * gp)), hZ = fma(e.bR, gp, -(e.bp * gR));    // (b x g)_R, (b x g)_Z
     const T qA = T(sp.qom) * f.A;
     const T eR = fma(-qA, SR, hR), eZ = fma(-qA, SZ, hZ);                          // Bss * delta Xdot
-    const T dr = e.r - T(sp.r0);
-    const T thT = fma(T(-2.0), rcp_nr(exp_nr(dr * T(sp.two_inv_wT_a)) + T(1.0)), T(1.0));
-    const T thn = sp.same_w ? thT : fma(T(-2.0), rcp_nr(exp_nr(dr * T(sp.two_inv_wn_a)) + T(1.0)), T(1.0));
-    const T dlnT = T(-sp.kT_R0) * fma(-thT, thT, T(1.0)), dlnn = T(-sp.kn_R0) * fma(-thn, thn, T(1.0));
-    const T iT = exp_nr(T(sp.cT) * thT);                                           // 1/T(r), Eq.(8)
     const T En = fma(T(0.5) * u, u, mu * e.B);
-    const T cr = fma(dlnT, fma(En, iT, T(-1.5)), dlnn);
-    const T muT = mu * iT;
+    const T cr = fma(pre.dlnT, fma(En, pre.iT, T(-1.5)), pre.dlnn);
+    const T muT = mu * pre.iT;
     const T glR = fma(cr, e.c, -(muT * e.gBR)), glZ = fma(cr, e.s, -(muT * e.gBZ));
     const T pw = sp.weight_mode ? (p - w) : p;
-    d[4] = -((pw * iBss) * fma(eR, glR, fma(eZ, glZ, Sqg * (u * iT))));
+    d[4] = -((pw * iBss) * fma(eR, glR, fma(eZ, glZ, Sqg * (u * pre.iT))));
+}
+template <class T>
+TRIMEG_DI void rhs_eval(const EquilP& ep, const SpeciesP& sp, T R, T Z, T u, T w, T mu, T p, const FieldsG<T>& f, T d[5]) {
+    RhsPre<T> pre;
+    rhs_pre(ep, sp, R, Z, pre);
+    rhs_post(sp, pre, u, w, mu, p, f, d);
 }
 
 }  // namespace trimeg

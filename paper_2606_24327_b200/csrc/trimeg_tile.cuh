@@ -24,11 +24,17 @@ template <int TP_, int SMAX_, int WK_, int NBUF_, int K_>
 struct TileCfg {
     static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD;
     // 16 warps: one light warp-group (stager, two publishers, one spare) and three compute warp-groups
-    static constexpr int NLIGHT = 4, NPUB = 2, NCOMP = 12;
+    #ifndef TRIMEG_NCOMP
+#define TRIMEG_NCOMP 12
+#endif
+#ifndef TRIMEG_REG_COMP
+#define TRIMEG_REG_COMP 152
+#endif
+    static constexpr int NLIGHT = 4, NPUB = 2, NCOMP = TRIMEG_NCOMP;
     static constexpr int NWARPS = NLIGHT + NCOMP, NTHREADS = 32 * NWARPS;
     // register hand-over (setmaxnreg): 16 warps launch with 128 registers; the light warps drop to 40, the compute warps
     // take 24 more each (12 x 24 <= 4 x 88)
-    static constexpr int REG_LIGHT = 40, REG_COMP = 152;
+    static constexpr int REG_LIGHT = 40, REG_COMP = TRIMEG_REG_COMP;
     static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
     static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
     static constexpr int CPS = TP * WK;              // cells per super-cell
@@ -36,45 +42,58 @@ struct TileCfg {
     static constexpr int NBUF = NBUF_;               // ring of staged blocks
     static constexpr int K = K_;                     // chunk slots: one per compute warp + look-ahead
     static_assert(K % NPUB == 0, "a chunk slot is always served by the same publisher warp (an odd K hung on the GPU)");
-    // slot GEOMETRY (96 B per slot) is staged for SGEOM slots, coefficients only for the first SMAX of them: the walk that
+    // slot GEOMETRY (64 B per slot) is staged for SGEOM slots, coefficients only for the first SMAX of them: the walk that
     // locates the next phase's first evaluation point needs no coefficients and stays in shared memory further out
     static constexpr int SGEOM = 32;
     static_assert(SMAX <= SGEOM, "one slot per lane of the stager");
     // shared memory carve-up (bytes): NBUF x { coefficients, slot geometry, slot triangles }, control, chunk slots
     static constexpr size_t COEF_BYTES = sizeof(double) * SMAX * SLOT_DOUBLES;
-    static constexpr size_t GEOM_BYTES = 96 * SGEOM;
+    static constexpr size_t GEOM_BYTES = 64 * SGEOM;
     static constexpr size_t BLOCK_BYTES = COEF_BYTES + GEOM_BYTES + 4 * SGEOM;
-    static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;                   // BlockCtrl (64 B) per ring entry
-    static constexpr size_t OFF_BAR = OFF_CTRL + 64 * NBUF;                  // per ring entry: full, seen (8 B each)
+    static constexpr size_t CTRL_BYTES = 320;                                // BlockCtrl per ring entry
+    static constexpr size_t OFF_CTRL = BLOCK_BYTES * NBUF;
+    static constexpr size_t OFF_BAR = OFF_CTRL + CTRL_BYTES * NBUF;          // per ring entry: full, seen (8 B each)
     static constexpr size_t OFF_DESC = OFF_BAR + 16 * NBUF;                  // per chunk slot: ChunkDesc (16 B)
     static constexpr size_t OFF_CBAR = OFF_DESC + 16 * K;                    // per chunk slot: full, empty (8 B each)
-    static constexpr size_t OFF_HEAD = OFF_CBAR + 16 * K;                    // ticket counter
-    static constexpr int CHUNK = 32;                                         // marker records per chunk slot (one per lane)
+    static constexpr size_t OFF_LTAB = OFF_CBAR + 16 * K;                    // per chunk slot: lane -> record row (32 B)
+    static constexpr size_t OFF_HEAD = OFF_LTAB + 32 * K;                    // ticket counter (16 B), then the prefetch mailbox
+    static constexpr int PFQ = 8;                                            // mailbox entries (begin, end) + sequence number
+    static constexpr size_t OFF_PFQ = OFF_HEAD + 16;
+    static constexpr int CHUNK = 32;                                         // lanes (<= marker records) per chunk slot
     static constexpr size_t WSTAGE = CHUNK * 128;
-    static constexpr size_t OFF_STAGE = (OFF_HEAD + 16 + 127) / 128 * 128;
+    static constexpr size_t OFF_STAGE = (OFF_PFQ + 8 * PFQ + 16 + 127) / 128 * 128;
     static constexpr size_t BYTES = OFF_STAGE + WSTAGE * K;
+    static_assert(BLOCK_BYTES % 16 == 0 && OFF_CTRL % 16 == 0, "TMA destinations and control blocks are 16-byte aligned");
     static_assert(BYTES <= 227 * 1024, "shared memory per CTA");
 };
-struct BlockCtrl {   // 64 B per ring entry
-    int sc, begin, end, patch, k0, ns;
+// Control block of one ring entry (one super-cell = TP triangles x WK toroidal intervals = 32 cells).
+// Lanes of a chunk are laid out over the cells PADDED TO EVEN sizes: an LDS.128 whose lane pairs (2i, 2i+1) read the same
+// address takes 2 shared-memory cycles, one with a pair split across two cells takes 4 (measured, profiles/r02b_lds.md), so
+// every cell starts on an even lane; an odd cell leaves one lane idle.
+struct __align__(16) BlockCtrl {
+    int sc, patch, k0, ns;
     int nchunks;     // chunks that will be cut from this entry
     int done;        // chunks finished (compute warps count up)
-    int pad[8];
+    int npad;        // lanes of the entry = sum of the padded cell sizes
+    int pad0;
+    double ox, oy;   // origin of the slot geometry's affine forms (a vertex of the patch)
+    int cell_off[33];   // offsets of the 32 cells in the cell-sorted store, and the end
+    int pad_incl[32];   // inclusive prefix sums of the padded cell sizes
 };
-struct ChunkDesc { int m0, end, b, pad; };   // m0 < 0: no more work
+static_assert(sizeof(BlockCtrl) <= 320, "BlockCtrl");
+struct ChunkDesc { int m0, nrec, b, ticket; };   // records m0 .. m0 + nrec - 1 of the destination (m0 < 0: no more work); ticket the slot was filled for
 
-// Geometry of one staged slot, 96 B.  The edge walk tests the three barycentrics in the form l = a R + b Z + c (two
-// dependent FMAs each; their rounding, ~1e-13, only matters within the walk's 1e-12 tolerance band, where either
-// neighbour is a correct answer); the coordinates handed to the polynomial evaluation are recomputed once, for the
-// triangle found, in the cancellation-free form a (R - v0x) + b (Z - v0y).
+// Geometry of one staged slot, 64 B: the barycentrics as affine forms of the position RELATIVE TO THE PATCH ORIGIN,
+//   xi = a11 dR + a12 dZ + c1,  eta = a21 dR + a22 dZ + c2,  (dR, dZ) = (R, Z) - (ox, oy),  1 - xi - eta the third.
+// With the origin a vertex of the patch, |c| is a few units and the forms carry no cancellation (the same numbers serve
+// the inside test of the edge walk and the polynomial evaluation); all three neighbours come with one load.
 struct __align__(16) SlotGeom {
-    double a11, a12, a21, a22;    // J^-1: xi = a11 (R - v0x) + a12 (Z - v0y), eta = a21 (..) + a22 (..)
-    double c1, c2;                // xi = a11 R + a12 Z + c1, eta = a21 R + a22 Z + c2
-    double l0a, l0b, l0c;         // 1 - xi - eta = l0a R + l0b Z + l0c
+    double a11, a12, a21, a22;    // J^-1
+    double c1, c2;
     short nbr[4];                 // slot across edge 0 (eta = 0), 1 (1 - xi - eta = 0), 2 (xi = 0): -1 not staged, -2 mesh boundary
-    double v0x, v0y;
+    int pad[2];
 };
-static_assert(sizeof(SlotGeom) == 96, "SlotGeom");
+static_assert(sizeof(SlotGeom) == 64, "SlotGeom");
 
 TRIMEG_DI unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 TRIMEG_DI void mbar_init(void* bar, int count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count)); }

@@ -199,3 +199,26 @@ def test_abi_null_pointers_and_bad_memspace():
     g.markers_bind(*[mk[k] for k in KEYS])
     g.push_rk4(0.05, 1)
     g.sync()
+
+
+def test_push_is_bitwise_reproducible():
+    """The phase kernel hands chunks of markers to whichever compute warp is free, so the order of execution differs from
+    run to run; the result must not (every marker's arithmetic is its own).  A race on a record, a chunk slot or a staged
+    coefficient block would show up here as a run-to-run difference (profiles/r02_sanitizer.md: compute-sanitizer is
+    closed on this pool, this test stands in for racecheck)."""
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, n_markers=300_007)
+    RZ, tri, o, g, m = _make(cfg)
+    d = _dev(m)
+    runs = []
+    for rep in range(3):
+        g.set_push_variant(0)
+        g.set_sort_interval(1 if rep < 2 else 3)
+        g.markers_bind(*[d[k] for k in KEYS])
+        g.push_rk4(0.05, 6)
+        runs.append(g.markers_get(host=True))
+    for k in ("R", "Z", "phi", "u", "w", "status"):
+        assert np.array_equal(runs[0][k], runs[1][k]), k
+    # a stale order changes which markers take the follow-up path (same formulas, other rounding): agreement to rounding only
+    for k in ("R", "Z", "phi", "u", "w"):
+        assert _rel(runs[2][k], runs[0][k], cfg.phi_period if k == "phi" else None) < 1e-12, k
+    assert np.array_equal(runs[0]["status"], runs[2]["status"])
