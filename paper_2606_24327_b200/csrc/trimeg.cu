@@ -625,16 +625,15 @@ int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]) {
 
 }  // extern "C"
 
-#ifdef TRIMEG_WAITSTATS
-extern "C" int trimeg_debug_wait(unsigned long long out[16], int reset) {
+#if defined(TRIMEG_WAITSTATS) || defined(TRIMEG_WATCHDOG)
+// tuning / debugging builds only (see trimeg_ws.cuh); not part of include/trimeg.h
+extern "C" int trimeg_debug_wait(unsigned long long out[160], int reset) {
     if (cudaDeviceSynchronize() != cudaSuccess) return -4;
-    if (cudaMemcpyFromSymbol(out, trimeg::g_wait, sizeof(unsigned long long) * 16) != cudaSuccess) return -4;
-    if (reset) { unsigned long long z[16] = {}; cudaMemcpyToSymbol(trimeg::g_wait, z, sizeof z); }
+    static unsigned long long h[160][160];
+    if (cudaMemcpyFromSymbol(h, trimeg::g_wait, sizeof h) != cudaSuccess) return -4;
+    for (int i = 0; i < 160; ++i) { out[i] = 0; for (int b = 0; b < 160; ++b) out[i] += h[b][i]; }
+    if (reset) { memset(h, 0, sizeof h); cudaMemcpyToSymbol(trimeg::g_wait, h, sizeof h); }
     return 0;
-}
-extern "C" int trimeg_debug_cnt(unsigned* out, int block) {
-    cudaDeviceSynchronize();
-    return cudaMemcpyFromSymbol(out, trimeg::g_cnt, sizeof(unsigned) * 4 * 32, sizeof(unsigned) * 4 * 32 * block) == cudaSuccess ? 0 : -4;
 }
 extern "C" int trimeg_debug_dbg(unsigned long long out[64]) {
     cudaError_t e = cudaDeviceSynchronize();

@@ -30,11 +30,14 @@ struct TileCfg {
 #ifndef TRIMEG_REG_COMP
 #define TRIMEG_REG_COMP 152
 #endif
-    static constexpr int NLIGHT = 4, NPUB = 2, NCOMP = TRIMEG_NCOMP;
+#ifndef TRIMEG_NPUB
+#define TRIMEG_NPUB 2
+#endif
+    static constexpr int NLIGHT = 4, NPUB = TRIMEG_NPUB, NCOMP = TRIMEG_NCOMP;   // light warps: stager, NPUB publishers, (prefetcher if NPUB = 2)
     static constexpr int NWARPS = NLIGHT + NCOMP, NTHREADS = 32 * NWARPS;
     // register hand-over (setmaxnreg): 16 warps launch with 128 registers; the light warps drop to 40, the compute warps
     // take 24 more each (12 x 24 <= 4 x 88)
-    static constexpr int REG_LIGHT = 40, REG_COMP = TRIMEG_REG_COMP;
+    static constexpr int REG_LIGHT = 56, REG_COMP = TRIMEG_REG_COMP;
     static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
     static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
     static constexpr int CPS = TP * WK;              // cells per super-cell

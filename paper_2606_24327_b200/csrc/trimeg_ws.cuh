@@ -18,13 +18,23 @@
 
 namespace trimeg {
 
-#ifdef TRIMEG_WAITSTATS   // tuning builds only: cycles spent waiting, by role
-__device__ unsigned long long g_wait[16];
+// Tuning / debugging builds only (never shipped): -DTRIMEG_WAITSTATS accumulates the cycles each role spends waiting
+// (compute warps binned by the chunk count of their ring entry), -DTRIMEG_WATCHDOG replaces every barrier wait by one that
+// gives up after ~1 s, records who waited on what (g_dbg) and lets the kernel end (this is how the slot/ticket aliasing
+// deadlock fixed in this file was found; profiles/r02_sanitizer.md).
+#if defined(TRIMEG_WAITSTATS) || defined(TRIMEG_WATCHDOG)
+__device__ unsigned long long g_wait[160][160];   // [block][counter]: per-block, so that the counters do not contend
 __device__ int g_abort;
-__device__ unsigned g_cnt[160][4][32];   // per block, per slot: published, consumed, released, last ticket published
-#define WS_CNT(k, s, v) do { if ((threadIdx.x & 31) == 0) { if ((k) == 3) g_cnt[blockIdx.x][3][s] = (v); else atomicAdd(&g_cnt[blockIdx.x][k][s], 1u); } } while (0)
 __device__ unsigned long long g_dbg[64];
-// watchdog wait: gives up after ~1 s (or when another warp has given up), records who waited on what, and raises g_abort
+#endif
+#ifdef TRIMEG_WAITSTATS
+#define WS_T0() const long long ws_t0__ = clock64()
+#define WS_ADD(i) do { if ((threadIdx.x & 31) == 0) atomicAdd(&g_wait[blockIdx.x][i], (unsigned long long)(clock64() - ws_t0__)); } while (0)
+#else
+#define WS_T0() do {} while (0)
+#define WS_ADD(i) do {} while (0)
+#endif
+#ifdef TRIMEG_WATCHDOG
 TRIMEG_DI bool mbar_wait_wd(void* bar, unsigned parity, int code, int aux) {
     const long long t0 = clock64();
     bool recorded = false;
@@ -49,15 +59,10 @@ TRIMEG_DI bool mbar_wait_wd(void* bar, unsigned parity, int code, int aux) {
 #define MBW(bar, parity, code, aux) do { if (!mbar_wait_wd(bar, parity, code, aux)) return; } while (0)
 #define WS_ABORTED() (*(volatile int*)&g_abort)
 TRIMEG_DI bool mbar_wait_any(void* bar, unsigned parity, int code, int aux) { return mbar_wait_wd(bar, parity, code, aux); }
-#define WS_T0() const long long ws_t0__ = clock64()
-#define WS_ADD(i) do { if ((threadIdx.x & 31) == 0) atomicAdd(&g_wait[i], (unsigned long long)(clock64() - ws_t0__)); } while (0)
 #else
 #define MBW(bar, parity, code, aux) mbar_wait(bar, parity)
-#define WS_CNT(k, s, v) do {} while (0)
 #define WS_ABORTED() false
 TRIMEG_DI bool mbar_wait_any(void* bar, unsigned parity, int, int) { mbar_wait(bar, parity); return true; }
-#define WS_T0() do {} while (0)
-#define WS_ADD(i) do {} while (0)
 #endif
 
 // stager, part 1: take the next non-empty super-cell off the work list and pull everything its ring entry needs out of
@@ -187,7 +192,7 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
     auto ctl_of = [&](int b) { return reinterpret_cast<BlockCtrl*>(smem + C::OFF_CTRL + C::CTRL_BYTES * b); };
     if (tid == 0) {
         for (int b = 0; b < C::NBUF; ++b) { mbar_init(blk_bar + 2 * b, 1); mbar_init(blk_bar + 2 * b + 1, C::NPUB); }
-        for (int s = 0; s < C::K; ++s) { mbar_init(chunk_bar + 2 * s, 32); mbar_init(chunk_bar + 2 * s + 1, 1); }
+        for (int s = 0; s < C::K; ++s) { mbar_init(chunk_bar + 2 * s, 64); mbar_init(chunk_bar + 2 * s + 1, 1); }   // full: per lane one plain + one copy-completion arrival
         *cons_head = 0;
         *pf_seq = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -202,6 +207,9 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
             int posted = 0;
             auto post = [&](bool have_) {   // tell the prefetcher which records come next (begin = -1: no more work)
                 const int begin = __shfl_sync(FULL, w.off, 0);
+                if (C::NPUB + 1 >= C::NLIGHT) {   // no prefetcher warp
+                    return;
+                }
                 if (lane == 0) {
                     pfq[2 * (posted % C::PFQ)] = have_ ? begin : -1; pfq[2 * (posted % C::PFQ) + 1] = w.off_end;
                     __threadfence_block();
@@ -220,7 +228,7 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                     BlockCtrl* ctl = ctl_of(b);
                     if (lane == 0) {
                         const int need = ctl->nchunks;
-#ifdef TRIMEG_WAITSTATS
+#ifdef TRIMEG_WATCHDOG
                         const long long t0 = clock64();
                         while (*reinterpret_cast<volatile int*>(&ctl->done) < need) {
                             __nanosleep(64);
@@ -297,18 +305,28 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                     if (perm && lane < nrec) pr = perm[pr];
                     return m_first;
                 };
+                // software pipeline of depth 3: the permutation entries of a chunk are loaded (global memory: several microseconds
+                // under load) three of this publisher's chunks before its records are copied
                 unsigned t = t0 + (pid + C::NPUB - t0 % C::NPUB) % C::NPUB;
-                int m_next = 0, nrec_next = 0, rowl_next = 0, pr_next = 0;
-                if (t < t0 + nch) m_next = layout(t, nrec_next, rowl_next, pr_next);
+                int mq0 = 0, nq0 = 0, rq0 = 0, pq0 = 0, mq1 = 0, nq1 = 0, rq1 = 0, pq1 = 0, mq2 = 0, nq2 = 0, rq2 = 0, pq2 = 0;
+                if (t < t0 + nch) mq0 = layout(t, nq0, rq0, pq0);
+                if (t + C::NPUB < t0 + nch) mq1 = layout(t + C::NPUB, nq1, rq1, pq1);
+                if (t + 2 * C::NPUB < t0 + nch) mq2 = layout(t + 2 * C::NPUB, nq2, rq2, pq2);
                 for (; t < t0 + nch; t += C::NPUB) {
-                    const int m_first = m_next, nrec = nrec_next, rowl = rowl_next, pr = pr_next;
-                    if (t + C::NPUB < t0 + nch) m_next = layout(t + C::NPUB, nrec_next, rowl_next, pr_next);
+                    const int m_first = mq0, nrec = nq0, rowl = rq0, pr = pq0;
+                    mq0 = mq1; nq0 = nq1; rq0 = rq1; pq0 = pq1;
+                    mq1 = mq2; nq1 = nq2; rq1 = rq2; pq1 = pq2;
+                    { WS_T0(); if (t + 3 * C::NPUB < t0 + nch) mq2 = layout(t + 3 * C::NPUB, nq2, rq2, pq2); WS_ADD(8); }
                     const int s = slot_acquire(t);
                     if (s < 0) return;
                     if (lane == 0) { desc[s].m0 = m_first; desc[s].nrec = nrec; desc[s].b = b; desc[s].ticket = (int)t; }
                     ltab[s * 32 + lane] = (unsigned char)rowl;
-                    __threadfence_block();
+                    // descriptor and lane table are published by a plain (release) arrival of every lane: no fence here - a
+                    // membar would also wait for the copies still in flight and for the next chunk's permutation loads, i.e.
+                    // for a global-memory latency per chunk (that made the publishers the bottleneck: profiles/r02_summary.md)
                     __syncwarp();
+                    mbar_arrive(chunk_bar + 2 * s);
+                    WS_T0();
                     const unsigned ib = smem_u32(smem + C::OFF_STAGE + (size_t)s * C::WSTAGE);
                     const int ch = lane & 7, q = lane >> 3;
 #pragma unroll
@@ -324,7 +342,7 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                         }
                     }
                     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(chunk_bar + 2 * s)) : "memory");
-                    WS_CNT(0, s, 0); WS_CNT(3, s, t);
+                    WS_ADD(9);
                 }
             }
             // one end-of-work ticket per compute warp
@@ -332,11 +350,12 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                 if (ticket % C::NPUB != pid) continue;
                 const int s = slot_acquire(ticket);
                 if (s < 0) return;
-                if (lane == 0) { desc[s].m0 = -1; desc[s].ticket = (int)ticket; __threadfence_block(); }
+                if (lane == 0) { desc[s].m0 = -1; desc[s].ticket = (int)ticket; }
                 __syncwarp();
                 mbar_arrive(chunk_bar + 2 * s);
+                mbar_arrive(chunk_bar + 2 * s);
             }
-        } else {
+        } else if (wid < C::NLIGHT) {
             // ------------------------------------------------------------------ prefetcher (a hint only: nothing waits for it)
             for (int n = 0;; ++n) {
                 while (*pf_seq <= n) { __nanosleep(200); if (WS_ABORTED()) return; }
@@ -365,6 +384,7 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
             const unsigned s = t % C::K, gen = t / C::K;
 #ifdef TRIMEG_WAITSTATS
             const long long ws_it0 = clock64();
+            long long ws_wait = 0;
 #endif
             // A compute warp holds up to two tickets (the one it works on and the next), so more tickets can be outstanding
             // than there are chunk slots: a warp may reach its wait while the slot's PREVIOUS generation has not been published
@@ -375,9 +395,12 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                   if (*reinterpret_cast<volatile int*>(&desc[s].ticket) == (int)t) break;
                   __nanosleep(100);
               }
-              WS_ADD(4); }
+              WS_ADD(4);
+#ifdef TRIMEG_WAITSTATS
+              ws_wait = clock64() - ws_t0__;
+#endif
+            }
             const int m0 = desc[s].m0, nrec = desc[s].nrec, b = desc[s].b;
-            WS_CNT(1, s, 0);
             if (m0 < 0) break;
             const int rowi = ltab[s * 32 + lane];
             const bool valid = rowi != 0xff;
@@ -414,6 +437,10 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                     }
                 }
                 auto eval = [&](const double y[5], double d[5]) {
+#ifdef TRIMEG_NOEVAL   // tuning builds only: the record pipeline without the arithmetic
+                    d[0] = d[1] = d[2] = d[3] = d[4] = 0.0;
+                    return true;
+#endif
                     double xi, eta, jj[4], sf;
                     const int sl = slot_walk(sgeom, slot, y[0] - ox, y[1] - oy, xi, eta, jj);
                     const int k = interval_fast(tb.tor, y[2], sf);
@@ -518,11 +545,14 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                 atomicAdd(&ctl->done, 1);            // one more chunk of this ring entry done
                 bulk_wait_read0();                   // the copy has read the slot:
                 mbar_arrive(chunk_bar + 2 * s + 1);  // it may be refilled
-                WS_CNT(2, s, 0);
 #ifdef TRIMEG_WAITSTATS
-                atomicAdd(&g_wait[6], (unsigned long long)(clock64() - ws_tail0));
-                atomicAdd(&g_wait[5], (unsigned long long)(clock64() - ws_it0));
-                atomicAdd(&g_wait[7], 1ull);
+                atomicAdd(&g_wait[blockIdx.x][6], (unsigned long long)(clock64() - ws_tail0));
+                atomicAdd(&g_wait[blockIdx.x][5], (unsigned long long)(clock64() - ws_it0));
+                atomicAdd(&g_wait[blockIdx.x][7], 1ull);
+                const int bin = min(ctl->nchunks, 47);
+                atomicAdd(&g_wait[blockIdx.x][16 + bin], (unsigned long long)ws_wait);          // cycles waiting for the chunk
+                atomicAdd(&g_wait[blockIdx.x][64 + bin], (unsigned long long)(clock64() - ws_it0));
+                atomicAdd(&g_wait[blockIdx.x][112 + bin], 1ull);
 #endif
             }
         }
