@@ -156,7 +156,7 @@ def run_reference(args, cfg, rank, world):
     el = time.perf_counter() - t0
     val = n_sample * args.steps / el
     sample = f"{n_sample} markers of {cfg.name} (of {cfg.n_markers}) per step"
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": workload_config(cfg, n_sample, args),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle", "sample": sample},
@@ -164,9 +164,17 @@ def run_reference(args, cfg, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def _build_defs():
+    try:
+        from paper_2606_24327_b200.binding import build_info
+        return build_info()
+    except Exception:
+        return None
+
+
 def workload_config(cfg, n, args):
     return {"workload": f"{cfg.name}: {2 * cfg.nr * cfg.ntheta} triangles x {cfg.n_planes} planes, {n} markers/GPU, EM={cfg.em}, dt={cfg.dt}, RK4, sort every {args.sort_every} steps",
-            "markers_per_gpu": n, "triangles": 2 * cfg.nr * cfg.ntheta, "planes": cfg.n_planes, "dt": cfg.dt, "push_variant": args.variant, "sort_every": args.sort_every,
+            "build_defs": _build_defs(), "markers_per_gpu": n, "triangles": 2 * cfg.nr * cfg.ntheta, "planes": cfg.n_planes, "dt": cfg.dt, "push_variant": args.variant, "sort_every": args.sort_every,
             "l2": "inputs_exceed_l2" if n * 104 > 126e6 else "l2_flushed_between_steps"}
 
 
@@ -239,8 +247,19 @@ def main():
     cfg = synth.CONFIGS[args.config]
     if args.dt is not None:
         cfg = dataclasses.replace(cfg, dt=args.dt)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # no launcher: start the N ranks ourselves (one process per GPU, rendezvous on 127.0.0.1), same command line
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                                  "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != max(1, args.gpus):
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch one rank per GPU", file=sys.stderr)
+        sys.exit(2)
     if args.impl == "reference":
         run_reference(args, cfg, rank, world)
         return
@@ -260,7 +279,29 @@ def main():
     start, _ = shard.marker_slice(n, rank, world)
 
     g = Trimeg(local)
-    setup_case(cfg, g)
+    fields_bcast = None
+    if world > 1:
+        # the one collective of the path: every rank loads the mesh, rank 0 alone turns the nodal DOFs into the
+        # coefficient table, which is broadcast over NCCL (NCCL_DEBUG=INFO shows the transport: NVLink / NVLS)
+        RZ, tri = synth.make_mesh(cfg)
+        g.equilibrium_set(**synth.equilibrium_args(cfg))
+        g.species_set(**synth.species_args(cfg))
+        g.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+        if rank == 0:
+            dphi, dap = synth.make_fields(cfg, RZ)
+            g.fields_set(0, dphi)
+            g.fields_set(1, dap)
+        torch.cuda.synchronize()
+        dist.barrier()
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b0.record()
+        moved = shard.broadcast_fields(g, dist, src=0)
+        b1.record()
+        torch.cuda.synchronize()
+        bsec = shard.reduce_max_seconds(b0.elapsed_time(b1) * 1e-3, dist)
+        fields_bcast = {"bytes": moved, "ms": 1e3 * bsec, "GBps": moved / bsec / 1e9, "what": "export + dist.broadcast (NCCL) + import of the coefficient table"}
+    else:
+        setup_case(cfg, g)
     host, views = make_inputs(cfg, n, start, pinned=True)
     dev = {k: v.cuda(non_blocking=True) for k, v in host.items()}
     torch.cuda.synchronize()
@@ -377,7 +418,7 @@ def main():
                              "whole_step_frac": step_achieved / FP64_PEAK_TFLOPS,
                              "hbm_algorithmic_GBps": ALGO_BYTES_PER_LAUNCH * n / kern_s / 1e9},
                 "step_breakdown_ms": {"sort": sort_ms, "push": 1e3 * kern_s * launches_per_step, "finish": finish_ms},
-                "slow_path_evals": slow, "retired_markers": retired, "parity": parity}
+                "slow_path_evals": slow, "retired_markers": retired, "parity": parity, "fields_bcast": fields_bcast}
         if not args.no_cpu_baseline:
             cpu_n = min(n, args.cpu_sample)
             v, cores, secs = time_oracle(cfg, cpu_n, 4, oracle=oracle_obj)

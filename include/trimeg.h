@@ -95,6 +95,16 @@ int trimeg_fields_set(trimeg_ctx* ctx, int which, const double* dof, int memspac
 int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi, double* out,
                   int32_t* tri_out, int memspace);
 
+/* The per-triangle coefficient table that trimeg_fields_set builds (both fields), as one opaque block: its size in bytes
+ * (0 without a mesh), a copy of it into / out of caller-owned DEVICE memory (enqueued on the context's stream).  For the one
+ * collective of a multi-GPU run (mesh and fields replicated on every rank): one rank runs
+ * trimeg_fields_set, exports, the block is broadcast (NCCL), the other ranks import.  The layout is private to this build
+ * of the library and to the mesh it was loaded with (same mesh_load arguments on every rank).
+ * Errors: BAD_ARG (null, wrong size), BAD_STATE (no mesh), CUDA. */
+size_t trimeg_fields_bytes(const trimeg_ctx* ctx);
+int trimeg_fields_export(trimeg_ctx* ctx, void* dst_device, size_t bytes);
+int trimeg_fields_import(trimeg_ctx* ctx, const void* src_device, size_t bytes);
+
 /* Bytes of DEVICE scratch trimeg_markers_bind needs for n markers (0 on error): 268 bytes per marker (two buffers of
  * 128-byte records for the re-sorting phases + sort key, permutation and follow-up list, 4 bytes each): 26.8 GB at 1e8
  * markers.  This is twice the structure-of-arrays budget of SURVEY.md 8(a) (a1); DESIGN.md section 5 says why. */
@@ -148,6 +158,8 @@ int trimeg_push_variant_used(trimeg_ctx* ctx, int32_t* out);
 /* Diagnostics used by the benchmark: achieved FP64 FMA throughput of this device in TFLOP/s
  * (a register-only DFMA loop; the roofline's measured "alu" peak). */
 int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops);
+/* The -D options this library was built with beyond the defaults ("" for the shipped configuration). */
+const char* trimeg_build_info(void);
 /* Counters of the last trimeg_push_rk4 call: [0] kernel launches, [1] right-hand-side evaluations that took the
  * slow (out-of-block) path in the follow-up kernel, [2] marker-phases that left their staged block (summed over
  * phases and steps), [3] permutations built. */

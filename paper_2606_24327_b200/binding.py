@@ -21,6 +21,7 @@ EXPORTS = [
     "trimeg_species_set", "trimeg_mesh_load", "trimeg_fields_set", "trimeg_gather", "trimeg_scratch_bytes",
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
     "trimeg_rhs", "trimeg_set_push_variant", "trimeg_push_variant_used", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
+    "trimeg_fields_bytes", "trimeg_fields_export", "trimeg_fields_import", "trimeg_build_info",
 ]
 
 
@@ -66,6 +67,12 @@ def load_library():
     lib.trimeg_mesh_load.argtypes = [vp, i64, vp, i64, vp, i32, dbl]
     lib.trimeg_fields_set.argtypes = [vp, C.c_int, vp, C.c_int]
     lib.trimeg_gather.argtypes = [vp, i64, vp, vp, vp, vp, vp, C.c_int]
+    lib.trimeg_build_info.argtypes = []
+    lib.trimeg_build_info.restype = C.c_char_p
+    lib.trimeg_fields_bytes.argtypes = [vp]
+    lib.trimeg_fields_bytes.restype = C.c_size_t
+    lib.trimeg_fields_export.argtypes = [vp, vp, C.c_size_t]
+    lib.trimeg_fields_import.argtypes = [vp, vp, C.c_size_t]
     lib.trimeg_scratch_bytes.argtypes = [vp, i64]
     lib.trimeg_scratch_bytes.restype = C.c_size_t
     lib.trimeg_markers_bind.argtypes = [vp, i64] + [vp] * 7 + [C.c_int, vp, C.c_size_t]
@@ -92,6 +99,11 @@ def _ptr(x):
         return x.ctypes.data, HOST
     assert x.is_contiguous()
     return x.data_ptr(), (DEVICE if x.is_cuda else HOST)
+
+
+def build_info() -> str:
+    """-D options of a tuning build ("" for the shipped configuration)."""
+    return load_library().trimeg_build_info().decode()
 
 
 class Trimeg:
@@ -156,6 +168,26 @@ class Trimeg:
             assert tuple(dof.shape) == (self.n_planes, self.n_nodes, 6), tuple(dof.shape)
         p, ms = _ptr(dof)
         self._ck(self._lib.trimeg_fields_set(self._h, int(which), p, ms), "trimeg_fields_set")
+
+    @staticmethod
+    def build_info():
+        return build_info()
+
+    def fields_bytes(self):
+        return int(self._lib.trimeg_fields_bytes(self._h))
+
+    def fields_export(self, out=None):
+        """-> uint8 CUDA tensor holding the coefficient table (opaque; for a broadcast to other ranks)."""
+        n = self.fields_bytes()
+        if out is None:
+            out = self._torch.empty(n, dtype=self._torch.uint8, device=self.device)
+        assert out.is_cuda and out.is_contiguous() and out.numel() * out.element_size() == n
+        self._ck(self._lib.trimeg_fields_export(self._h, out.data_ptr(), n), "trimeg_fields_export")
+        return out
+
+    def fields_import(self, buf):
+        assert buf.is_cuda and buf.is_contiguous()
+        self._ck(self._lib.trimeg_fields_import(self._h, buf.data_ptr(), buf.numel() * buf.element_size()), "trimeg_fields_import")
 
     # ---- gather
     def gather(self, R, Z, phi, out=None, tri_out=None, want_tri=True):

@@ -303,6 +303,32 @@ int trimeg_fields_set(trimeg_ctx* ctx, int which, const double* dof, int memspac
     return TRIMEG_OK;
 }
 
+size_t trimeg_fields_bytes(const trimeg_ctx* ctx) {
+    if (!ctx || !ctx->have_mesh) return 0;
+    return (size_t)ctx->T * (size_t)ctx->NPP * PLANE_STRIDE * sizeof(double);
+}
+
+// the coefficient table as one opaque block of DEVICE memory: lets N ranks run fields_set on one of them and hand the result
+// to the others with one collective; the layout is private to this library version
+int trimeg_fields_export(trimeg_ctx* ctx, void* dst_device, size_t bytes) {
+    if (!ctx || !dst_device) return fail(ctx, TRIMEG_ERR_BAD_ARG, "fields_export: null argument");
+    if (!ctx->have_mesh) return fail(ctx, TRIMEG_ERR_BAD_STATE, "fields_export: call trimeg_mesh_load first");
+    if (bytes != trimeg_fields_bytes(ctx)) return fail(ctx, TRIMEG_ERR_BAD_ARG, "fields_export: need exactly %zu bytes", trimeg_fields_bytes(ctx));
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaMemcpyAsync(dst_device, ctx->d_coef, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    return TRIMEG_OK;
+}
+
+int trimeg_fields_import(trimeg_ctx* ctx, const void* src_device, size_t bytes) {
+    if (!ctx || !src_device) return fail(ctx, TRIMEG_ERR_BAD_ARG, "fields_import: null argument");
+    if (!ctx->have_mesh) return fail(ctx, TRIMEG_ERR_BAD_STATE, "fields_import: call trimeg_mesh_load first");
+    if (bytes != trimeg_fields_bytes(ctx)) return fail(ctx, TRIMEG_ERR_BAD_ARG, "fields_import: need exactly %zu bytes", trimeg_fields_bytes(ctx));
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaMemcpyAsync(ctx->d_coef, src_device, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    invalidate_step_state(ctx);   // the cached k1 was evaluated with the old fields
+    return TRIMEG_OK;
+}
+
 int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi, double* out, int32_t* tri_out, int memspace) {
     if (!ctx || n < 0 || (n > 0 && (!R || !Z || !phi || !out)) || (memspace != TRIMEG_HOST && memspace != TRIMEG_DEVICE))
         return fail(ctx, TRIMEG_ERR_BAD_ARG, "gather: bad argument");
@@ -535,6 +561,11 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps) {
     }
     return TRIMEG_OK;
 }
+
+#ifndef TRIMEG_BUILD_DEFS
+#define TRIMEG_BUILD_DEFS ""
+#endif
+const char* trimeg_build_info(void) { return TRIMEG_BUILD_DEFS; }
 
 int trimeg_push_variant_used(trimeg_ctx* ctx, int32_t* out) {
     if (!ctx || !out) return fail(ctx, TRIMEG_ERR_BAD_ARG, "push_variant_used: null argument");

@@ -4,10 +4,8 @@
 // Eq.(7), Eq.(8) L314.  Formulation notes (what differs from a literal transcription) are in DESIGN.md
 // section 6 "Kernel arithmetic".
 //
-// Every routine is a template over the scalar type T: `double` (one marker per thread: gather, rhs, follow-up and
-// simple-push kernels) or `D2` (two markers per lane, the phase kernel: the two markers of a lane sit in the same
-// cell, so one shared-memory coefficient load feeds both Horner chains and the FP64 pipe sees two independent
-// dependency chains per warp).
+// The routines are templates over the scalar type T (double everywhere in this build; round 2 also tried a two-markers-
+// per-lane type with shared coefficient loads).
 #pragma once
 #include <cstdint>
 
@@ -23,18 +21,6 @@ constexpr double INSIDE_TOL = -1e-12;
 
 #define TRIMEG_DI __device__ __forceinline__
 
-// ---- two markers per lane ---------------------------------------------------------------------------
-struct D2 {
-    double a, b;
-    TRIMEG_DI D2() {}
-    TRIMEG_DI D2(double x) : a(x), b(x) {}
-    TRIMEG_DI D2(double x, double y) : a(x), b(y) {}
-};
-TRIMEG_DI D2 operator+(D2 x, D2 y) { return D2(x.a + y.a, x.b + y.b); }
-TRIMEG_DI D2 operator-(D2 x, D2 y) { return D2(x.a - y.a, x.b - y.b); }
-TRIMEG_DI D2 operator*(D2 x, D2 y) { return D2(x.a * y.a, x.b * y.b); }
-TRIMEG_DI D2 operator-(D2 x) { return D2(-x.a, -x.b); }
-TRIMEG_DI D2 fma(D2 x, D2 y, D2 z) { return D2(::fma(x.a, y.a, z.a), ::fma(x.b, y.b, z.b)); }
 using ::fma;
 
 struct EquilP {
@@ -102,9 +88,6 @@ TRIMEG_DI double exp_nr(double x) {
     for (int k = 12; k >= 0; --k) p = fma(p, r, c_expk[k]);
     return p * __hiloint2double((n + 1023) << 20, 0);
 }
-TRIMEG_DI D2 rcp_nr(D2 x) { return D2(rcp_nr(x.a), rcp_nr(x.b)); }
-TRIMEG_DI D2 rsqrt_nr(D2 x) { return D2(rsqrt_nr(x.a), rsqrt_nr(x.b)); }
-TRIMEG_DI D2 exp_nr(D2 x) { return D2(exp_nr(x.a), exp_nr(x.b)); }
 
 // ---- toroidal uniform periodic cubic B-spline (L35) -------------------------------------------------
 // interval index k in [0, P) and fraction s in [0, 1] of phi (any real)
@@ -144,8 +127,7 @@ TRIMEG_DI int bspline_weights(const TorP& tp, double phi, double w[4], double dw
 // ---- reduced quintic in reference coordinates --------------------------------------------------------
 // Coefficients j-major: a_j(xi) = sum_{i<=5-j} c[off_j + i] xi^i, p = sum_j eta^j a_j(xi).
 // Two fields interleaved: c[2*idx + f].  38 FMA per field: value, d/dxi, d/deta.
-// ld(idx, c0, c1) fetches coefficient idx of field 0 and 1 as doubles; the Horner state is T, so with T = D2 one fetch
-// serves both markers of the lane.
+// ld(idx, c0, c1) fetches coefficient idx of field 0 and 1 as doubles.
 template <int N, class T, class Ld>
 TRIMEG_DI void horner2(Ld ld, int off, T x, T& v0, T& d0, T& v1, T& d1) {
     double c0, c1;
@@ -198,28 +180,6 @@ TRIMEG_DI void gather_cell(LdPlane ldp, T xi, T eta, const T w[4], const T dw[4]
         quintic_pair_accum<WITH_P>(ld, xi, eta, w[j], dw[j], acc);
     }
 }
-// The same with the plane loop ROLLED (one copy of the 168-FMA plane body: the phase kernel's hot loop has to fit the
-// 32 KB instruction cache) and the B-spline weights formed inside the loop from their polynomials in s,
-//   w_j(s) = sum_i c_bw[j][i] s^i,   d w_j / d s = sum_i c_bd[j][i] s^i   (j = plane k-1+j of interval k, L35),
-// whose coefficients sit in constant memory and are indexed by the (warp-uniform) loop counter.  The phi-derivative sums
-// acc[3], acc[7] are scaled by 1/dphi at the end.  base = shared-space byte address of the cell's first plane.
-__constant__ double c_bw[4][4] = {{1.0 / 6, -0.5, 0.5, -1.0 / 6}, {2.0 / 3, 0.0, -1.0, 0.5}, {1.0 / 6, 0.5, 0.5, -0.5}, {0.0, 0.0, 0.0, 1.0 / 6}};
-__constant__ double c_bd[4][3] = {{-0.5, 1.0, -0.5}, {0.0, -2.0, 1.5}, {0.5, 1.0, -1.5}, {0.0, 0.0, 0.5}};
-template <bool WITH_P, class T, class LdBase>
-TRIMEG_DI void gather_cell_rolled(unsigned base, T xi, T eta, T s, double inv_dphi, T acc[8]) {
-#pragma unroll
-    for (int q = 0; q < 8; ++q) acc[q] = T(0.0);
-#pragma unroll 1
-    for (int j = 0; j < 4; ++j) {
-        const T w = fma(fma(fma(T(c_bw[j][3]), s, T(c_bw[j][2])), s, T(c_bw[j][1])), s, T(c_bw[j][0]));
-        const T dw = fma(fma(T(c_bd[j][2]), s, T(c_bd[j][1])), s, T(c_bd[j][0]));
-        LdBase ld{base + (unsigned)(j * PLANE_STRIDE * sizeof(double))};
-        quintic_pair_accum<WITH_P>(ld, xi, eta, w, dw, acc);
-    }
-    acc[3] = acc[3] * T(inv_dphi);
-    acc[7] = acc[7] * T(inv_dphi);
-}
-
 // reference gradient -> physical gradient (grad_phys = J^-T grad_ref)
 TRIMEG_DI void to_fields(const TriGeom& g, const double acc[8], Fields& f) {
     f.P = acc[0]; f.PR = fma(g.a11, acc[1], g.a21 * acc[2]); f.PZ = fma(g.a12, acc[1], g.a22 * acc[2]); f.Pp = acc[3];

@@ -26,3 +26,15 @@ def reduce_max_seconds(seconds: float, dist=None) -> float:
     t = torch.tensor([seconds], dtype=torch.float64, device=dev)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def broadcast_fields(backend, dist, src: int = 0):
+    """The one collective of a multi-rank run: rank `src` has run fields_set; its coefficient table is
+    exported into a byte buffer, broadcast (NCCL over NVLink for CUDA buffers) and imported by every other rank.
+    `backend` needs fields_export() -> buffer and fields_import(buffer); returns the bytes moved."""
+    rank = dist.get_rank()
+    buf = backend.fields_export()
+    dist.broadcast(buf, src=src)
+    if rank != src:
+        backend.fields_import(buf)
+    return int(buf.numel() * buf.element_size())

@@ -132,6 +132,17 @@ assert secs == float(world), secs
 tot = torch.tensor([b - a], dtype=torch.int64)
 dist.all_reduce(tot)
 assert int(tot) == n * world
+# the one collective of the path (SURVEY 8(e)): rank 0's field table reaches every rank through shard.broadcast_fields
+class FakeBackend:
+    def __init__(self, rank):
+        self.table = (torch.arange(1000, dtype=torch.float64) * 0.5 if rank == 0 else torch.zeros(1000, dtype=torch.float64))
+    def fields_export(self):
+        return self.table.clone().view(torch.uint8)
+    def fields_import(self, buf):
+        self.table = buf.view(torch.float64).clone()
+fb = FakeBackend(rank)
+moved = shard.broadcast_fields(fb, dist, src=0)
+assert moved == 8000 and torch.equal(fb.table, torch.arange(1000, dtype=torch.float64) * 0.5)
 if rank == 0:
     print("RATE", shard.job_rate(n, world, secs))
 dist.barrier()
@@ -150,3 +161,18 @@ def test_two_rank_gloo_sharding_and_timing(tmp_path):
     r = subprocess.run(cmd, capture_output=True, text=True, timeout=300)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "RATE 5000.0" in r.stdout
+
+
+def test_bench_gpus_2_spawns_two_ranks_and_reports_them():
+    """`python bench.py --gpus 2` without a launcher must start its own two ranks (re-exec under torch.distributed.run on
+    127.0.0.1) and print ONE line with n_gpus = 2; checked here on the reference arm (the oracle; needs no GPU)."""
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference", "--config", "0", "--steps", "1", "--warmup", "0",
+           "--ref-markers", "500"]
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode == 0, r.stdout + r.stderr
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    import json
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["cpu_baseline"]["kind"] == "oracle"
