@@ -178,12 +178,15 @@ def workload_config(cfg, n, args):
             "l2": "inputs_exceed_l2" if n * 104 > 126e6 else "l2_flushed_between_steps"}
 
 
-def run_gather(args, cfg):
-    """BASELINE configs[4]: one field evaluation per point, random order and then the same points sorted by cell.
-    Prints one JSON line ("mode": "gather"); not the headline metric (that is the push)."""
+def run_gather(args, cfg, n=None, steps=None, warmup=None):
+    """BASELINE configs[4]: one field evaluation per point, points in random order and the same points sorted by cell, through
+    trimeg_gather's staged path (the library bins the points itself, TMA-staged coefficient blocks) and through the direct
+    one-thread-per-point kernel.  Returns the record ("mode": "gather"); not the headline metric (that is the push)."""
     import torch
     from paper_2606_24327_b200.binding import Trimeg
-    n = args.markers if args.markers is not None else cfg.n_markers
+    n = n if n is not None else (args.markers if args.markers is not None else cfg.n_markers)
+    steps = steps or args.steps
+    warmup = args.warmup if warmup is None else warmup
     g = Trimeg(0)
     setup_case(cfg, g)
     host, views = make_inputs(cfg, n, 0, pinned=False)
@@ -191,36 +194,52 @@ def run_gather(args, cfg):
     out = torch.empty((8, n), dtype=torch.float64, device="cuda")
     tri = torch.empty(n, dtype=torch.int32, device="cuda")
 
-    def timed(P):
-        for _ in range(args.warmup):
+    def timed(P, mode):
+        g.set_gather_mode(mode)
+        for _ in range(warmup):
             g.gather(P["R"], P["Z"], P["phi"], out=out, tri_out=tri)
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-        ev[0].record()
-        for s in range(args.steps):
-            g.gather(P["R"], P["Z"], P["phi"], out=out, tri_out=tri)
-            ev[s + 1].record()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
-        return statistics.mean(ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)) * 1e-3
+        a.record()
+        for s in range(steps):
+            g.gather(P["R"], P["Z"], P["phi"], out=out, tri_out=tri)
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) * 1e-3 / steps, (g.gather_kernel_ms() if mode != 1 else None)
 
-    t_rand = timed(pts)
+    t_rand_auto, parts_rand_auto = timed(pts, 0)
+    t_rand, parts_rand = timed(pts, 2)
+    t_rand_direct, _ = timed(pts, 1)
     # cell key = triangle x toroidal interval (caller numbering is enough to make the reads of a cell adjacent)
     k = torch.clamp((pts["phi"] % cfg.phi_period) / cfg.phi_period * cfg.n_planes, max=cfg.n_planes - 1).to(torch.int64)
     key = tri.to(torch.int64) * cfg.n_planes + k
     order = torch.argsort(key)
     spts = {q: v[order].contiguous() for q, v in pts.items()}
     del key, order, k
-    t_sort = timed(spts)
+    t_sort_auto, parts_sort_auto = timed(spts, 0)
+    t_sort, parts_sort = timed(spts, 2)
+    t_sort_direct, _ = timed(spts, 1)
     T, Pn = 2 * cfg.nr * cfg.ntheta, cfg.n_planes
-    table = T * (Pn + 5) * 336
-    algo = n * (24 + 4 + 64) + table          # points in, triangle id + 8 values out, one pass over the coefficient table
+    table = T * Pn * 336
+    algo = n * (24 + 4 + 64) + table          # points in, triangle id + 8 values out, one pass over the coefficient table (SURVEY 8(d))
     peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"] if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else 6650.0
-    line = {"mode": "gather", "metric": "field gathers/s (fp64, 1 B200)", "unit": "gathers/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
-            "value": n / t_sort, "value_unsorted": n / t_rand, "ms_sorted": 1e3 * t_sort, "ms_unsorted": 1e3 * t_rand, "dtype": "f64", "data": "synthetic",
+    line = {"mode": "gather", "metric": "field gathers/s (fp64, 1 B200)", "unit": "gathers/s", "n_gpus": 1, "steps": steps, "warmup": warmup,
+            "value": n / t_rand_auto, "value_sorted_input": n / t_sort_auto, "dtype": "f64", "data": "synthetic",
+            "ms": {"auto_unsorted_input": 1e3 * t_rand_auto, "auto_sorted_input": 1e3 * t_sort_auto, "staged_unsorted_input": 1e3 * t_rand, "staged_sorted_input": 1e3 * t_sort, "direct_unsorted_input": 1e3 * t_rand_direct,
+                   "direct_sorted_input": 1e3 * t_sort_direct},
+            "parts_ms": {"auto_unsorted_input": parts_rand_auto, "auto_sorted_input": parts_sort_auto, "staged_unsorted_input": parts_rand,
+                         "staged_sorted_input": parts_sort},
             "config": {"workload": f"{cfg.name}: {T} triangles x {Pn} planes, {n} points, one evaluation of phi, A_par and gradients per point",
-                       "l2": "inputs_exceed_l2"},
-            "roofline": {"bound": "hbm", "achieved": algo / t_sort / 1e9, "achieved_unsorted": algo / t_rand / 1e9, "peak": peak, "unit": "GB/s",
-                         "frac": algo / t_sort / 1e9 / peak, "traffic": None, "kernel": "k_gather", "algorithmic_bytes": algo}}
-    print(json.dumps(line), flush=True)
+                       "l2": "inputs_exceed_l2", "build_defs": _build_defs()},
+            "roofline": {"bound": "hbm", "achieved": algo / t_rand_auto / 1e9, "achieved_sorted_input": algo / t_sort_auto / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": algo / t_rand_auto / 1e9 / peak, "frac_sorted_input": algo / t_sort_auto / 1e9 / peak,
+                         "frac_direct_unsorted_input": algo / t_rand_direct / 1e9 / peak, "traffic": None,
+                         "kernel": "trimeg_gather, whole call in automatic mode (unsorted input: probe + k_gather_keys + scan + k_gather_scatter + k_gather_staged + k_gather_unsort; cell-sorted input: probe + k_gather)",
+                         "algorithmic_bytes": algo, "peak_kind": "MEASURED_PEAKS.json hbm_gbs" if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else "fallback"}}
+    g.close()
+    del pts, spts, out, tri
+    torch.cuda.empty_cache()
+    return line
 
 
 def main():
@@ -265,7 +284,7 @@ def main():
         return
     if args.gather:
         if rank == 0:
-            run_gather(args, cfg)
+            print(json.dumps(run_gather(args, cfg)), flush=True)
         return
 
     import torch

@@ -105,6 +105,20 @@ size_t trimeg_fields_bytes(const trimeg_ctx* ctx);
 int trimeg_fields_export(trimeg_ctx* ctx, void* dst_device, size_t bytes);
 int trimeg_fields_import(trimeg_ctx* ctx, const void* src_device, size_t bytes);
 
+/* How trimeg_gather runs on the device.  Two paths: the direct kernel (one thread per point, coefficients through L1/L2:
+ * fastest when the caller's points are already clustered by cell) and the staged path (the library bins the points by cell,
+ * stages the coefficient blocks in shared memory by TMA and un-sorts the results; csrc/trimeg_gather.cuh: 4x faster on
+ * points in random order).  0 (default): direct below 65536 points, otherwise chosen on the device from a sample of the
+ * points (share of neighbours in the same cell); 1 forces the direct kernel, 2 the staged path.  The staged path keeps a
+ * library-owned DEVICE workspace of 108 bytes per point (grow-only, freed by mesh_load / destroy).  Results do not depend
+ * on the mode beyond rounding.  Errors: BAD_ARG. */
+int trimeg_set_gather_mode(trimeg_ctx* ctx, int32_t mode);
+/* Device time (CUDA events on the context's stream; blocks until they completed) of the last gather of >= 65536 points that
+ * was not forced onto the direct kernel, milliseconds: [0] locate + keys + histogram, [1] scan, [2] scatter into cell order,
+ * [3] staged evaluation, [4] un-sort into the caller's arrays, [5] direct kernel (the path not taken returns at once).
+ * Errors: BAD_ARG, BAD_STATE (no such gather yet), CUDA. */
+int trimeg_gather_kernel_ms(trimeg_ctx* ctx, double out[6]);
+
 /* Bytes of DEVICE scratch trimeg_markers_bind needs for n markers (0 on error): 268 bytes per marker (two buffers of
  * 128-byte records for the re-sorting phases + sort key, permutation and follow-up list, 4 bytes each): 26.8 GB at 1e8
  * markers.  This is twice the structure-of-arrays budget of SURVEY.md 8(a) (a1); DESIGN.md section 5 says why. */

@@ -21,7 +21,7 @@ EXPORTS = [
     "trimeg_species_set", "trimeg_mesh_load", "trimeg_fields_set", "trimeg_gather", "trimeg_scratch_bytes",
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
     "trimeg_rhs", "trimeg_set_push_variant", "trimeg_push_variant_used", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
-    "trimeg_fields_bytes", "trimeg_fields_export", "trimeg_fields_import", "trimeg_build_info",
+    "trimeg_fields_bytes", "trimeg_fields_export", "trimeg_fields_import", "trimeg_build_info", "trimeg_set_gather_mode", "trimeg_gather_kernel_ms",
 ]
 
 
@@ -67,6 +67,8 @@ def load_library():
     lib.trimeg_mesh_load.argtypes = [vp, i64, vp, i64, vp, i32, dbl]
     lib.trimeg_fields_set.argtypes = [vp, C.c_int, vp, C.c_int]
     lib.trimeg_gather.argtypes = [vp, i64, vp, vp, vp, vp, vp, C.c_int]
+    lib.trimeg_set_gather_mode.argtypes = [vp, i32]
+    lib.trimeg_gather_kernel_ms.argtypes = [vp, C.POINTER(dbl)]
     lib.trimeg_build_info.argtypes = []
     lib.trimeg_build_info.restype = C.c_char_p
     lib.trimeg_fields_bytes.argtypes = [vp]
@@ -188,6 +190,15 @@ class Trimeg:
     def fields_import(self, buf):
         assert buf.is_cuda and buf.is_contiguous()
         self._ck(self._lib.trimeg_fields_import(self._h, buf.data_ptr(), buf.numel() * buf.element_size()), "trimeg_fields_import")
+
+    def set_gather_mode(self, mode):
+        """0 automatic, 1 direct kernel, 2 staged path."""
+        self._ck(self._lib.trimeg_set_gather_mode(self._h, int(mode)), "trimeg_set_gather_mode")
+
+    def gather_kernel_ms(self):
+        a = (C.c_double * 6)()
+        self._ck(self._lib.trimeg_gather_kernel_ms(self._h, a), "trimeg_gather_kernel_ms")
+        return dict(keys=a[0], scan=a[1], scatter=a[2], staged=a[3], unsort=a[4], direct=a[5])
 
     # ---- gather
     def gather(self, R, Z, phi, out=None, tri_out=None, want_tri=True):

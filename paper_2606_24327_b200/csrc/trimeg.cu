@@ -66,7 +66,18 @@ struct trimeg_ctx {
     TileTables tt{};
     CellMap cm{};
     bool tiled_ok = false;
+    // staged gather (trimeg_gather with many points): its own cell numbering and counting-sort arrays, a grow-only workspace
+    GatherMap gm{};
+    long long g_ncell = 0;
+    int g_nunits = 0;
+    int *d_orig = nullptr, *d_ghist = nullptr, *d_goffs = nullptr, *d_gfill = nullptr, *d_gsums = nullptr, *d_gwork = nullptr;
+    void* d_gws = nullptr;
+    size_t gws_bytes = 0;
+    int gather_mode = 0;        // 0 automatic (staged for n >= GATHER_STAGED_MIN), 1 always direct, 2 always staged
+    double gather_ms[5] = {0, 0, 0, 0, 0};   // device time of the last staged gather: keys, scan, scatter, staged, unsort
+    cudaEvent_t gev[7] = {};
 };
+static constexpr long long GATHER_STAGED_MIN = 1 << 16;
 
 static int fail(trimeg_ctx* c, int code, const char* fmt, ...) {
     if (c) {
@@ -97,6 +108,8 @@ static void free_mesh(trimeg_ctx* c) {
     cudaFree(c->d_RZ); cudaFree(c->d_K); cudaFree(c->d_coef);
     cudaFree(c->d_hist); cudaFree(c->d_offs); cudaFree(c->d_fill); cudaFree(c->d_sums);
     cudaFree(c->d_pslots); cudaFree(c->d_pnslots); cudaFree(c->d_pnbr); cudaFree(c->d_work); cudaFree(c->d_stats);
+    cudaFree(c->d_orig); cudaFree(c->d_ghist); cudaFree(c->d_goffs); cudaFree(c->d_gfill); cudaFree(c->d_gsums); cudaFree(c->d_gwork); cudaFree(c->d_gws);
+    c->d_orig = c->d_ghist = c->d_goffs = c->d_gfill = c->d_gsums = c->d_gwork = nullptr; c->d_gws = nullptr; c->gws_bytes = 0;
     c->d_pslots = c->d_pnslots = c->d_work = nullptr; c->d_pnbr = nullptr; c->d_stats = nullptr;
     c->d_geom = nullptr; c->d_tri = c->d_head = c->d_list = nullptr;
     c->d_RZ = c->d_K = c->d_coef = nullptr;
@@ -138,6 +151,7 @@ int trimeg_create(trimeg_ctx** out, int device, void* cuda_stream) {
         return TRIMEG_ERR_CUDA;
     }
     for (auto& st : c->ev) for (auto& e : st) if (cudaEventCreate(&e) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
+    for (auto& e : c->gev) if (cudaEventCreate(&e) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
     *out = c;
     return TRIMEG_OK;
 }
@@ -147,6 +161,7 @@ int trimeg_destroy(trimeg_ctx* ctx) {
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     for (auto& st : ctx->ev) for (auto& e : st) if (e) cudaEventDestroy(e);
+    for (auto& e : ctx->gev) if (e) cudaEventDestroy(e);
     free_mesh(ctx);
     delete ctx;
     return TRIMEG_OK;
@@ -247,6 +262,24 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
     CU(cudaMalloc(&ctx->d_pnbr, sizeof(short) * hp.nbr.size()));
     CU(cudaMalloc(&ctx->d_work, sizeof(int) * 8));
     CU(cudaMalloc(&ctx->d_stats, sizeof(unsigned long long) * 4));
+    {   // staged gather: cells = (patch of GT triangles) x (window of GW intervals) x GT x GW
+        const int gnwin = (n_planes + GW - 1) / GW, gnpatch = (T + GT - 1) / GT;
+        ctx->gm.nwin = gnwin;
+        ctx->g_nunits = gnpatch * gnwin;
+        ctx->g_ncell = (long long)ctx->g_nunits * GCELLS;
+        if ((double)ctx->g_nunits * GCELLS + 2 > 2.0e9) return fail(ctx, TRIMEG_ERR_BAD_ARG, "mesh_load: too many cells for int32 ids");
+        const size_t gcnt = (size_t)ctx->g_ncell + 2;
+        CU(cudaMalloc(&ctx->d_orig, sizeof(int) * T));
+        CU(cudaMalloc(&ctx->d_ghist, sizeof(int) * gcnt));
+        CU(cudaMalloc(&ctx->d_goffs, sizeof(int) * gcnt));
+        CU(cudaMalloc(&ctx->d_gfill, sizeof(int) * gcnt));
+        CU(cudaMalloc(&ctx->d_gsums, sizeof(int) * (gcnt / SCAN_CHUNK + 2)));
+        CU(cudaMalloc(&ctx->d_gwork, sizeof(int) * 4));
+        CU(cudaMemcpyAsync(ctx->d_orig, hm.orig_of_new.data(), sizeof(int) * T, cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaMemsetAsync(ctx->d_ghist, 0, sizeof(int) * gcnt, ctx->stream));
+        CU(cudaMemsetAsync(ctx->d_gfill, 0, sizeof(int) * gcnt, ctx->stream));
+        CU(cudaFuncSetAttribute(k_gather_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GatherSmem::BYTES));
+    }
     CU(cudaMemcpyAsync(ctx->d_pslots, hp.slots.data(), sizeof(int) * hp.slots.size(), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_pnslots, hp.nslots.data(), sizeof(int) * hp.nslots.size(), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_pnbr, hp.nbr.data(), sizeof(short) * hp.nbr.size(), cudaMemcpyHostToDevice, ctx->stream));
@@ -329,17 +362,72 @@ int trimeg_fields_import(trimeg_ctx* ctx, const void* src_device, size_t bytes) 
     return TRIMEG_OK;
 }
 
+// DEVICE pointers; the staged path for many points (trimeg_gather.cuh), the direct kernel otherwise
+static int gather_device(trimeg_ctx* ctx, long long n, const double* R, const double* Z, const double* phi, double* out, int32_t* tri_out) {
+    if (ctx->gather_mode == 1 || (ctx->gather_mode == 0 && n < GATHER_STAGED_MIN)) {
+        k_gather<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, n, R, Z, phi, out, tri_out, nullptr);
+        KCHECK();
+        return TRIMEG_OK;
+    }
+    if (n > 2000000000LL) return fail(ctx, TRIMEG_ERR_BAD_ARG, "gather: n exceeds int32 point ids");
+    // workspace (library-owned, grows on demand, kept for the next call): keys, triangles, positions, point and result records
+    const size_t need = 3 * align256(sizeof(int) * (size_t)n) + align256(sizeof(GPoint) * (size_t)n) + align256(sizeof(double) * 8 * (size_t)n);
+    if (need > ctx->gws_bytes) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_gws); ctx->d_gws = nullptr; ctx->gws_bytes = 0;
+        CU(cudaMalloc(&ctx->d_gws, need));
+        ctx->gws_bytes = need;
+    }
+    char* ptr = (char*)ctx->d_gws;
+    int* keys = (int*)ptr; ptr += align256(sizeof(int) * (size_t)n);
+    int* tris = (int*)ptr; ptr += align256(sizeof(int) * (size_t)n);
+    int* inv = (int*)ptr; ptr += align256(sizeof(int) * (size_t)n);
+    GPoint* pts = (GPoint*)ptr; ptr += align256(sizeof(GPoint) * (size_t)n);
+    double* res = (double*)ptr;
+    const long long gcnt = ctx->g_ncell + 2;
+    const int nb = (int)((gcnt + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    // d_gwork: [0] work counter of the staged kernel, [1] path flag (1 direct, 2 staged), [2..3] probe counters
+    int* flag = ctx->d_gwork + 1;
+    CU(cudaMemsetAsync(ctx->d_gwork, 0, sizeof(int) * 4, ctx->stream));
+    if (ctx->gather_mode == 0) {
+        const int runs = (int)std::min<long long>(GPROBE_RUNS, std::max<long long>(1, n / 32));
+        k_gather_probe<<<runs, 32, 0, ctx->stream>>>(ctx->tb, ctx->gm, n, R, Z, phi, ctx->d_gwork + 2);
+        KCHECK();
+    }
+    k_gather_decide<<<1, 1, 0, ctx->stream>>>(ctx->gather_mode, ctx->d_gwork + 2, flag);
+    KCHECK();
+    CU(cudaEventRecord(ctx->gev[0], ctx->stream));
+    k_gather_keys<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, ctx->gm, n, R, Z, phi, (int)ctx->g_ncell, keys, tris, ctx->d_ghist, flag);
+    KCHECK();
+    CU(cudaEventRecord(ctx->gev[1], ctx->stream));
+    k_scan_reduce<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums);
+    k_scan_sums<<<1, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_gsums, nb);
+    k_scan_apply<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums, ctx->d_goffs, ctx->d_gfill);   // also clears histogram and fill
+    KCHECK();
+    CU(cudaEventRecord(ctx->gev[2], ctx->stream));
+    k_gather_scatter<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(n, R, Z, phi, keys, tris, ctx->d_goffs, ctx->d_gfill, pts, inv, flag);
+    KCHECK();
+    CU(cudaEventRecord(ctx->gev[3], ctx->stream));
+    k_gather_staged<<<ctx->num_sms * 2, GTHREADS, GatherSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->g_nunits, ctx->NPP, ctx->d_goffs, pts, res, ctx->d_gwork, flag);
+    KCHECK();
+    CU(cudaEventRecord(ctx->gev[4], ctx->stream));
+    k_gather_unsort<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(n, tris, inv, res, ctx->d_orig, out, tri_out, flag);
+    KCHECK();
+    CU(cudaEventRecord(ctx->gev[5], ctx->stream));
+    k_gather<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, n, R, Z, phi, out, tri_out, flag);
+    KCHECK();
+    CU(cudaEventRecord(ctx->gev[6], ctx->stream));
+    ctx->gather_ms[0] = -1.0;   // events recorded: trimeg_gather_kernel_ms reads them
+    return TRIMEG_OK;
+}
+
 int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi, double* out, int32_t* tri_out, int memspace) {
     if (!ctx || n < 0 || (n > 0 && (!R || !Z || !phi || !out)) || (memspace != TRIMEG_HOST && memspace != TRIMEG_DEVICE))
         return fail(ctx, TRIMEG_ERR_BAD_ARG, "gather: bad argument");
     if (!ctx->have_mesh) return fail(ctx, TRIMEG_ERR_BAD_STATE, "gather: call trimeg_mesh_load first");
     if (n == 0) return TRIMEG_OK;
     CU(cudaSetDevice(ctx->device));
-    if (memspace == TRIMEG_DEVICE) {
-        k_gather<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, n, R, Z, phi, out, tri_out);
-        KCHECK();
-        return TRIMEG_OK;
-    }
+    if (memspace == TRIMEG_DEVICE) return gather_device(ctx, n, R, Z, phi, out, tri_out);
     double* d = nullptr;
     int* dt = nullptr;
     CU(cudaMalloc(&d, sizeof(double) * 11 * (size_t)n));
@@ -349,12 +437,35 @@ int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, 
     step(cudaMemcpyAsync(d, R, sizeof(double) * n, cudaMemcpyHostToDevice, ctx->stream));
     step(cudaMemcpyAsync(d + n, Z, sizeof(double) * n, cudaMemcpyHostToDevice, ctx->stream));
     step(cudaMemcpyAsync(d + 2 * n, phi, sizeof(double) * n, cudaMemcpyHostToDevice, ctx->stream));
-    if (e == cudaSuccess) { k_gather<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, n, d, d + n, d + 2 * n, d + 3 * n, dt); step(cudaGetLastError()); }
-    step(cudaMemcpyAsync(out, d + 3 * n, sizeof(double) * 8 * n, cudaMemcpyDeviceToHost, ctx->stream));
-    if (tri_out) step(cudaMemcpyAsync(tri_out, dt, sizeof(int) * n, cudaMemcpyDeviceToHost, ctx->stream));
+    int rc = TRIMEG_OK;
+    if (e == cudaSuccess) rc = gather_device(ctx, n, d, d + n, d + 2 * n, d + 3 * n, dt);
+    if (rc == TRIMEG_OK) {
+        step(cudaMemcpyAsync(out, d + 3 * n, sizeof(double) * 8 * n, cudaMemcpyDeviceToHost, ctx->stream));
+        if (tri_out) step(cudaMemcpyAsync(tri_out, dt, sizeof(int) * n, cudaMemcpyDeviceToHost, ctx->stream));
+    }
     step(cudaStreamSynchronize(ctx->stream));
     cudaFree(d); cudaFree(dt);
+    if (rc != TRIMEG_OK) return rc;
     if (e != cudaSuccess) return fail(ctx, TRIMEG_ERR_CUDA, "gather: %s", cudaGetErrorString(e));
+    return TRIMEG_OK;
+}
+
+int trimeg_set_gather_mode(trimeg_ctx* ctx, int32_t mode) {
+    if (!ctx || mode < 0 || mode > 2) return fail(ctx, TRIMEG_ERR_BAD_ARG, "set_gather_mode: 0 automatic, 1 direct, 2 staged");
+    ctx->gather_mode = mode;
+    return TRIMEG_OK;
+}
+
+int trimeg_gather_kernel_ms(trimeg_ctx* ctx, double out[6]) {
+    if (!ctx || !out) return fail(ctx, TRIMEG_ERR_BAD_ARG, "gather_kernel_ms: null argument");
+    if (ctx->gather_ms[0] != -1.0) return fail(ctx, TRIMEG_ERR_BAD_STATE, "gather_kernel_ms: no staged gather has run");
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaEventSynchronize(ctx->gev[6]));
+    for (int i = 0; i < 6; ++i) {
+        float ms = 0;
+        CU(cudaEventElapsedTime(&ms, ctx->gev[i], ctx->gev[i + 1]));
+        out[i] = ms;
+    }
     return TRIMEG_OK;
 }
 

@@ -1,0 +1,192 @@
+// Staged grid-to-particle gather for many points in any order (trimeg_gather; BASELINE configs[4]).
+//
+// One field evaluation reads 8 x 168 B of coefficients per point; through L1/L2 with the points in caller order that is
+// 7x the algorithmic HBM traffic on config 4 (profiles/r01c_gather_cfg4.md).  Here the library bins the points itself:
+//   1. k_gather_keys     caller order: box-grid locate (L89, L125-140), toroidal interval -> cell key, histogram;
+//   2. scan              (the push's counting-sort kernels) -> cell offsets;
+//   3. k_gather_scatter  caller order: position in the cell order; 32-byte point record written there (a full sector),
+//                        position kept per caller index;
+//   4. k_gather_staged   persistent CTAs, one super-cell (GT triangles x GW toroidal intervals) at a time: its coefficient
+//                        block arrives by TMA bulk copies (double-buffered, mbarrier), warps evaluate its points from
+//                        shared memory and write 64-byte result records in cell order (coalesced);
+//   5. k_gather_unsort   caller order: result record -> the caller's eight arrays (coalesced writes), triangle id.
+// HBM bytes per point: 32 + 68 + (96 + coefficients) + 140, against 92 + coefficients algorithmic; DESIGN.md section 6.
+#pragma once
+
+namespace trimeg {
+
+constexpr int GT = 8, GW = 8;                       // triangles x toroidal intervals per gather super-cell
+constexpr int GNPL = GW + 3;                        // staged planes per triangle
+constexpr int GSLOT = GNPL * PLANE_STRIDE;          // doubles per staged triangle
+constexpr int GCELLS = GT * GW;                     // cells per super-cell
+constexpr int GTHREADS = 256;
+
+struct GatherMap {   // cell numbering of the gather: super-cell (patch, window) major, then triangle, then interval
+    int nwin;
+    __host__ __device__ __forceinline__ int cell(int t, int k) const {
+        const int patch = t / GT, tl = t - patch * GT, w = k / GW, kl = k - w * GW;
+        return ((patch * nwin + w) * GT + tl) * GW + kl;
+    }
+};
+struct __align__(16) GPoint { double R, Z, phi; int id, tri; };   // one point in cell order (32 B)
+static_assert(sizeof(GPoint) == 32, "GPoint");
+
+// Which path?  A strided sample of runs of 32 consecutive points: if most neighbours share a cell the caller's order is
+// already clustered and the direct kernel (coefficients through L1/L2) is the faster one; otherwise the points are binned.
+// flag[0] = 1 direct, 2 staged; every kernel of either path returns at once if the flag names the other path, so the choice
+// costs no host round trip.
+constexpr int GPROBE_RUNS = 2048;
+__global__ void __launch_bounds__(32) k_gather_probe(DevTables tb, GatherMap gm, long long n, const double* __restrict__ R, const double* __restrict__ Z,
+                                                     const double* __restrict__ phi, int* __restrict__ cnt) {
+    const long long nruns = n / 32;
+    const long long run = (long long)blockIdx.x * (nruns / gridDim.x > 0 ? nruns / gridDim.x : 1);
+    const long long i = run * 32 + threadIdx.x;
+    int key = -2 - (int)threadIdx.x;
+    if (i < n) {
+        const int t = locate_box(tb.bg, tb.geom, R[i], Z[i]);
+        double s;
+        const int k = toroidal_interval(tb.tor, phi[i], s);
+        key = t < 0 ? -1 : gm.cell(t, k);
+    }
+    const int up = __shfl_down_sync(0xffffffffu, key, 1);
+    const unsigned same = __ballot_sync(0xffffffffu, threadIdx.x < 31 && up == key);
+    if (threadIdx.x == 0) { atomicAdd(cnt, __popc(same)); atomicAdd(cnt + 1, 31); }
+}
+__global__ void k_gather_decide(int mode, const int* __restrict__ cnt, int* __restrict__ flag) {
+    // clustered if more than 30 % of the sampled neighbours share a cell (cell-sorted input: ~60 % at 2.6 points per cell;
+    // random input: ~0)
+    flag[0] = mode == 1 ? 1 : (mode == 2 ? 2 : (10 * cnt[0] > 3 * cnt[1] ? 1 : 2));
+}
+
+__global__ void __launch_bounds__(256) k_gather_keys(DevTables tb, GatherMap gm, long long n, const double* __restrict__ R, const double* __restrict__ Z,
+                                                     const double* __restrict__ phi, int ncell, int* __restrict__ keys, int* __restrict__ tris,
+                                                     int* __restrict__ hist, const int* __restrict__ flag) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || *flag != 2) return;
+    const int t = locate_box(tb.bg, tb.geom, R[i], Z[i]);
+    double s;
+    const int k = toroidal_interval(tb.tor, phi[i], s);
+    const int key = t < 0 ? ncell : gm.cell(t, k);
+    keys[i] = key;
+    tris[i] = t;
+    atomicAdd(hist + key, 1);
+}
+
+__global__ void __launch_bounds__(256) k_gather_scatter(long long n, const double* __restrict__ R, const double* __restrict__ Z, const double* __restrict__ phi,
+                                                        const int* __restrict__ keys, const int* __restrict__ tris, const int* __restrict__ offs,
+                                                        int* __restrict__ fill, GPoint* __restrict__ pts, int* __restrict__ inv, const int* __restrict__ flag) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || *flag != 2) return;
+    const int key = keys[i];
+    const int pos = offs[key] + atomicAdd(fill + key, 1);
+    double2* dst = reinterpret_cast<double2*>(pts + pos);
+    dst[0] = make_double2(R[i], Z[i]);
+    dst[1] = make_double2(phi[i], __hiloint2double(tris[i], (int)i));     // (id, tri) in the low and high word
+    inv[i] = pos;
+}
+
+// shared memory of one CTA: GNST stages of { coefficients [GT][GSLOT], geometry [GT] }, then control.  Two CTAs per SM, one
+// stage being evaluated and two in flight each: ~120 KB of coefficient copies in flight per SM (HBM latency x bandwidth / SM
+// is ~90 KB)
+constexpr int GNST = 3;
+struct GatherSmem {
+    static constexpr size_t COEF = sizeof(double) * GT * GSLOT;
+    static constexpr size_t STAGE = COEF + sizeof(TriGeom) * GT;
+    static constexpr size_t OFF_CTRL = GNST * STAGE;      // per stage: mbarrier (8 B), unit, begin, end (ints)
+    static constexpr size_t BYTES = OFF_CTRL + GNST * 32;
+};
+
+__global__ void __launch_bounds__(GTHREADS, 2)
+k_gather_staged(DevTables tb, GatherMap gm, int nunits, int NPP, const int* __restrict__ offs, const GPoint* __restrict__ pts,
+                double* __restrict__ res, int* __restrict__ work_counter, const int* __restrict__ flag) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    if (*flag != 2) return;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    auto bar_of = [&](int s) { return reinterpret_cast<unsigned long long*>(smem + GatherSmem::OFF_CTRL + 32 * s); };
+    auto ctl_of = [&](int s) { return reinterpret_cast<int*>(smem + GatherSmem::OFF_CTRL + 32 * s + 8); };
+    if (tid == 0) {
+        for (int q = 0; q < GNST; ++q) mbar_init(bar_of(q), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    // warp 0 stages: next non-empty super-cell off the work list -> stage s (its previous contents have been consumed)
+    auto stage = [&](int s) {
+        int u = 0, begin = 0, end = 0;
+        for (;;) {
+            if (lane == 0) u = atomicAdd(work_counter, 1);
+            u = __shfl_sync(0xffffffffu, u, 0);
+            if (u >= nunits) { u = -1; break; }
+            begin = offs[(long long)u * GCELLS]; end = offs[(long long)(u + 1) * GCELLS];
+            if (begin != end) break;
+        }
+        int* ctl = ctl_of(s);
+        if (lane == 0) { ctl[0] = u; ctl[1] = begin; ctl[2] = end; }
+        if (u < 0) { __syncwarp(); if (lane == 0) mbar_arrive(bar_of(s)); return; }
+        const int patch = u / gm.nwin, w = u - patch * gm.nwin;
+        const int pp0 = w * GW + PLANE_PAD, npl = min(GNPL, NPP - pp0);
+        const int t = patch * GT + lane;
+        const bool has = lane < GT && t < tb.T;
+        double* coef = reinterpret_cast<double*>(smem + GatherSmem::STAGE * s);
+        TriGeom* geom = reinterpret_cast<TriGeom*>(smem + GatherSmem::STAGE * s + GatherSmem::COEF);
+        if (has) geom[lane] = tb.geom[t];
+        const unsigned bytes = (unsigned)(npl * PLANE_STRIDE * sizeof(double));
+        const int cnt = __popc(__ballot_sync(0xffffffffu, has));
+        fence_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_expect_tx(bar_of(s), cnt * bytes);
+        __syncwarp();
+        if (has) tma_bulk_g2s(coef + (size_t)lane * GSLOT, tb.coef + (long long)t * tb.tri_stride + (long long)pp0 * PLANE_STRIDE, bytes, bar_of(s));
+    };
+    if (wid == 0) { for (int q = 0; q < GNST - 1; ++q) stage(q); }
+    for (unsigned it = 0;; ++it) {
+        const int s = it % GNST;
+        if (wid == 0) stage((it + GNST - 1) % GNST);      // that stage was released by the barrier at the end of the last round
+        mbar_wait(bar_of(s), (it / GNST) & 1);
+        const int* ctl = ctl_of(s);
+        const int u = ctl[0], begin = ctl[1], end = ctl[2];
+        if (u < 0) break;
+        const int patch = u / gm.nwin, w = u - patch * gm.nwin;
+        const double* coef = reinterpret_cast<const double*>(smem + GatherSmem::STAGE * s);
+        const TriGeom* geom = reinterpret_cast<const TriGeom*>(smem + GatherSmem::STAGE * s + GatherSmem::COEF);
+        for (int pos = begin + tid; pos < end; pos += GTHREADS) {
+            GPoint p;
+            {
+                const double2* src = reinterpret_cast<const double2*>(pts + pos);
+                const double2 a = __ldcs(src), b = __ldcs(src + 1);
+                p.R = a.x; p.Z = a.y; p.phi = b.x;
+                p.id = __double2loint(b.y); p.tri = __double2hiint(b.y);
+            }
+            const int tl = p.tri - patch * GT;
+            const TriGeom& g = geom[tl];
+            double xi, eta, bw[4], dw[4], acc[8];
+            ref_coords(g, p.R, p.Z, xi, eta);
+            const int k = bspline_weights(tb.tor, p.phi, bw, dw);
+            LdShared ld{smem_u32(coef + (size_t)tl * GSLOT + (size_t)(k - w * GW) * PLANE_STRIDE)};
+            gather_cell<true, double>(ld, xi, eta, bw, dw, acc);
+            Fields f;
+            to_fields(g, acc, f);
+            double2* o = reinterpret_cast<double2*>(res + 8ll * pos);
+            __stcs(o, make_double2(f.P, f.PR)); __stcs(o + 1, make_double2(f.PZ, f.Pp));
+            __stcs(o + 2, make_double2(f.A, f.AR)); __stcs(o + 3, make_double2(f.AZ, f.Ap));
+        }
+        __syncthreads();                                  // everybody is done with stage s
+    }
+}
+
+__global__ void __launch_bounds__(256) k_gather_unsort(long long n, const int* __restrict__ tris, const int* __restrict__ inv, const double* __restrict__ res,
+                                                       const int* __restrict__ orig, double* __restrict__ out, int* __restrict__ tri_out,
+                                                       const int* __restrict__ flag) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || *flag != 2) return;
+    const int t = tris[i];
+    double2 a = make_double2(0, 0), b = a, c = a, d = a;
+    if (t >= 0) {
+        const double2* r = reinterpret_cast<const double2*>(res + 8ll * inv[i]);
+        a = __ldcs(r); b = __ldcs(r + 1); c = __ldcs(r + 2); d = __ldcs(r + 3);
+    }
+    out[i] = a.x; out[n + i] = a.y; out[2 * n + i] = b.x; out[3 * n + i] = b.y;
+    out[4 * n + i] = c.x; out[5 * n + i] = c.y; out[6 * n + i] = d.x; out[7 * n + i] = d.y;
+    if (tri_out) tri_out[i] = t < 0 ? -1 : orig[t];
+}
+
+}  // namespace trimeg

@@ -203,9 +203,10 @@ __device__ __forceinline__ void gather_at(const DevTables& tb, int t, double R, 
 }
 
 __global__ void __launch_bounds__(256, 4) k_gather(DevTables tb, long long n, const double* __restrict__ R, const double* __restrict__ Z,
-                                                const double* __restrict__ phi, double* __restrict__ out, int* __restrict__ tri_out) {
+                                                const double* __restrict__ phi, double* __restrict__ out, int* __restrict__ tri_out,
+                                                const int* __restrict__ flag) {   // flag: null, or the path chosen on the device (1 = this kernel)
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (m >= n) return;
+    if (m >= n || (flag && *flag != 1)) return;
     double r = R[m], z = Z[m];
     int t = locate_box(tb.bg, tb.geom, r, z);
     Fields f;
@@ -439,6 +440,7 @@ struct RetireList {
 
 }  // namespace trimeg
 #include "trimeg_ws.cuh"
+#include "trimeg_gather.cuh"
 namespace trimeg {
 
 // ============================================================================================ counting sort by cell

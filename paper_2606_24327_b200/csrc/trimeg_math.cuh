@@ -225,6 +225,7 @@ __device__ inline int locate_box(const BoxGrid& bg, const TriGeom* __restrict__ 
         double xi, eta;
         ref_coords(geom[t], R, Z, xi, eta);
         double m = fmin(fmin(xi, eta), 1.0 - xi - eta);
+        if (m >= 0.0) return t;     // inside: no other candidate can beat it by more than an edge tie
         if (m >= bestmin) { bestmin = m; best = t; }
     }
     return best;

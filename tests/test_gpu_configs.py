@@ -222,3 +222,45 @@ def test_push_is_bitwise_reproducible():
     for k in ("R", "Z", "phi", "u", "w"):
         assert _rel(runs[2][k], runs[0][k], cfg.phi_period if k == "phi" else None) < 1e-12, k
     assert np.array_equal(runs[0]["status"], runs[2]["status"])
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_gather_direct_and_staged_paths(mode):
+    """trimeg_gather's two device paths (one thread per point through L1/L2; library-side binning + TMA-staged coefficient
+    blocks) against the oracle: config 0 with all markers, the unstructured EM mesh with a ragged count, points outside the
+    mesh and in the hole mixed in, phi far outside [0, 2 pi), n = 1 and n = 2 through the staged path."""
+    import torch
+    cfg = synth.CONFIGS[0]
+    RZ, tri, o, g, m = _make(cfg)
+    g.set_gather_mode(mode)
+    R, Z, phi = m["R"].copy(), m["Z"].copy(), m["phi"].copy()
+    R[::97] = cfg.R0 + 2.0 * cfg.a          # outside
+    R[5::101] = cfg.R0 + 0.01 * cfg.a       # in the hole
+    Z[5::101] = 0.0
+    phi[::7] += 5 * cfg.phi_period
+    phi[3::11] -= 3 * cfg.phi_period
+    ref, tref = o.gather(R, Z, phi)
+    out, tout = g.gather(torch.from_numpy(R).cuda(), torch.from_numpy(Z).cuda(), torch.from_numpy(phi).cuda())
+    out, tout = out.cpu().numpy(), tout.cpu().numpy()
+    assert ((tout < 0) == (tref < 0)).all() and (tref < 0).sum() > 150
+    assert np.abs(out[:, tref < 0]).max() == 0.0
+    for q in range(8):
+        assert _rel(out[q], ref[q]) < GATHER_TOL, (q, _rel(out[q], ref[q]))
+    assert (tout == tref).mean() > 0.995
+    for n in (1, 2, 33):
+        o1, t1 = g.gather(R[:n].copy(), Z[:n].copy(), phi[:n].copy())     # HOST buffers
+        for q in range(8):
+            assert np.abs(o1[q] - ref[q][:n]).max() <= GATHER_TOL * np.abs(ref[q]).max()
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, n_markers=70_001)
+    RZ, tri, o, g, m = _make(cfg)
+    g.set_gather_mode(mode)
+    ref, tref = o.gather(m["R"], m["Z"], m["phi"])
+    d = _dev({k: m[k] for k in ("R", "Z", "phi")})
+    out, tout = g.gather(d["R"], d["Z"], d["phi"])
+    for q in range(8):
+        assert _rel(out[q].cpu().numpy(), ref[q]) < GATHER_TOL
+    if mode == 2:
+        assert sum(g.gather_kernel_ms().values()) > 0
+        g.set_gather_mode(1)
+        out1, tout1 = g.gather(d["R"], d["Z"], d["phi"])
+        assert torch.equal(tout, tout1) and float((out - out1).abs().max()) <= 1e-13 * float(out1.abs().max())
