@@ -57,6 +57,9 @@ def _load():
         lib.orc_ln_f0.restype = C.c_double
         lib.orc_grad_ln_f0.argtypes = [C.c_void_p] + [C.c_double] * 4 + [_d]
         lib.orc_rhs.argtypes = [C.c_void_p, C.c_int64] + [_d] * 7 + [_d, _i]
+        lib.orc_pullback.argtypes = [C.c_void_p, C.c_int64] + [_d] * 7 + [_i]
+        lib.orc_density_g2p.argtypes = [C.c_void_p, C.c_int, C.c_int64, _d, _d, _d, _d]
+        lib.orc_f_interp.argtypes = [C.c_void_p, C.c_int64] + [_d] * 6
         lib.orc_push_rk4.argtypes = [C.c_void_p, C.c_int64] + [_d] * 7 + [_i, C.c_double, C.c_int32]
         _lib = lib
     return _lib
@@ -167,6 +170,26 @@ class Oracle:
         outside = np.zeros(n, dtype=np.int32)
         self._ck(self._lib.orc_rhs(self._h, n, *a, out, outside), "rhs")
         return out, outside
+
+    def pullback(self, R, Z, phi, u, w, mu, p):
+        """-> new (u, w, status); the other inputs are unchanged by the map."""
+        R, Z, phi, mu, p = [_f(x) for x in (R, Z, phi, mu, p)]
+        u, w = _f(u).copy(), _f(w).copy()
+        st = np.zeros(R.shape[0], dtype=np.int32)
+        self._ck(self._lib.orc_pullback(self._h, R.shape[0], R, Z, phi, u, w, mu, p, st), "pullback")
+        return u, w, st
+
+    def density_g2p(self, which, R, Z, phi):
+        R, Z, phi = _f(R), _f(Z), _f(phi)
+        out = np.zeros(R.shape[0])
+        self._ck(self._lib.orc_density_g2p(self._h, int(which), R.shape[0], R, Z, phi, out), "density_g2p")
+        return out
+
+    def f_interp(self, R, Z, phi, u, mu):
+        R, Z, phi, u, mu = [_f(x) for x in (R, Z, phi, u, mu)]
+        out = np.zeros(R.shape[0])
+        self._ck(self._lib.orc_f_interp(self._h, R.shape[0], R, Z, phi, u, mu, out), "f_interp")
+        return out
 
     def push_rk4(self, R, Z, phi, u, w, mu, p, dt, nsteps, status=None):
         """Returns new (R, Z, phi, u, w, status); inputs are not modified."""

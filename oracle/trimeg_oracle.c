@@ -31,10 +31,22 @@
  *       its integrator, L89).
  *   O9  a marker evaluated outside the mesh feels zero perturbed field and
  *       gets a sticky status bit.
+ *   O10 the three other grid-to-particle kernels of L97-103 ("pullback
+ *       treatment", "density calculation", "distribution-function
+ *       interpolation": one sentence each in the paper, "all these kernels rely
+ *       on the same G2P function"; readings R22-R24 of DESIGN.md):
+ *       pullback = the linearised mixed-variable -> symplectic map of Eq.(1),
+ *       (6) with dA^h = A_par:  u <- u - (q/m) A_par,  w <- w + p (q/m) A_par
+ *       d ln f0/du (at the old u);  density = the value of one grid field at
+ *       every marker;  f-interpolation = f0 (Maxwellian, Eq.(8) profiles, up to
+ *       its constant factor) at the marker's position and physical parallel
+ *       velocity v_par = u - (q/m) A_par.
  *
  * Parity unpinned (choices the paper does not fix and nothing external can
  * check): the element family itself (R1), the unit system (R8), linear vs
- * nonlinear weight equation (R13), the domain-exit rule (R15).  Everything
+ * nonlinear weight equation (R13), the domain-exit rule (R15), and WHICH maps the
+ * paper's three "other kernels" are (R22-R24: the paper names them in one
+ * sentence each; the maps chosen here are pinned as maps, P17-P19).  Everything
  * else is pinned by tests/test_oracle_*.py.
  *
  * Arithmetic: IEEE double everywhere except the element LU and the 21-term polynomial sums
@@ -431,6 +443,51 @@ static int rhs_one(const orc *c, double R, double Z, double phi, double u, doubl
     d5[0] = X[0]; d5[1] = X[2]; d5[2] = X[1] / R; d5[3] = udot; d5[4] = -pw * (dot3(dX, gl) + dudot * glu);
     return t < 0;
 }
+/* --------------------------------------------------------------- O10 ---- */
+/* L99 "Kernel for pullback treatment ... compute a correction term for the perturbed magnetic potential dA^h for each
+ * particle marker": Eq.(6) u = v_par + (q/m)<dA^h>; with dA^h = A_par (R6) the map to the v_par picture is
+ * u <- u - (q/m) A_par(R), and the perturbed distribution follows to first order: df <- df + (q/m) A_par df0/du, i.e.
+ * w <- w + p (q/m) A_par d ln f0/du evaluated at the OLD u.  Outside the mesh A_par = 0 (O9) and the status bit is set. */
+int orc_pullback(orc *c, int64_t n, const double *R, const double *Z, const double *phi, double *u, double *w, const double *mu, const double *p,
+                 int32_t *status) {
+    if (!c || !c->head) return -1;
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < n; m++) {
+        int64_t t = locate_one(c, R[m], Z[m], 0); double f[4];
+        field_at(c, 1, t, R[m], Z[m], phi[m], f);
+        if (t < 0) { if (status) status[m] |= 1; continue; }
+        equil e; equil_eval(c, R[m], Z[m], &e); double gl[3], glu;
+        grad_ln_f0(c, &e, R[m], Z[m], u[m], mu[m], gl, &glu);
+        double shift = c->qom * f[0];
+        w[m] += p[m] * shift * glu;
+        u[m] -= shift;
+    }
+    return 0;
+}
+/* L100 "Kernel for density calculation": the value of grid field `which` at every marker position (zero outside the mesh) */
+int orc_density_g2p(orc *c, int which, int64_t n, const double *R, const double *Z, const double *phi, double *out) {
+    if (!c || !c->head || which < 0 || which > 1) return -1;
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < n; m++) {
+        int64_t t = locate_one(c, R[m], Z[m], 0); double f[4];
+        field_at(c, which, t, R[m], Z[m], phi[m], f);
+        out[m] = f[0];
+    }
+    return 0;
+}
+/* L101 "Kernel for distribution-function interpolation": f0 (up to its constant factor: n T^-3/2 exp(-E/T), L63) at the
+ * marker's position and at its physical parallel velocity v_par = u - (q/m) A_par (Eq.(6)) */
+int orc_f_interp(orc *c, int64_t n, const double *R, const double *Z, const double *phi, const double *u, const double *mu, double *out) {
+    if (!c || !c->head) return -1;
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < n; m++) {
+        int64_t t = locate_one(c, R[m], Z[m], 0); double f[4];
+        field_at(c, 1, t, R[m], Z[m], phi[m], f);
+        out[m] = exp(ln_f0(c, R[m], Z[m], u[m] - c->qom * f[0], mu[m]));
+    }
+    return 0;
+}
+
 int orc_rhs(orc *c, int64_t n, const double *R, const double *Z, const double *phi, const double *u, const double *w, const double *mu, const double *p, double *out /*[5][n]*/, int32_t *outside) {
     if (!c || !c->have_eq || !c->have_sp || !c->head) return -2;
 #pragma omp parallel for schedule(static)

@@ -332,3 +332,68 @@ def test_lost_marker_status_and_zero_field_outside(cfg0_oracle):
     for q in range(5):
         assert far[q][0] == ref[q][0]
     assert far[4][0] == 0.0  # w stays 0: no perturbed field, no weight drive
+
+
+# ------------------------------------------------------------------------------------------- O10: the other G2P kernels
+def test_other_g2p_kernels_pullback_density_f_interp(cfg0_oracle):
+    """Pins P17-P19 for the three grid-to-particle kernels of PAPER.md L97-103 (readings R22-R24).
+    P17 pullback: identity where A_par = 0 (here: with a zero A_par field) and outside the mesh (status set); for a spatially
+         constant A_par = a0 every marker's u shifts by exactly (q/m) a0 (Eq.(6)) and w by p (q/m) a0 d ln f0/du with
+         d ln f0/du from a central difference of ln f0 (an independent route); forth and back (a0, then -a0) restores u and
+         leaves w off by exactly -p ((q/m) a0)^2 / T(r), the second-order term the linearisation drops.
+    P18 density: equals row 0 / row 4 of the pinned gather, and a0 for the constant field.
+    P19 f-interpolation: equals exp(ln f0) at the shifted velocity; with A_par = 0 it is f0(u); ratio of two markers that differ
+         only in u is exp(-(u1^2 - u2^2) / 2T)."""
+    from oracle import Oracle
+    cfg, RZ, tri, o, (dphi, dap) = cfg0_oracle
+    m = synth.make_markers(cfg, 400)
+    R, Z, phi, u, w, mu, p = [m[k] for k in ("R", "Z", "phi", "u", "w", "mu", "p")]
+    qom = cfg.qom
+    # constant A_par = a0: nodal value a0, all derivatives zero, every plane (spline coefficients of a constant are the constant)
+    a0 = 3.0e-3
+    z = Oracle()
+    z.equilibrium_set(**synth.equilibrium_args(cfg))
+    z.species_set(**synth.species_args(cfg))
+    z.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+    const = np.zeros((cfg.n_planes, RZ.shape[0], 6))
+    const[:, :, 0] = a0
+    z.fields_set(0, np.zeros_like(const))
+    z.fields_set(1, const)
+    u1, w1, st = z.pullback(R, Z, phi, u, w, mu, p)
+    assert not st.any()
+    assert np.abs((u - u1) - qom * a0).max() < 1e-13 * qom * a0 * 10
+    h = 1e-5
+    dlnf = np.array([(z.ln_f0(a, b, c + h, d) - z.ln_f0(a, b, c - h, d)) / (2 * h) for a, b, c, d in zip(R, Z, u, mu)])
+    assert np.abs((w1 - w) - p * qom * a0 * dlnf).max() < 1e-8 * np.abs(w1 - w).max()
+    # back with -a0
+    const[:, :, 0] = -a0
+    z.fields_set(1, const)
+    u2, w2, _ = z.pullback(R, Z, phi, u1, w1, mu, p)
+    assert np.abs(u2 - u).max() < 1e-14
+    T = np.array([-(c) / z.grad_ln_f0(a, b, c, d)[2] for a, b, c, d in zip(R, Z, u, mu)])      # d ln f0/du = -u/T
+    assert np.abs((w2 - w) + p * (qom * a0) ** 2 / T).max() < 1e-10 * (qom * a0) ** 2
+    # zero A_par: identity; outside the mesh: identity + status
+    const[:, :, 0] = 0.0
+    z.fields_set(1, const)
+    u3, w3, st3 = z.pullback(R, Z, phi, u, w, mu, p)
+    assert np.array_equal(u3, u) and np.array_equal(w3, w) and not st3.any()
+    Ro = R.copy()
+    Ro[:5] = cfg.R0 + 1.5 * cfg.a
+    u4, w4, st4 = o.pullback(Ro, Z, phi, u, w, mu, p)
+    assert st4[:5].all() and not st4[5:].any() and np.array_equal(u4[:5], u[:5]) and np.array_equal(w4[:5], w[:5])
+    assert np.abs(u4[5:] - u[5:]).max() > 0          # the config-0 field does move the others
+    # P18
+    g, _ = o.gather(R, Z, phi)
+    assert np.array_equal(o.density_g2p(0, R, Z, phi), g[0]) and np.array_equal(o.density_g2p(1, R, Z, phi), g[4])
+    const[:, :, 0] = a0
+    z.fields_set(1, const)
+    assert np.abs(z.density_g2p(1, R, Z, phi) - a0).max() < 1e-15
+    # P19
+    fi = z.f_interp(R, Z, phi, u, mu)
+    ref = np.exp([z.ln_f0(a, b, c - qom * a0, d) for a, b, c, d in zip(R, Z, u, mu)])
+    assert np.abs(fi - ref).max() <= 1e-15 * ref.max()
+    const[:, :, 0] = 0.0
+    z.fields_set(1, const)
+    f_a = z.f_interp(R, Z, phi, u, mu)
+    f_b = z.f_interp(R, Z, phi, 0.5 * u, mu)
+    assert np.abs(np.log(f_a / f_b) + (u ** 2 - (0.5 * u) ** 2) / (2 * T)).max() < 1e-11
