@@ -172,6 +172,21 @@ int trimeg_push_variant_used(trimeg_ctx* ctx, int32_t* out);
 /* Diagnostics used by the benchmark: achieved FP64 FMA throughput of this device in TFLOP/s
  * (a register-only DFMA loop; the roofline's measured "alu" peak). */
 int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops);
+/* The three other grid-to-particle kernels of the paper ("pullback treatment", "density calculation",
+ * "distribution-function interpolation"; "all these kernels rely on the same G2P function").  The paper gives each one
+ * sentence; what they compute here is DESIGN.md readings R22-R24.  All work on the bound marker store.
+ *  - trimeg_pullback: the linearised map from the p_par (Hamiltonian, dA^h = A_par) to the v_par (symplectic) picture,
+ *    Eq.(1), (6): for every marker  u <- u - (q/m) A_par(R, Z, phi),  w <- w + p (q/m) A_par d ln f0/du (at the old u;
+ *    d ln f0/du = -u / T(r) for the Maxwellian of L63 with the Eq.(8) temperature).  A marker outside the mesh is left
+ *    unchanged and gets its status bit.  In place; invalidates the cached stage of the push.
+ *  - trimeg_density_g2p: out[i] = value of grid field `which` (0 or 1) at marker i (0 outside the mesh), caller order.
+ *  - trimeg_f_interp: out[i] = n(r) T(r)^-3/2 exp(-(v^2/2 + mu B)/T(r)) at marker i with v = u - (q/m) A_par (Eq.(6)):
+ *    the equilibrium distribution f0 up to its constant factor, at the marker's physical parallel velocity.
+ * out: n doubles in `memspace`.  Errors: BAD_ARG, BAD_STATE (mesh, equilibrium, species, markers), CUDA. */
+int trimeg_pullback(trimeg_ctx* ctx);
+int trimeg_density_g2p(trimeg_ctx* ctx, int which, double* out, int memspace);
+int trimeg_f_interp(trimeg_ctx* ctx, double* out, int memspace);
+
 /* The -D options this library was built with beyond the defaults ("" for the shipped configuration). */
 const char* trimeg_build_info(void);
 /* Counters of the last trimeg_push_rk4 call: [0] kernel launches, [1] right-hand-side evaluations that took the

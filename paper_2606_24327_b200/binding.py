@@ -22,6 +22,7 @@ EXPORTS = [
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
     "trimeg_rhs", "trimeg_set_push_variant", "trimeg_push_variant_used", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
     "trimeg_fields_bytes", "trimeg_fields_export", "trimeg_fields_import", "trimeg_build_info", "trimeg_set_gather_mode", "trimeg_gather_kernel_ms",
+    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp",
 ]
 
 
@@ -69,6 +70,9 @@ def load_library():
     lib.trimeg_gather.argtypes = [vp, i64, vp, vp, vp, vp, vp, C.c_int]
     lib.trimeg_set_gather_mode.argtypes = [vp, i32]
     lib.trimeg_gather_kernel_ms.argtypes = [vp, C.POINTER(dbl)]
+    lib.trimeg_pullback.argtypes = [vp]
+    lib.trimeg_density_g2p.argtypes = [vp, C.c_int, vp, C.c_int]
+    lib.trimeg_f_interp.argtypes = [vp, vp, C.c_int]
     lib.trimeg_build_info.argtypes = []
     lib.trimeg_build_info.restype = C.c_char_p
     lib.trimeg_fields_bytes.argtypes = [vp]
@@ -281,6 +285,25 @@ class Trimeg:
         out = np.empty((5, self.n)) if host else t.empty((5, self.n), dtype=t.float64, device=self.device)
         p, ms = _ptr(out)
         self._ck(self._lib.trimeg_rhs(self._h, p, ms), "trimeg_rhs")
+        return out
+
+    def pullback(self):
+        self._ck(self._lib.trimeg_pullback(self._h), "trimeg_pullback")
+
+    def _scalar_out(self, host):
+        t = self._torch
+        return np.empty(self.n) if host else t.empty(self.n, dtype=t.float64, device=self.device)
+
+    def density_g2p(self, which, host=False):
+        out = self._scalar_out(host)
+        p, ms = _ptr(out)
+        self._ck(self._lib.trimeg_density_g2p(self._h, int(which), p, ms), "trimeg_density_g2p")
+        return out
+
+    def f_interp(self, host=False):
+        out = self._scalar_out(host)
+        p, ms = _ptr(out)
+        self._ck(self._lib.trimeg_f_interp(self._h, p, ms), "trimeg_f_interp")
         return out
 
     def sync(self):

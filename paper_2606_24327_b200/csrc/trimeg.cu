@@ -128,6 +128,7 @@ static void derive_species(trimeg_ctx* ctx) {
     p.kn_R0 = s->kappa_n / eq.R0; p.kT_R0 = s->kappa_T / eq.R0;
     p.two_inv_wn_a = 2.0 / (s->w_n * eq.a); p.two_inv_wT_a = 2.0 / (s->w_T * eq.a); p.r0 = s->r0;
     p.cT = s->kappa_T * s->w_T * eq.a / eq.R0;
+    p.cn = s->kappa_n * s->w_n * eq.a / eq.R0;
     p.same_w = (s->w_n == s->w_T) ? 1 : 0;
     p.bstar_exact = s->bstar_exact ? 1 : 0; p.weight_mode = s->weight_mode ? 1 : 0;
 }
@@ -724,6 +725,41 @@ int trimeg_rhs(trimeg_ctx* ctx, double* out, int memspace) {
     if (e != cudaSuccess) return fail(ctx, TRIMEG_ERR_CUDA, "rhs: %s", cudaGetErrorString(e));
     return TRIMEG_OK;
 }
+
+// the three other grid-to-particle kernels (readings R22-R24)
+int trimeg_pullback(trimeg_ctx* ctx) {
+    if (!ctx) return TRIMEG_ERR_BAD_ARG;
+    if (!ctx->have_mesh || !ctx->have_eq || !ctx->have_sp || !ctx->have_markers)
+        return fail(ctx, TRIMEG_ERR_BAD_STATE, "pullback: mesh, equilibrium, species and markers must be set first");
+    CU(cudaSetDevice(ctx->device));
+    k_pullback<<<blocks_for(ctx->n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->recs[ctx->cur], ctx->n);
+    KCHECK();
+    invalidate_step_state(ctx);   // u and w changed: the cached k1 = f(y_n) no longer belongs to the state
+    return TRIMEG_OK;
+}
+
+static int per_marker_scalar(trimeg_ctx* ctx, int kind, int which, double* out, int memspace, const char* what) {
+    if (!ctx || !out || (memspace != TRIMEG_HOST && memspace != TRIMEG_DEVICE) || which < 0 || which > 1) return fail(ctx, TRIMEG_ERR_BAD_ARG, "%s: bad argument", what);
+    if (!ctx->have_mesh || !ctx->have_eq || !ctx->have_sp || !ctx->have_markers)
+        return fail(ctx, TRIMEG_ERR_BAD_STATE, "%s: mesh, equilibrium, species and markers must be set first", what);
+    CU(cudaSetDevice(ctx->device));
+    const long long n = ctx->n;
+    double* d = out;
+    if (memspace == TRIMEG_HOST) CU(cudaMalloc(&d, sizeof(double) * (size_t)n));
+    if (kind == 0) k_density_g2p<<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, which, ctx->recs[ctx->cur], n, d);
+    else k_f_interp<<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->recs[ctx->cur], n, d);
+    cudaError_t e = cudaGetLastError();
+    if (memspace == TRIMEG_HOST) {
+        if (e == cudaSuccess) e = cudaMemcpyAsync(out, d, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream);
+        cudaError_t e2 = cudaStreamSynchronize(ctx->stream);
+        if (e == cudaSuccess) e = e2;
+        cudaFree(d);
+    }
+    if (e != cudaSuccess) return fail(ctx, TRIMEG_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+    return TRIMEG_OK;
+}
+int trimeg_density_g2p(trimeg_ctx* ctx, int which, double* out, int memspace) { return per_marker_scalar(ctx, 0, which, out, memspace, "density_g2p"); }
+int trimeg_f_interp(trimeg_ctx* ctx, double* out, int memspace) { return per_marker_scalar(ctx, 1, 0, out, memspace, "f_interp"); }
 
 int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops) {
     if (!ctx || !tflops) return fail(ctx, TRIMEG_ERR_BAD_ARG, "bench_dfma: null argument");

@@ -428,6 +428,61 @@ __global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP s
     for (int q = 0; q < 5; ++q) out[(long long)q * n + r.id] = d[q];
 }
 
+// ============================================================================================ the other G2P kernels
+// "pullback treatment", "density calculation", "distribution-function interpolation" - "all these kernels
+// rely on the same G2P function; therefore, they have nearly identical structures".  One thread per marker record, fields
+// through L1/L2 (the store is cell-sorted after a push, so neighbouring threads read the same coefficient blocks).
+// Readings R22-R24: what each kernel computes is the paper's one sentence made concrete.
+__device__ __forceinline__ double profile_th(const SpeciesP& sp, double two_inv_w_a, double r) {   // tanh((r - r0) / (w a))
+    return 1.0 - 2.0 / (exp((r - sp.r0) * two_inv_w_a) + 1.0);
+}
+// pullback (L99, Eq.(1), (6)): u <- u - (q/m) A_par,  w <- w + p (q/m) A_par d ln f0/du at the old u,  d ln f0/du = -u / T(r)
+__global__ void __launch_bounds__(128) k_pullback(DevTables tb, EquilP ep, SpeciesP sp, Rec* __restrict__ recs, long long n) {
+    long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    Rec r;
+    rec_load(recs, m, r);
+    const int t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
+    if (t < 0) { r.st |= 1; }
+    else {
+        Fields f;
+        gather_at(tb, t, r.y[0], r.y[1], r.y[2], f);
+        const double x = r.y[0] - ep.R0, rr = sqrt(x * x + r.y[1] * r.y[1]);
+        const double iT = exp(sp.cT * profile_th(sp, sp.two_inv_wT_a, rr));
+        const double shift = sp.qom * f.A;
+        r.y[4] += r.p * shift * (-r.y[3] * iT);
+        r.y[3] -= shift;
+    }
+    rec_store(recs, m, r);   // the triangle hint stays (it belongs to the cached next evaluation point, now invalid anyway)
+}
+// density (L100): value of grid field `which` at every marker, caller order
+__global__ void __launch_bounds__(128) k_density_g2p(DevTables tb, int which, const Rec* __restrict__ recs, long long n, double* __restrict__ out) {
+    long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    Rec r;
+    rec_load(recs, m, r);
+    const int t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
+    Fields f;
+    gather_at(tb, t, r.y[0], r.y[1], r.y[2], f);
+    out[r.id] = which ? f.A : f.P;
+}
+// distribution-function interpolation (L101): f0 = n T^-3/2 exp(-(v^2/2 + mu B)/T) at the marker's position and v = u - (q/m) A_par
+__global__ void __launch_bounds__(128) k_f_interp(DevTables tb, EquilP ep, SpeciesP sp, const Rec* __restrict__ recs, long long n, double* __restrict__ out) {
+    long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    Rec r;
+    rec_load(recs, m, r);
+    const int t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
+    Fields f;
+    gather_at(tb, t, r.y[0], r.y[1], r.y[2], f);
+    Equil<double> e;
+    equil_eval<double>(ep, r.y[0], r.y[1], e);
+    const double thT = profile_th(sp, sp.two_inv_wT_a, e.r), thn = profile_th(sp, sp.two_inv_wn_a, e.r);
+    const double iT = exp(sp.cT * thT), dens = exp(-sp.cn * thn);
+    const double v = r.y[3] - sp.qom * f.A;
+    out[r.id] = dens * iT * sqrt(iT) * exp(-(0.5 * v * v + r.mu * e.B) * iT);
+}
+
 // ============================================================================================ phase kernel: helpers
 // markers that left their staged block during a phase: positions in the cell order, finished by k_phase_global
 // and markers whose NEXT evaluation point left the staged geometry (record done, triangle and sort key still to be found by

@@ -32,6 +32,7 @@ struct SpeciesP {
     double kn_R0, kT_R0;               // kappa_n / R0, kappa_T / R0   (d ln H/dr = -(kappa_H/R0) sech^2)
     double two_inv_wn_a, two_inv_wT_a, r0;     // 2/(w_n a), 2/(w_T a): tanh x = 1 - 2/(exp(2x) + 1)
     double cT;                         // kappa_T w_T a / R0 : 1/T = exp(cT tanh)
+    double cn;                         // kappa_n w_n a / R0 : n = exp(-cn tanh)
     int same_w, bstar_exact, weight_mode;
 };
 struct TorP {

@@ -264,3 +264,48 @@ def test_gather_direct_and_staged_paths(mode):
         g.set_gather_mode(1)
         out1, tout1 = g.gather(d["R"], d["Z"], d["phi"])
         assert torch.equal(tout, tout1) and float((out - out1).abs().max()) <= 1e-13 * float(out1.abs().max())
+
+
+def test_other_g2p_kernels_match_oracle():
+    """trimeg_pullback / trimeg_density_g2p / trimeg_f_interp (readings R22-R24) against the oracle, in
+    caller order, on a fresh store and on a store that has been pushed (cell-sorted, stale triangle hints), with markers
+    outside the mesh; gradient profiles on (config-2-like loading so that T(r) and n(r) matter)."""
+    cfg = dataclasses.replace(synth.CONFIGS[2], nr=12, ntheta=40, n_planes=8, n_markers=20_003)
+    RZ, tri, o, g, m = _make(cfg)
+    m["R"][::211] = cfg.R0 + 1.2 * cfg.a      # outside
+    d = _dev(m)
+
+    def check(state, tag):
+        R, Z, phi, u, w = [state[k] for k in ("R", "Z", "phi", "u", "w")]
+        for which in (0, 1):
+            got = g.density_g2p(which, host=True)
+            ref = o.density_g2p(which, R, Z, phi)
+            assert np.abs(got - ref).max() <= GATHER_TOL * np.abs(ref).max(), (tag, which)
+        got = g.f_interp(host=True)
+        ref = o.f_interp(R, Z, phi, u, m["mu"])
+        assert np.abs(got - ref).max() <= 1e-12 * np.abs(ref).max(), tag
+        got_dev = g.f_interp().cpu().numpy()
+        assert np.array_equal(got_dev, got)
+        u1, w1, st1 = o.pullback(R, Z, phi, u, w, m["mu"], m["p"])
+        g.pullback()
+        res = g.markers_get(host=True)
+        assert np.abs(res["u"] - u1).max() <= 1e-13 * np.abs(u1).max(), tag
+        assert np.abs(res["w"] - w1).max() <= 1e-12 * np.abs(w1).max(), tag
+        assert np.array_equal(res["R"], R) and np.array_equal(res["phi"], phi)
+        assert ((res["status"] != 0) >= (st1 != 0)).all()
+        return res
+
+    g.markers_bind(*[d[k] for k in KEYS])
+    check(m, "fresh store")
+    # after a push: records are in cell order with hints of the next evaluation point
+    g.markers_bind(*[d[k] for k in KEYS])
+    g.set_sort_interval(1)
+    g.push_rk4(cfg.dt, 3)
+    state = g.markers_get(host=True)
+    after = check(state, "pushed store")
+    # the pullback invalidated the cached stage: pushing on must equal the oracle pushing the pulled-back state
+    g.push_rk4(cfg.dt, 2)
+    res = g.markers_get(host=True)
+    exp = o.push_rk4(after["R"], after["Z"], after["phi"], after["u"], after["w"], m["mu"], m["p"], cfg.dt, 2, status=after["status"])
+    for q, k in enumerate(("R", "Z", "phi", "u", "w")):
+        assert _rel(res[k], exp[q], cfg.phi_period if k == "phi" else None) < STATE_TOL, k
