@@ -242,6 +242,58 @@ def run_gather(args, cfg, n=None, steps=None, warmup=None):
     return line
 
 
+def run_push_extra(cfg, sort_every, steps=10, warmup=3, parity_n=2000):
+    """One more BASELINE config through the same library on cuda:0 (device-resident, both phases' kernels, sort inside the
+    timed region), with a small oracle sample; for the `other_configs` record of the bench line."""
+    import torch
+    from oracle import Oracle
+    from paper_2606_24327_b200.binding import Trimeg
+    g = Trimeg(0)
+    setup_case(cfg, g)
+    n = cfg.n_markers
+    host, views = make_inputs(cfg, n, 0, pinned=False)
+    dev = {k: v.cuda() for k, v in host.items()}
+    g.set_push_variant(0)
+    g.set_sort_interval(sort_every)
+    g.markers_bind(*[dev[k] for k in KEYS])
+    g.push_rk4(cfg.dt, warmup)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    g.push_rk4(cfg.dt, steps)
+    b.record()
+    torch.cuda.synchronize()
+    sec = a.elapsed_time(b) * 1e-3
+    st, km = g.push_stats(), g.push_kernel_ms()
+    o = Oracle()
+    setup_case(cfg, o)
+    idx = np.unique(np.concatenate([np.arange(0, n, max(1, n // parity_n)), [n - 1]]))
+    got = g.markers_get()
+    tidx = torch.from_numpy(idx).cuda()
+    got = {k: v[tidx].cpu().numpy() for k, v in got.items()}
+    nst = warmup + steps
+    exp = o.push_rk4(*[views[k][idx] for k in KEYS], cfg.dt, nst)
+    errs = []
+    for q, k in enumerate(("R", "Z", "phi", "u", "w")):
+        dlt = np.abs(got[k] - exp[q])
+        if k == "phi":
+            dlt = np.minimum(dlt, np.abs(dlt - cfg.phi_period))
+        errs.append(float(dlt.max() / max(np.abs(exp[q]).max(), 1e-300)))
+    tol = PARITY_TOL_10 * max(1.0, (nst / 10.0) ** 2)
+    evals = 4.0 * n - st["slow_path"] / steps
+    rec = {"workload": f"{cfg.name}: {2 * cfg.nr * cfg.ntheta} triangles x {cfg.n_planes} planes, {n} markers, dt={cfg.dt}, sort every {sort_every} steps",
+           "ms_per_step": 1e3 * sec / steps, "value": n * steps / sec, "unit": UNIT, "steps": steps, "warmup": warmup,
+           "step_breakdown_ms": km, "retired_fraction_per_phase": st["retired"] / (2.0 * steps * n),
+           "kernel_frac": (FLOP_PER_PUSH / 4.0) * evals / 2 / (km["push"] * 1e-3 / 2) / 1e12 / FP64_PEAK_TFLOPS,
+           "whole_step_frac": FLOP_PER_PUSH * n / (sec / steps) / 1e12 / FP64_PEAK_TFLOPS,
+           "parity": {"n": int(idx.shape[0]), "steps": nst, "max_rel": max(errs), "tol": tol,
+                      "lost_set_equal": bool(((got["status"] != 0) == (exp[5] != 0)).all()), "ok": bool(max(errs) < tol)}}
+    g.close()
+    del dev, got
+    torch.cuda.empty_cache()
+    return rec
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -258,6 +310,7 @@ def main():
     ap.add_argument("--ref-markers", type=int, default=200_000, help="markers per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parity", action="store_true", help="skip the sampled oracle check of the timed run")
+    ap.add_argument("--no-extras", action="store_true", help="skip the other BASELINE configs (1, 2 at both sort intervals, 4 gather) appended to the line")
     ap.add_argument("--parity-sample", type=int, default=10_000, help="markers of the timed run compared with the oracle")
     ap.add_argument("--gather", action="store_true", help="gather-only stress test (use with --config 4), unsorted vs cell-sorted points")
     args = ap.parse_args()
@@ -438,6 +491,20 @@ def main():
                              "hbm_algorithmic_GBps": ALGO_BYTES_PER_LAUNCH * n / kern_s / 1e9},
                 "step_breakdown_ms": {"sort": sort_ms, "push": 1e3 * kern_s * launches_per_step, "finish": finish_ms},
                 "slow_path_evals": slow, "retired_markers": retired, "parity": parity, "fields_bcast": fields_bcast}
+        if not args.no_extras and world == 1 and args.config == 3 and n == cfg.n_markers:
+            # the other BASELINE configs, same library, same run (not the headline)
+            del dev, pinned_out, host, views
+            g.close()
+            torch.cuda.empty_cache()
+            extras = {}
+            try:
+                extras["cfg1"] = run_push_extra(synth.CONFIGS[1], 1)
+                extras["cfg2_sort_every_1"] = run_push_extra(synth.CONFIGS[2], 1)
+                extras["cfg2_sort_every_10_as_BASELINE_states"] = run_push_extra(synth.CONFIGS[2], 10)
+                extras["gather_cfg4"] = run_gather(args, synth.CONFIGS[4], n=synth.CONFIGS[4].n_markers, steps=3, warmup=1)
+            except Exception as ex:   # the headline line must not be lost to an extra
+                extras["error"] = repr(ex)
+            line["other_configs"] = extras
         if not args.no_cpu_baseline:
             cpu_n = min(n, args.cpu_sample)
             v, cores, secs = time_oracle(cfg, cpu_n, 4, oracle=oracle_obj)
