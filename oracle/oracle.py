@@ -60,6 +60,7 @@ def _load():
         lib.orc_pullback.argtypes = [C.c_void_p, C.c_int64] + [_d] * 7 + [_i]
         lib.orc_density_g2p.argtypes = [C.c_void_p, C.c_int, C.c_int64, _d, _d, _d, _d]
         lib.orc_f_interp.argtypes = [C.c_void_p, C.c_int64] + [_d] * 6
+        lib.orc_deposit.argtypes = [C.c_void_p, C.c_int64, _d, _d, _d, _d, _d]
         lib.orc_push_rk4.argtypes = [C.c_void_p, C.c_int64] + [_d] * 7 + [_i, C.c_double, C.c_int32]
         _lib = lib
     return _lib
@@ -189,6 +190,13 @@ class Oracle:
         R, Z, phi, u, mu = [_f(x) for x in (R, Z, phi, u, mu)]
         out = np.zeros(R.shape[0])
         self._ck(self._lib.orc_f_interp(self._h, R.shape[0], R, Z, phi, u, mu, out), "f_interp")
+        return out
+
+    def deposit(self, R, Z, phi, q):
+        """P2G: -> b[n_planes][n_nodes][6], the transpose of the gather applied to the marker charges q."""
+        R, Z, phi, q = [_f(x) for x in (R, Z, phi, q)]
+        out = np.zeros((self.n_planes, self.n_nodes, 6))
+        self._ck(self._lib.orc_deposit(self._h, R.shape[0], R, Z, phi, q, out), "deposit")
         return out
 
     def push_rk4(self, R, Z, phi, u, w, mu, p, dt, nsteps, status=None):

@@ -42,6 +42,13 @@
  *       its constant factor) at the marker's position and physical parallel
  *       velocity v_par = u - (q/m) A_par.
  *
+ *   O11 particle-to-grid deposition onto the C1 x B-spline basis (L35 "projecting
+ *       the quantities stored at the particle locations ... onto the finite
+ *       element grid"; L288, L372: what the paper left on the CPU): the
+ *       transpose of O3.  b[k][v][c] = sum_p q_p N_{v,c}(R_p, Z_p) B_k(phi_p)
+ *       with N_{v,c} the element's nodal basis functions (the interpolant of the
+ *       unit DOF vector) and B_k the toroidal spline (reading R25).
+ *
  * Parity unpinned (choices the paper does not fix and nothing external can
  * check): the element family itself (R1), the unit system (R8), linear vs
  * nonlinear weight equation (R13), the domain-exit rule (R15), and WHICH maps the
@@ -443,6 +450,32 @@ static int rhs_one(const orc *c, double R, double Z, double phi, double u, doubl
     d5[0] = X[0]; d5[1] = X[2]; d5[2] = X[1] / R; d5[3] = udot; d5[4] = -pw * (dot3(dX, gl) + dudot * glu);
     return t < 0;
 }
+/* --------------------------------------------------------------- O11 ---- */
+/* P2G: out[P][n_nodes][6] += q_p * (basis function of every DOF of the marker's triangle, on its four planes).  The basis
+ * function of local DOF j is the element's interpolant of the unit vector e_j (one element solve each: slow and literal).
+ * Markers outside the mesh deposit nothing.  Serial over markers: the sum is in marker order. */
+int orc_deposit(orc *c, int64_t n, const double *R, const double *Z, const double *phi, const double *q, double *out) {
+    if (!c || !c->head) return -1;
+    memset(out, 0, sizeof(double) * (size_t)c->P * (size_t)c->n_nodes * 6);
+    for (int64_t m = 0; m < n; m++) {
+        int64_t t = locate_one(c, R[m], Z[m], 0);
+        if (t < 0) continue;
+        int k; double w[4], dw[4]; bspline(c, phi[m], &k, w, dw);
+        for (int j = 0; j < 18; j++) {
+            double e[18], coef[NM], v[6];
+            for (int i = 0; i < 18; i++) e[i] = (i == j) ? 1.0 : 0.0;
+            element_solve(c, t, e, coef);
+            poly_eval(c, t, coef, R[m], Z[m], v);
+            int node = c->tri[3 * t + j / 6], comp = j % 6;
+            for (int a = 0; a < 4; a++) {
+                int pl = ((k - 1 + a) % c->P + c->P) % c->P;
+                out[((size_t)pl * c->n_nodes + node) * 6 + comp] += q[m] * w[a] * v[0];
+            }
+        }
+    }
+    return 0;
+}
+
 /* --------------------------------------------------------------- O10 ---- */
 /* L99 "Kernel for pullback treatment ... compute a correction term for the perturbed magnetic potential dA^h for each
  * particle marker": Eq.(6) u = v_par + (q/m)<dA^h>; with dA^h = A_par (R6) the map to the v_par picture is

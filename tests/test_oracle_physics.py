@@ -397,3 +397,46 @@ def test_other_g2p_kernels_pullback_density_f_interp(cfg0_oracle):
     f_a = z.f_interp(R, Z, phi, u, mu)
     f_b = z.f_interp(R, Z, phi, 0.5 * u, mu)
     assert np.abs(np.log(f_a / f_b) + (u ** 2 - (0.5 * u) ** 2) / (2 * T)).max() < 1e-11
+
+
+# ------------------------------------------------------------------------------------------- O11: particle-to-grid
+def test_P20_deposit_is_the_transpose_of_the_gather(cfg0_oracle):
+    """Pin P20 for the P2G deposition (reading R25).  b = G^T q is fixed by the pinned gather G through the
+    adjoint identity  sum_dof b_dof d_dof = sum_p q_p F_d(x_p)  for EVERY DOF vector d: checked for random d (all six
+    components, all planes), for d = the constant 1 (total deposited charge = sum of the charges inside the mesh: quintics
+    contain constants, B-splines sum to one), and through locality: a marker touches only the three nodes of its triangle
+    on the four planes of its toroidal interval, and markers outside the mesh deposit nothing."""
+    from oracle import Oracle
+    cfg, RZ, tri, o, _ = cfg0_oracle
+    m = synth.make_markers(cfg, 300)
+    R, Z, phi = m["R"].copy(), m["Z"].copy(), m["phi"]
+    R[:4] = cfg.R0 + 1.4 * cfg.a                       # outside
+    q = synth.uniform(5, 1, 300) - 0.3
+    b = o.deposit(R, Z, phi, q)
+    assert b.shape == (cfg.n_planes, RZ.shape[0], 6)
+    z = Oracle()
+    z.equilibrium_set(**synth.equilibrium_args(cfg))
+    z.species_set(**synth.species_args(cfg))
+    z.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+    rng = np.random.default_rng(3)
+    scale = np.array([1.0, 5.0, 5.0, 25.0, 25.0, 25.0])          # derivative DOFs in their natural units (1/a powers)
+    for trial in range(3):
+        d = rng.normal(size=b.shape) * scale
+        z.fields_set(0, d)
+        F, t = z.gather(R, Z, phi)
+        lhs, rhs = float((b * d).sum()), float((q * F[0]).sum())
+        assert abs(lhs - rhs) < 1e-11 * np.abs(q * F[0]).sum(), (trial, lhs, rhs)
+    one = np.zeros(b.shape)
+    one[:, :, 0] = 1.0
+    inside = o.locate(R, Z) >= 0
+    assert inside.sum() == 296
+    assert abs(float((b * one).sum()) - q[inside].sum()) < 1e-12 * np.abs(q).sum()
+    # locality of one marker
+    i = 10
+    b1 = o.deposit(R[i:i + 1], Z[i:i + 1], phi[i:i + 1], np.ones(1))
+    k, w, dw = o.bspline(phi[i])
+    planes = sorted({(k - 1 + a) % cfg.n_planes for a in range(4)})
+    nodes = sorted(tri[o.locate(R[i:i + 1], Z[i:i + 1])[0]])
+    nz = np.argwhere(np.abs(b1).max(axis=2) > 0)
+    assert sorted(set(nz[:, 0])) == planes and sorted(set(nz[:, 1])) == nodes
+    assert np.abs(o.deposit(R[:4], Z[:4], phi[:4], np.ones(4))).max() == 0.0
