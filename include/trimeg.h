@@ -187,6 +187,16 @@ int trimeg_pullback(trimeg_ctx* ctx);
 int trimeg_density_g2p(trimeg_ctx* ctx, int which, double* out, int memspace);
 int trimeg_f_interp(trimeg_ctx* ctx, double* out, int memspace);
 
+/* Particle-to-grid deposition onto the C1 x B-spline basis ("projecting the quantities stored at the particle
+ * locations ... onto the finite element grid"; what the paper left on the CPU, L288, L372): the transpose of the gather.
+ * dof_out[n_planes][n_nodes][6] (the layout of trimeg_fields_set's `dof`, in `memspace`) is zeroed and receives
+ *   sum over the bound markers of  q_p * B_k(phi_p) * N_{v,c}(R_p, Z_p),
+ * N_{v,c} the nodal basis functions of the element containing the marker, B_k the toroidal cubic B-spline, and the marker
+ * charge q_p = w (quantity 0: density moment) or w u_par (quantity 1: parallel-current moment).  Markers outside the mesh
+ * deposit nothing.  Sums are accumulated with floating-point atomics: the result is reproducible to rounding, not bitwise.
+ * Errors: BAD_ARG, BAD_STATE (mesh, markers), CUDA, OOM. */
+int trimeg_deposit(trimeg_ctx* ctx, int quantity, double* dof_out, int memspace);
+
 /* The -D options this library was built with beyond the defaults ("" for the shipped configuration). */
 const char* trimeg_build_info(void);
 /* Counters of the last trimeg_push_rk4 call: [0] kernel launches, [1] right-hand-side evaluations that took the

@@ -22,7 +22,7 @@ EXPORTS = [
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
     "trimeg_rhs", "trimeg_set_push_variant", "trimeg_push_variant_used", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
     "trimeg_fields_bytes", "trimeg_fields_export", "trimeg_fields_import", "trimeg_build_info", "trimeg_set_gather_mode", "trimeg_gather_kernel_ms",
-    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp",
+    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp", "trimeg_deposit",
 ]
 
 
@@ -73,6 +73,7 @@ def load_library():
     lib.trimeg_pullback.argtypes = [vp]
     lib.trimeg_density_g2p.argtypes = [vp, C.c_int, vp, C.c_int]
     lib.trimeg_f_interp.argtypes = [vp, vp, C.c_int]
+    lib.trimeg_deposit.argtypes = [vp, C.c_int, vp, C.c_int]
     lib.trimeg_build_info.argtypes = []
     lib.trimeg_build_info.restype = C.c_char_p
     lib.trimeg_fields_bytes.argtypes = [vp]
@@ -304,6 +305,15 @@ class Trimeg:
         out = self._scalar_out(host)
         p, ms = _ptr(out)
         self._ck(self._lib.trimeg_f_interp(self._h, p, ms), "trimeg_f_interp")
+        return out
+
+    def deposit(self, quantity=0, host=False):
+        """P2G: -> b[n_planes][n_nodes][6]; quantity 0: charges w, 1: w * u."""
+        t = self._torch
+        shape = (self.n_planes, self.n_nodes, 6)
+        out = np.empty(shape) if host else t.empty(shape, dtype=t.float64, device=self.device)
+        p, ms = _ptr(out)
+        self._ck(self._lib.trimeg_deposit(self._h, int(quantity), p, ms), "trimeg_deposit")
         return out
 
     def sync(self):

@@ -761,6 +761,29 @@ static int per_marker_scalar(trimeg_ctx* ctx, int kind, int which, double* out, 
 int trimeg_density_g2p(trimeg_ctx* ctx, int which, double* out, int memspace) { return per_marker_scalar(ctx, 0, which, out, memspace, "density_g2p"); }
 int trimeg_f_interp(trimeg_ctx* ctx, double* out, int memspace) { return per_marker_scalar(ctx, 1, 0, out, memspace, "f_interp"); }
 
+// particle-to-grid: the transpose of the gather (reading R25)
+int trimeg_deposit(trimeg_ctx* ctx, int quantity, double* dof_out, int memspace) {
+    if (!ctx || !dof_out || quantity < 0 || quantity > 1 || (memspace != TRIMEG_HOST && memspace != TRIMEG_DEVICE)) return fail(ctx, TRIMEG_ERR_BAD_ARG, "deposit: bad argument");
+    if (!ctx->have_mesh || !ctx->have_markers) return fail(ctx, TRIMEG_ERR_BAD_STATE, "deposit: mesh and markers must be set first");
+    CU(cudaSetDevice(ctx->device));
+    const size_t bytes = sizeof(double) * 6 * (size_t)ctx->n_nodes * ctx->P;
+    double* d = dof_out;
+    if (memspace == TRIMEG_HOST) CU(cudaMalloc(&d, bytes));
+    cudaError_t e = cudaMemsetAsync(d, 0, bytes, ctx->stream);
+    if (e == cudaSuccess) {
+        k_deposit<<<blocks_for(ctx->n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->P, quantity, ctx->recs[ctx->cur], ctx->n, ctx->d_tri, ctx->d_RZ, ctx->d_K, ctx->n_nodes, d);
+        e = cudaGetLastError();
+    }
+    if (memspace == TRIMEG_HOST) {
+        if (e == cudaSuccess) e = cudaMemcpyAsync(dof_out, d, bytes, cudaMemcpyDeviceToHost, ctx->stream);
+        cudaError_t e2 = cudaStreamSynchronize(ctx->stream);
+        if (e == cudaSuccess) e = e2;
+        cudaFree(d);
+    }
+    if (e != cudaSuccess) return fail(ctx, TRIMEG_ERR_CUDA, "deposit: %s", cudaGetErrorString(e));
+    return TRIMEG_OK;
+}
+
 int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops) {
     if (!ctx || !tflops) return fail(ctx, TRIMEG_ERR_BAD_ARG, "bench_dfma: null argument");
     CU(cudaSetDevice(ctx->device));

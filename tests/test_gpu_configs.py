@@ -309,3 +309,38 @@ def test_other_g2p_kernels_match_oracle():
     exp = o.push_rk4(after["R"], after["Z"], after["phi"], after["u"], after["w"], m["mu"], m["p"], cfg.dt, 2, status=after["status"])
     for q, k in enumerate(("R", "Z", "phi", "u", "w")):
         assert _rel(res[k], exp[q], cfg.phi_period if k == "phi" else None) < STATE_TOL, k
+
+
+def test_deposit_matches_oracle_and_is_the_transpose_of_the_gather():
+    """trimeg_deposit (P2G onto the C1 x B-spline basis, reading R25) against the oracle's literal transpose of the gather on
+    an unstructured mesh, fresh and pushed stores, both moments; tolerance 1e-11 of the largest entry of each DOF component
+    (sums of ~100 contributions per entry in a different order on each side); and the adjoint identity against the
+    library's OWN gather with a random DOF vector."""
+    import torch
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, nr=8, ntheta=24, n_planes=8, n_markers=6011)
+    RZ, tri, o, g, m = _make(cfg)
+    m["R"][::301] = cfg.R0 + 1.3 * cfg.a
+    d = _dev(m)
+    g.markers_bind(*[d[k] for k in KEYS])
+
+    def check(state, tag):
+        for quantity, q in ((0, state["w"]), (1, state["w"] * state["u"])):
+            ref = o.deposit(state["R"], state["Z"], state["phi"], q)
+            got = g.deposit(quantity, host=True)
+            for c in range(6):
+                assert np.abs(got[:, :, c] - ref[:, :, c]).max() <= 1e-11 * np.abs(ref[:, :, c]).max(), (tag, quantity, c)
+            got_dev = g.deposit(quantity).cpu().numpy()
+            assert np.abs(got_dev - got).max() <= 1e-12 * np.abs(got).max()
+        return got
+
+    check(m, "fresh")
+    g.set_sort_interval(1)
+    g.push_rk4(cfg.dt, 2)
+    state = g.markers_get(host=True)
+    b = check(state, "pushed")           # last: quantity 1
+    rng = np.random.default_rng(5)
+    dof = rng.normal(size=b.shape) * np.array([1.0, 3.0, 3.0, 9.0, 9.0, 9.0])
+    g.fields_set(0, dof)
+    F, t = g.gather(state["R"], state["Z"], state["phi"])
+    q = state["w"] * state["u"]
+    assert abs(float((b * dof).sum()) - float((q * F[0]).sum())) < 1e-10 * np.abs(q * F[0]).sum()
