@@ -489,70 +489,114 @@ __global__ void __launch_bounds__(128) k_f_interp(DevTables tb, EquilP ep, Speci
 //   b[k][v][c] += q_p B_k(phi_p) N_{v,c}(R_p, Z_p),
 // N_{v,c} = the element's nodal basis functions.  With F = m . c (m = the 21 monomials at the point), c = c0 - Nul (K c0_5),
 // c0 = Aplus d_ref, d_ref = T_J d (k_fields_set), the 18 basis values are N = T_J^T Aplus^T (m - S^T K^T Nul^T m).
-// One thread per marker record, atomics on the nodal vector (first version: no per-cell reduction yet).
+// One thread per marker record.  The 72 contributions of a marker (3 nodes x 6 components x 4 planes) go to addresses that
+// depend on its cell (triangle, toroidal interval) only, and the store is in cell order after a push: a warp then holds a
+// few runs of markers of the same cell, each run is summed with warp shuffles and added with ONE atomic per address
+// (a per-cell segmented reduction); a warp with many different cells (unsorted store) falls back to per-marker atomics.
 __global__ void __launch_bounds__(128) k_deposit(DevTables tb, int P, int quantity, const Rec* __restrict__ recs, long long n, const int* __restrict__ tri,
                                                  const double* __restrict__ RZ, const double* __restrict__ Kmat, long long n_nodes, double* __restrict__ out) {
-    long long mi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (mi >= n) return;
-    Rec r;
-    rec_load(recs, mi, r);
-    const int t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
-    if (t < 0) return;
-    const TriGeom g = tb.geom[t];
-    double xi, eta, w[4], dw[4];
-    ref_coords(g, r.y[0], r.y[1], xi, eta);
-    const int k = bspline_weights(tb.tor, r.y[2], w, dw);
-    // monomials xi^i eta^j at j-major index off_j + i
-    double m[21];
-    {
-        double xp[6], ep[6];
-        xp[0] = ep[0] = 1.0;
+    constexpr unsigned FULL = 0xffffffffu;
+    const long long mi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    int t = -1, k = 0, key = -1;
+    int nd[3] = {0, 0, 0};
+    double N[18], w[4] = {0.0, 0.0, 0.0, 0.0}, charge = 0.0;
 #pragma unroll
-        for (int i = 1; i < 6; ++i) { xp[i] = xp[i - 1] * xi; ep[i] = ep[i - 1] * eta; }
-        int idx = 0;
+    for (int q = 0; q < 18; ++q) N[q] = 0.0;
+    if (mi < n) {
+        Rec r;
+        rec_load(recs, mi, r);
+        t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
+        if (t >= 0) {
+            const TriGeom g = tb.geom[t];
+            double xi, eta, dw[4];
+            ref_coords(g, r.y[0], r.y[1], xi, eta);
+            k = bspline_weights(tb.tor, r.y[2], w, dw);
+            key = t * P + k;
+            charge = quantity == 0 ? r.y[4] : r.y[4] * r.y[3];
+            // monomials xi^i eta^j at j-major index off_j + i
+            double m[21];
+            {
+                double xp[6], ep[6];
+                xp[0] = ep[0] = 1.0;
 #pragma unroll
-        for (int j = 0; j < 6; ++j)
+                for (int i = 1; i < 6; ++i) { xp[i] = xp[i - 1] * xi; ep[i] = ep[i - 1] * eta; }
+                int idx = 0;
 #pragma unroll
-            for (int i = 0; i < 6 - j; ++i) m[idx++] = xp[i] * ep[j];
-    }
-    double y[3] = {0.0, 0.0, 0.0};
+                for (int j = 0; j < 6; ++j)
 #pragma unroll
-    for (int i = 0; i < 21; ++i) { y[0] = fma(c_Nul[i * 3], m[i], y[0]); y[1] = fma(c_Nul[i * 3 + 1], m[i], y[1]); y[2] = fma(c_Nul[i * 3 + 2], m[i], y[2]); }
-    const int qi[6] = {5, 6 + 4, 11 + 3, 15 + 2, 18 + 1, 20};
-    const double* K = Kmat + (long long)t * 18;
+                    for (int i = 0; i < 6 - j; ++i) m[idx++] = xp[i] * ep[j];
+            }
+            double y[3] = {0.0, 0.0, 0.0};
 #pragma unroll
-    for (int mm = 0; mm < 6; ++mm) m[qi[mm]] -= fma(y[0], K[mm], fma(y[1], K[6 + mm], y[2] * K[12 + mm]));
-    double a[18];
+            for (int i = 0; i < 21; ++i) { y[0] = fma(c_Nul[i * 3], m[i], y[0]); y[1] = fma(c_Nul[i * 3 + 1], m[i], y[1]); y[2] = fma(c_Nul[i * 3 + 2], m[i], y[2]); }
+            const int qi[6] = {5, 6 + 4, 11 + 3, 15 + 2, 18 + 1, 20};
+            const double* K = Kmat + (long long)t * 18;
 #pragma unroll
-    for (int q = 0; q < 18; ++q) {
-        double s = 0.0;
+            for (int mm = 0; mm < 6; ++mm) m[qi[mm]] -= fma(y[0], K[mm], fma(y[1], K[6 + mm], y[2] * K[12 + mm]));
+            double a[18];
 #pragma unroll
-        for (int i = 0; i < 21; ++i) s = fma(c_Aplus[i * 18 + q], m[i], s);
-        a[q] = s;
-    }
-    const int nd[3] = {tri[3 * t], tri[3 * t + 1], tri[3 * t + 2]};
-    const double x0 = RZ[2 * nd[0]], y0 = RZ[2 * nd[0] + 1];
-    const double j11 = RZ[2 * nd[1]] - x0, j21 = RZ[2 * nd[1] + 1] - y0, j12 = RZ[2 * nd[2]] - x0, j22 = RZ[2 * nd[2] + 1] - y0;
-    const double charge = quantity == 0 ? r.y[4] : r.y[4] * r.y[3];
+            for (int q = 0; q < 18; ++q) {
+                double s = 0.0;
 #pragma unroll
-    for (int v = 0; v < 3; ++v) {
-        const double* av = a + 6 * v;
-        double N[6];
-        N[0] = av[0];
-        N[1] = fma(j11, av[1], j12 * av[2]);
-        N[2] = fma(j21, av[1], j22 * av[2]);
-        N[3] = fma(j11 * j11, av[3], fma(j11 * j12, av[4], j12 * j12 * av[5]));
-        N[4] = fma(2.0 * j11 * j21, av[3], fma(j11 * j22 + j21 * j12, av[4], 2.0 * j12 * j22 * av[5]));
-        N[5] = fma(j21 * j21, av[3], fma(j21 * j22, av[4], j22 * j22 * av[5]));
+                for (int i = 0; i < 21; ++i) s = fma(c_Aplus[i * 18 + q], m[i], s);
+                a[q] = s;
+            }
+            nd[0] = tri[3 * t]; nd[1] = tri[3 * t + 1]; nd[2] = tri[3 * t + 2];
+            const double x0 = RZ[2 * nd[0]], y0 = RZ[2 * nd[0] + 1];
+            const double j11 = RZ[2 * nd[1]] - x0, j21 = RZ[2 * nd[1] + 1] - y0, j12 = RZ[2 * nd[2]] - x0, j22 = RZ[2 * nd[2] + 1] - y0;
 #pragma unroll
-        for (int pa = 0; pa < 4; ++pa) {
-            int pl = k - 1 + pa;
-            if (pl < 0) pl += P; else if (pl >= P) pl -= P;
-            double* base = out + ((long long)pl * n_nodes + nd[v]) * 6;
-            const double qw = charge * w[pa];
-#pragma unroll
-            for (int c = 0; c < 6; ++c) atomicAdd(base + c, qw * N[c]);
+            for (int v = 0; v < 3; ++v) {
+                const double* av = a + 6 * v;
+                N[6 * v + 0] = av[0];
+                N[6 * v + 1] = fma(j11, av[1], j12 * av[2]);
+                N[6 * v + 2] = fma(j21, av[1], j22 * av[2]);
+                N[6 * v + 3] = fma(j11 * j11, av[3], fma(j11 * j12, av[4], j12 * j12 * av[5]));
+                N[6 * v + 4] = fma(2.0 * j11 * j21, av[3], fma(j11 * j22 + j21 * j12, av[4], 2.0 * j12 * j22 * av[5]));
+                N[6 * v + 5] = fma(j21 * j21, av[3], fma(j21 * j22, av[4], j22 * j22 * av[5]));
+            }
         }
+    }
+    auto addr = [&](int v, int pa, int kk, const int* nodes) {
+        int pl = kk - 1 + pa;
+        if (pl < 0) pl += P; else if (pl >= P) pl -= P;
+        return out + ((long long)pl * n_nodes + nodes[v]) * 6;
+    };
+    const int prevk = __shfl_up_sync(FULL, key, 1);
+    const unsigned starts = __ballot_sync(FULL, lane == 0 || prevk != key);
+    if (__popc(starts) <= 16) {
+        // segmented reduction over the runs of equal cells (contiguous lane ranges), all runs at once: after the five steps
+        // the first lane of every run holds the run's sum
+        const unsigned above = lane == 31 ? 0u : (starts & ~((2u << lane) - 1u));
+        const int run_end = above ? __ffs(above) - 1 : 32;
+        const bool leader = ((starts >> lane) & 1u) && key >= 0;
+#pragma unroll
+        for (int v = 0; v < 3; ++v)
+#pragma unroll
+            for (int pa = 0; pa < 4; ++pa) {
+                const double qw = charge * w[pa];
+                double* base = addr(v, pa, k, nd);
+#pragma unroll
+                for (int c = 0; c < 6; ++c) {
+                    double sum = qw * N[6 * v + c];
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const double up = __shfl_down_sync(FULL, sum, o);
+                        if (lane + o < run_end) sum += up;
+                    }
+                    if (leader) atomicAdd(base + c, sum);
+                }
+            }
+    } else if (t >= 0) {
+#pragma unroll
+        for (int v = 0; v < 3; ++v)
+#pragma unroll
+            for (int pa = 0; pa < 4; ++pa) {
+                double* base = addr(v, pa, k, nd);
+                const double qw = charge * w[pa];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) atomicAdd(base + c, qw * N[6 * v + c]);
+            }
     }
 }
 
