@@ -28,8 +28,15 @@ struct GatherMap {   // cell numbering of the gather: super-cell (patch, window)
         return ((patch * nwin + w) * GT + tl) * GW + kl;
     }
 };
-struct __align__(16) GPoint { double R, Z, phi; int id, tri; };   // one point in cell order (32 B)
+struct __align__(32) GPoint { double R, Z, phi; int id, tri; };   // one point in cell order (32 B = one sector)
 static_assert(sizeof(GPoint) == 32, "GPoint");
+// 256-bit global accesses (sm_100: LDG/STG.256): a 32-byte record is one request and one full sector
+TRIMEG_DI void ld256(const void* p, double& a, double& b, double& c, double& d) {
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
+TRIMEG_DI void st256(void* p, double a, double b, double c, double d) {
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
 
 // Which path?  A strided sample of runs of 32 consecutive points: if most neighbours share a cell the caller's order is
 // already clustered and the direct kernel (coefficients through L1/L2) is the faster one; otherwise the points are binned.
@@ -79,9 +86,7 @@ __global__ void __launch_bounds__(256) k_gather_scatter(long long n, const doubl
     if (i >= n || *flag != 2) return;
     const int key = keys[i];
     const int pos = offs[key] + atomicAdd(fill + key, 1);
-    double2* dst = reinterpret_cast<double2*>(pts + pos);
-    dst[0] = make_double2(R[i], Z[i]);
-    dst[1] = make_double2(phi[i], __hiloint2double(tris[i], (int)i));     // (id, tri) in the low and high word
+    st256(pts + pos, R[i], Z[i], phi[i], __hiloint2double(tris[i], (int)i));     // (id, tri) in the low and high word
     inv[i] = pos;
 }
 
@@ -151,10 +156,9 @@ k_gather_staged(DevTables tb, GatherMap gm, int nunits, int NPP, const int* __re
         for (int pos = begin + tid; pos < end; pos += GTHREADS) {
             GPoint p;
             {
-                const double2* src = reinterpret_cast<const double2*>(pts + pos);
-                const double2 a = __ldcs(src), b = __ldcs(src + 1);
-                p.R = a.x; p.Z = a.y; p.phi = b.x;
-                p.id = __double2loint(b.y); p.tri = __double2hiint(b.y);
+                double it;
+                ld256(pts + pos, p.R, p.Z, p.phi, it);
+                p.id = __double2loint(it); p.tri = __double2hiint(it);
             }
             const int tl = p.tri - patch * GT;
             const TriGeom& g = geom[tl];
@@ -165,9 +169,8 @@ k_gather_staged(DevTables tb, GatherMap gm, int nunits, int NPP, const int* __re
             gather_cell<true, double>(ld, xi, eta, bw, dw, acc);
             Fields f;
             to_fields(g, acc, f);
-            double2* o = reinterpret_cast<double2*>(res + 8ll * pos);
-            __stcs(o, make_double2(f.P, f.PR)); __stcs(o + 1, make_double2(f.PZ, f.Pp));
-            __stcs(o + 2, make_double2(f.A, f.AR)); __stcs(o + 3, make_double2(f.AZ, f.Ap));
+            st256(res + 8ll * pos, f.P, f.PR, f.PZ, f.Pp);
+            st256(res + 8ll * pos + 4, f.A, f.AR, f.AZ, f.Ap);
         }
         __syncthreads();                                  // everybody is done with stage s
     }
@@ -181,8 +184,9 @@ __global__ void __launch_bounds__(256) k_gather_unsort(long long n, const int* _
     const int t = tris[i];
     double2 a = make_double2(0, 0), b = a, c = a, d = a;
     if (t >= 0) {
-        const double2* r = reinterpret_cast<const double2*>(res + 8ll * inv[i]);
-        a = __ldcs(r); b = __ldcs(r + 1); c = __ldcs(r + 2); d = __ldcs(r + 3);
+        const double* r = res + 8ll * inv[i];
+        ld256(r, a.x, a.y, b.x, b.y);
+        ld256(r + 4, c.x, c.y, d.x, d.y);
     }
     out[i] = a.x; out[n + i] = a.y; out[2 * n + i] = b.x; out[3 * n + i] = b.y;
     out[4 * n + i] = c.x; out[5 * n + i] = c.y; out[6 * n + i] = d.x; out[7 * n + i] = d.y;
