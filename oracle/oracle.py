@@ -60,6 +60,7 @@ def _load():
         lib.orc_pullback.argtypes = [C.c_void_p, C.c_int64] + [_d] * 7 + [_i]
         lib.orc_density_g2p.argtypes = [C.c_void_p, C.c_int, C.c_int64, _d, _d, _d, _d]
         lib.orc_f_interp.argtypes = [C.c_void_p, C.c_int64] + [_d] * 6
+        lib.orc_gather_gyro.argtypes = [C.c_void_p, C.c_int64, _d, _d, _d, _d, C.c_int, _d, _i]
         lib.orc_deposit.argtypes = [C.c_void_p, C.c_int64, _d, _d, _d, _d, _d]
         lib.orc_push_rk4.argtypes = [C.c_void_p, C.c_int64] + [_d] * 7 + [_i, C.c_double, C.c_int32]
         _lib = lib
@@ -191,6 +192,15 @@ class Oracle:
         out = np.zeros(R.shape[0])
         self._ck(self._lib.orc_f_interp(self._h, R.shape[0], R, Z, phi, u, mu, out), "f_interp")
         return out
+
+    def gather_gyro(self, R, Z, phi, rho, npts):
+        """N-point gyro-average of the gather -> (out[8][n], tri[n] of the gyrocentres)."""
+        R, Z, phi, rho = [_f(x) for x in (R, Z, phi, rho)]
+        n = R.shape[0]
+        out = np.zeros((8, n))
+        tri = np.zeros(n, dtype=np.int32)
+        self._ck(self._lib.orc_gather_gyro(self._h, n, R, Z, phi, rho, int(npts), out, tri), "gather_gyro")
+        return out, tri
 
     def deposit(self, R, Z, phi, q):
         """P2G: -> b[n_planes][n_nodes][6], the transpose of the gather applied to the marker charges q."""

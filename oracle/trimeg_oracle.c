@@ -48,6 +48,9 @@
  *       transpose of O3.  b[k][v][c] = sum_p q_p N_{v,c}(R_p, Z_p) B_k(phi_p)
  *       with N_{v,c} the element's nodal basis functions (the interpolant of the
  *       unit DOF vector) and B_k the toroidal spline (reading R25).
+ *   O12 N-point gyro-average of the gather (the <...> of Eq.(4)-(6), L49-55; "switched
+ *       off" in the paper's runs, L320): the mean of O3 over N points on the gyro-ring
+ *       of radius rho in the poloidal plane around the gyrocentre (reading R26).
  *
  * Parity unpinned (choices the paper does not fix and nothing external can
  * check): the element family itself (R1), the unit system (R8), linear vs
@@ -472,6 +475,27 @@ int orc_deposit(orc *c, int64_t n, const double *R, const double *Z, const doubl
                 out[((size_t)pl * c->n_nodes + node) * 6 + comp] += q[m] * w[a] * v[0];
             }
         }
+    }
+    return 0;
+}
+
+/* --------------------------------------------------------------- O12 ---- */
+/* <F>(R, Z, phi) = (1/N) sum_j F(R + rho cos t_j, Z + rho sin t_j, phi), t_j = 2 pi j / N: the ring in the poloidal plane
+ * (the magnetic field is mostly toroidal), all N points on the same toroidal angle; ring points outside the mesh
+ * contribute zero (O9).  tri_out = triangle of the gyrocentre itself.  out[8][n] as in orc_gather. */
+int orc_gather_gyro(orc *c, int64_t n, const double *R, const double *Z, const double *phi, const double *rho, int npts, double *out, int32_t *tri_out) {
+    if (!c || !c->head || npts < 1) return -1;
+#pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < n; m++) {
+        double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (int j = 0; j < npts; j++) {
+            double th = 2.0 * 3.14159265358979323846 * (double)j / (double)npts;
+            double Rj = R[m] + rho[m] * cos(th), Zj = Z[m] + rho[m] * sin(th), f[4];
+            int64_t t = locate_one(c, Rj, Zj, 0);
+            for (int which = 0; which < 2; which++) { field_at(c, which, t, Rj, Zj, phi[m], f); for (int q = 0; q < 4; q++) acc[4 * which + q] += f[q]; }
+        }
+        for (int q = 0; q < 8; q++) out[(size_t)q * n + m] = acc[q] / (double)npts;
+        if (tri_out) tri_out[m] = (int32_t)locate_one(c, R[m], Z[m], 0);
     }
     return 0;
 }

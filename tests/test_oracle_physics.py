@@ -440,3 +440,43 @@ def test_P20_deposit_is_the_transpose_of_the_gather(cfg0_oracle):
     nz = np.argwhere(np.abs(b1).max(axis=2) > 0)
     assert sorted(set(nz[:, 0])) == planes and sorted(set(nz[:, 1])) == nodes
     assert np.abs(o.deposit(R[:4], Z[:4], phi[:4], np.ones(4))).max() == 0.0
+
+
+# ------------------------------------------------------------------------------------------- O12: gyro-average
+def test_P21_gyro_average_of_polynomial_fields_has_a_closed_form():
+    """Pin P21 for the N-point gyro-average (reading R26).  On fields that are global polynomials of degree <= 4 (inside the
+    element space, all planes equal) the ring average is known in closed form for N >= 5 points: with x = R - R0, z = Z,
+        <x^2> = x^2 + rho^2/2,  <x z> = x z,  <x^3> = x^3 + 3 x rho^2/2,  <x^2 z^2> = x^2 z^2 + (x^2 + z^2) rho^2/2 + rho^4/8,
+    the average of the gradient is the gradient of the average; rho = 0 and N = 1 give the plain gather; an odd-order
+    term survives with too few points (N = 2 on x^3 is exact only by symmetry of that ring: negative control with N = 3 on
+    x^2 z^2, which needs N >= 5)."""
+    cfg, o, m = _smooth_case(P=8, n=300, zero=True)
+    RZ, tri = synth.make_mesh(cfg)
+    X, Zc = RZ[:, 0] - cfg.R0, RZ[:, 1]
+    # Phi = x^2 z^2 + 0.5 x^3 ; A = x z + 2 x^2   (nodal value, gradient, Hessian)
+    dP = np.stack([X**2 * Zc**2 + 0.5 * X**3, 2 * X * Zc**2 + 1.5 * X**2, 2 * X**2 * Zc, 2 * Zc**2 + 3 * X, 4 * X * Zc, 2 * X**2], -1)
+    dA = np.stack([X * Zc + 2 * X**2, Zc + 4 * X, X, 4 * np.ones_like(X), np.ones_like(X), np.zeros_like(X)], -1)
+    o.fields_set(0, np.broadcast_to(dP, (8,) + dP.shape).copy())
+    o.fields_set(1, np.broadcast_to(dA, (8,) + dA.shape).copy())
+    rr = np.hypot(m["R"] - cfg.R0, m["Z"])
+    keep = (rr < 0.6 * cfg.a) & (rr > 0.35 * cfg.a)       # the whole ring (rho <= 0.05 = a/8) stays inside the annulus
+    R, Z, phi = m["R"][keep], m["Z"][keep], m["phi"][keep]
+    rho = 0.02 + 0.03 * synth.uniform(9, 1, R.shape[0])
+    x, z = R - cfg.R0, Z
+    for N in (5, 8):
+        g, t = o.gather_gyro(R, Z, phi, rho, N)
+        expP = x**2 * z**2 + (x**2 + z**2) * rho**2 / 2 + rho**4 / 8 + 0.5 * (x**3 + 1.5 * x * rho**2)
+        expPR = 2 * x * z**2 + x * rho**2 + 0.5 * (3 * x**2 + 1.5 * rho**2)
+        expPZ = 2 * x**2 * z + z * rho**2
+        expA = x * z + 2 * (x**2 + rho**2 / 2)
+        for got, exp in ((g[0], expP), (g[1], expPR), (g[2], expPZ), (g[4], expA), (g[5], z + 4 * x), (g[6], x)):
+            assert np.abs(got - exp).max() < 1e-12 * max(np.abs(exp).max(), 1e-3), N
+        assert np.abs(g[3]).max() < 1e-15 and np.abs(g[7]).max() < 1e-15      # all planes equal: no phi dependence
+    g3, _ = o.gather_gyro(R, Z, phi, rho, 3)
+    assert np.abs(g3[0] - expP).max() > 1e-9                                   # negative control: three points are too few for x^2 z^2
+    plain, tp = o.gather(R, Z, phi)
+    g1, t1 = o.gather_gyro(R, Z, phi, 0 * rho, 6)
+    assert np.abs(g1 - plain).max() < 1e-14 * np.abs(plain).max() and np.array_equal(t1, tp)      # six equal terms summed and divided by six
+    g1b, _ = o.gather_gyro(R + rho, Z, phi, rho, 1)                            # one point: the ring point at angle 0
+    pl2, _ = o.gather(R + 2 * rho, Z, phi)
+    assert np.abs(g1b - pl2).max() < 1e-14 * np.abs(pl2).max()
