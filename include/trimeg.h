@@ -105,6 +105,14 @@ size_t trimeg_fields_bytes(const trimeg_ctx* ctx);
 int trimeg_fields_export(trimeg_ctx* ctx, void* dst_device, size_t bytes);
 int trimeg_fields_import(trimeg_ctx* ctx, const void* src_device, size_t bytes);
 
+/* N-point gyro-average of the gather (the <...> of Eq.(4)-(6); off in the paper's runs, L320; DESIGN.md
+ * reading R26): out[q][i] = mean over j = 0 .. npts-1 of the gathered quantity q at (R_i + rho_i cos(2 pi j / npts),
+ * Z_i + rho_i sin(2 pi j / npts), phi_i); ring points outside the mesh contribute zero; rho_i >= 0 is the gyro-radius of
+ * point i in the units of R, Z; 1 <= npts <= 64.  out and tri_out (triangle of the gyrocentre itself, nullable) as in
+ * trimeg_gather.  Errors: BAD_ARG, BAD_STATE (no mesh), CUDA, OOM. */
+int trimeg_gather_gyro(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi, const double* rho,
+                       int32_t npts, double* out, int32_t* tri_out, int memspace);
+
 /* How trimeg_gather runs on the device.  Two paths: the direct kernel (one thread per point, coefficients through L1/L2:
  * fastest when the caller's points are already clustered by cell) and the staged path (the library bins the points by cell,
  * stages the coefficient blocks in shared memory by TMA and un-sorts the results; csrc/trimeg_gather.cuh: 4x faster on

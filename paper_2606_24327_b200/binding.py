@@ -22,7 +22,7 @@ EXPORTS = [
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
     "trimeg_rhs", "trimeg_set_push_variant", "trimeg_push_variant_used", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
     "trimeg_fields_bytes", "trimeg_fields_export", "trimeg_fields_import", "trimeg_build_info", "trimeg_set_gather_mode", "trimeg_gather_kernel_ms",
-    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp", "trimeg_deposit",
+    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp", "trimeg_deposit", "trimeg_gather_gyro",
 ]
 
 
@@ -73,6 +73,7 @@ def load_library():
     lib.trimeg_pullback.argtypes = [vp]
     lib.trimeg_density_g2p.argtypes = [vp, C.c_int, vp, C.c_int]
     lib.trimeg_f_interp.argtypes = [vp, vp, C.c_int]
+    lib.trimeg_gather_gyro.argtypes = [vp, i64, vp, vp, vp, vp, i32, vp, vp, C.c_int]
     lib.trimeg_deposit.argtypes = [vp, C.c_int, vp, C.c_int]
     lib.trimeg_build_info.argtypes = []
     lib.trimeg_build_info.restype = C.c_char_p
@@ -225,6 +226,20 @@ class Trimeg:
         pt, _ = _ptr(tri_out)
         self._ck(self._lib.trimeg_gather(self._h, n, pR, pZ, pP, po, pt, ms), "trimeg_gather")
         return out, tri_out
+
+    def gather_gyro(self, R, Z, phi, rho, npts):
+        """N-point gyro-average of the gather; all numpy (HOST) or all CUDA tensors (DEVICE) -> (out[8,n], tri[n])."""
+        ptrs = [_ptr(a) for a in (R, Z, phi, rho)]
+        ms = ptrs[0][1]
+        assert all(q[1] == ms for q in ptrs)
+        n = int(R.shape[0])
+        if ms == HOST:
+            out, tri = np.empty((8, n)), np.empty(n, dtype=np.int32)
+        else:
+            t = self._torch
+            out, tri = t.empty((8, n), dtype=t.float64, device=self.device), t.empty(n, dtype=t.int32, device=self.device)
+        self._ck(self._lib.trimeg_gather_gyro(self._h, n, *[q[0] for q in ptrs], int(npts), _ptr(out)[0], _ptr(tri)[0], ms), "trimeg_gather_gyro")
+        return out, tri
 
     # ---- markers
     def scratch_bytes(self, n):

@@ -451,6 +451,35 @@ int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, 
     return TRIMEG_OK;
 }
 
+int trimeg_gather_gyro(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi, const double* rho, int32_t npts, double* out,
+                       int32_t* tri_out, int memspace) {
+    if (!ctx || n < 0 || npts < 1 || npts > 64 || (n > 0 && (!R || !Z || !phi || !rho || !out)) || (memspace != TRIMEG_HOST && memspace != TRIMEG_DEVICE))
+        return fail(ctx, TRIMEG_ERR_BAD_ARG, "gather_gyro: bad argument (1 <= npts <= 64)");
+    if (!ctx->have_mesh) return fail(ctx, TRIMEG_ERR_BAD_STATE, "gather_gyro: call trimeg_mesh_load first");
+    if (n == 0) return TRIMEG_OK;
+    CU(cudaSetDevice(ctx->device));
+    if (memspace == TRIMEG_DEVICE) {
+        k_gather_gyro<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, n, R, Z, phi, rho, npts, out, tri_out);
+        KCHECK();
+        return TRIMEG_OK;
+    }
+    double* d = nullptr;
+    int* dt = nullptr;
+    CU(cudaMalloc(&d, sizeof(double) * 12 * (size_t)n));
+    if (cudaMalloc(&dt, sizeof(int) * (size_t)n) != cudaSuccess) { cudaFree(d); return fail(ctx, TRIMEG_ERR_OOM, "gather_gyro: out of device memory"); }
+    cudaError_t e = cudaSuccess;
+    auto step = [&](cudaError_t x) { if (e == cudaSuccess) e = x; };
+    const double* src[4] = {R, Z, phi, rho};
+    for (int q = 0; q < 4; ++q) step(cudaMemcpyAsync(d + q * n, src[q], sizeof(double) * n, cudaMemcpyHostToDevice, ctx->stream));
+    if (e == cudaSuccess) { k_gather_gyro<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, n, d, d + n, d + 2 * n, d + 3 * n, npts, d + 4 * n, dt); step(cudaGetLastError()); }
+    step(cudaMemcpyAsync(out, d + 4 * n, sizeof(double) * 8 * n, cudaMemcpyDeviceToHost, ctx->stream));
+    if (tri_out) step(cudaMemcpyAsync(tri_out, dt, sizeof(int) * n, cudaMemcpyDeviceToHost, ctx->stream));
+    step(cudaStreamSynchronize(ctx->stream));
+    cudaFree(d); cudaFree(dt);
+    if (e != cudaSuccess) return fail(ctx, TRIMEG_ERR_CUDA, "gather_gyro: %s", cudaGetErrorString(e));
+    return TRIMEG_OK;
+}
+
 int trimeg_set_gather_mode(trimeg_ctx* ctx, int32_t mode) {
     if (!ctx || mode < 0 || mode > 2) return fail(ctx, TRIMEG_ERR_BAD_ARG, "set_gather_mode: 0 automatic, 1 direct, 2 staged");
     ctx->gather_mode = mode;

@@ -216,6 +216,33 @@ __global__ void __launch_bounds__(256, 4) k_gather(DevTables tb, long long n, co
     if (tri_out) tri_out[m] = t < 0 ? -1 : tb.geom[t].orig;
 }
 
+// N-point gyro-average of the gather (the <...> of Eq.(4)-(6); switched off in the paper's runs, L320;
+// reading R26): mean over npts points of the ring of radius rho in the poloidal plane around (R, Z), same toroidal angle; ring
+// points outside the mesh contribute zero.  The ring points of one gyrocentre lie within a few elements of each other, so
+// every point after the first is found by an edge walk from its predecessor's triangle.
+__global__ void __launch_bounds__(256, 3) k_gather_gyro(DevTables tb, long long n, const double* __restrict__ R, const double* __restrict__ Z,
+                                                        const double* __restrict__ phi, const double* __restrict__ rho, int npts, double* __restrict__ out,
+                                                        int* __restrict__ tri_out) {
+    long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    const double r0 = R[m], z0 = Z[m], ph = phi[m], rh = rho[m];
+    double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int t = -1;
+    for (int j = 0; j < npts; ++j) {
+        double sn, cs;
+        sincospi(2.0 * (double)j / (double)npts, &sn, &cs);
+        const double rj = fma(rh, cs, r0), zj = fma(rh, sn, z0);
+        t = t >= 0 ? locate_walk(tb.bg, tb.geom, t, rj, zj) : locate_box(tb.bg, tb.geom, rj, zj);
+        Fields f;
+        gather_at(tb, t, rj, zj, ph, f);
+        acc[0] += f.P; acc[1] += f.PR; acc[2] += f.PZ; acc[3] += f.Pp; acc[4] += f.A; acc[5] += f.AR; acc[6] += f.AZ; acc[7] += f.Ap;
+    }
+    const double inv = 1.0 / (double)npts;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) out[(long long)q * n + m] = acc[q] * inv;
+    if (tri_out) { const int tc = locate_box(tb.bg, tb.geom, r0, z0); tri_out[m] = tc < 0 ? -1 : tb.geom[tc].orig; }
+}
+
 // one right-hand-side evaluation for one marker, fields through L1/L2; updates the triangle hint; returns 1 if outside
 __device__ __forceinline__ int stage_simple(const DevTables& tb, const EquilP& ep, const SpeciesP& sp, int& t, double R, double Z,
                                             double phi, double u, double w, double mu, double p, double d[5]) {

@@ -344,3 +344,27 @@ def test_deposit_matches_oracle_and_is_the_transpose_of_the_gather():
     F, t = g.gather(state["R"], state["Z"], state["phi"])
     q = state["w"] * state["u"]
     assert abs(float((b * dof).sum()) - float((q * F[0]).sum())) < 1e-10 * np.abs(q * F[0]).sum()
+
+
+@pytest.mark.parametrize("npts", [1, 4, 8])
+def test_gather_gyro_matches_oracle(npts):
+    """trimeg_gather_gyro (N-point gyro-average of the gather, reading R26) against the oracle on the unstructured EM mesh:
+    ring radii from zero to several elements, rings that leave the mesh through the outer boundary and through the hole,
+    HOST and DEVICE buffers.  Tolerance 1e-12 per quantity (the cos / sin of the ring angles differ in the last bit)."""
+    import torch
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, n_markers=20_011)
+    RZ, tri, o, g, m = _make(cfg)
+    R, Z, phi = m["R"], m["Z"], m["phi"]
+    rho = 0.08 * cfg.a * synth.uniform(31, 1, R.shape[0])
+    rho[::5] = 0.0
+    ref, tref = o.gather_gyro(R, Z, phi, rho, npts)
+    out, tout = g.gather_gyro(R, Z, phi, rho, npts)
+    for q in range(8):
+        assert _rel(out[q], ref[q]) < GATHER_TOL, (q, _rel(out[q], ref[q]))
+    assert (tout == tref).mean() > 0.999
+    d = _dev({"R": R, "Z": Z, "phi": phi, "rho": rho})
+    out2, tout2 = g.gather_gyro(d["R"], d["Z"], d["phi"], d["rho"], npts)
+    assert np.array_equal(out2.cpu().numpy(), out) and np.array_equal(tout2.cpu().numpy(), tout)
+    if npts == 1:
+        plain, _ = g.gather(R + rho, Z, phi)
+        assert np.abs(out - plain).max() <= 1e-13 * np.abs(plain).max()
