@@ -44,6 +44,7 @@ def _load():
         lib.orc_num_threads.restype = C.c_int
         lib.orc_set_num_threads.argtypes = [C.c_int]
         lib.orc_equilibrium_set.argtypes = [C.c_void_p] + [C.c_double] * 6 + [C.c_int]
+        lib.orc_equilibrium_set_numeric.argtypes = [C.c_void_p, C.c_int, C.c_int] + [C.c_double] * 7 + [_d]
         lib.orc_species_set.argtypes = [C.c_void_p] + [C.c_double] * 6 + [C.c_int, C.c_int]
         lib.orc_mesh_load.argtypes = [C.c_void_p, C.c_int64, _d, C.c_int64, _i, C.c_int32, C.c_double]
         lib.orc_fields_set.argtypes = [C.c_void_p, C.c_int, _d]
@@ -103,6 +104,12 @@ class Oracle:
 
     def equilibrium_set(self, R0, a, B0, q0, q1, q2, qbar_sqrt=1):
         self._ck(self._lib.orc_equilibrium_set(self._h, R0, a, B0, q0, q1, q2, int(qbar_sqrt)), "equilibrium_set")
+
+    def equilibrium_set_numeric(self, nR, nZ, Rmin, Rmax, Zmin, Zmax, F, R0, a, coef):
+        """psi as tensor-product cubic B-spline coefficients coef[nR+3][nZ+3]; F = R B_phi; R0, a for the Eq.(8) profiles."""
+        coef = _f(coef)
+        assert coef.shape == (nR + 3, nZ + 3), coef.shape
+        self._ck(self._lib.orc_equilibrium_set_numeric(self._h, int(nR), int(nZ), Rmin, Rmax, Zmin, Zmax, F, R0, a, coef), "equilibrium_set_numeric")
 
     def species_set(self, qom, kappa_n=0.0, kappa_T=0.0, w_n=0.3, w_T=0.3, r0=0.0, bstar_exact=1, weight_mode=0):
         self._ck(self._lib.orc_species_set(self._h, qom, kappa_n, kappa_T, w_n, w_T, r0, int(bstar_exact),

@@ -51,6 +51,9 @@
  *   O12 N-point gyro-average of the gather (the <...> of Eq.(4)-(6), L49-55; "switched
  *       off" in the paper's runs, L320): the mean of O3 over N points on the gyro-ring
  *       of radius rho in the poloidal plane around the gyrocentre (reading R26).
+ *   O13 numeric equilibrium (L87 "equilibrium variables are represented using B-splines", L121, L142-146: the
+ *       paper's B-spline library): psi(R, Z) as a tensor-product uniform cubic B-spline on a rectangle, F = R B_phi
+ *       constant; B = grad psi x grad phi + F grad phi and everything O5 derives from it (reading R27).
  *
  * Parity unpinned (choices the paper does not fix and nothing external can
  * check): the element family itself (R1), the unit system (R8), linear vs
@@ -75,6 +78,7 @@
 
 typedef struct {
     /* O5 */ double R0, a, B0, q0, q1, q2; int qbar_sqrt, have_eq;
+    /* O13 */ int eq_numeric, gnR, gnZ; double gRmin, gRmax, gZmin, gZmax, gF; double *gcoef;
     /* O6/O7 */ double qom, kappa_n, kappa_T, w_n, w_T, r0; int bstar_exact, weight_mode, have_sp;
     /* mesh */ int64_t n_nodes, n_tri; double *RZ; int32_t *tri; int P; double period;
     /* O1 */ long double *LU; int *piv; double *org; double *hh;
@@ -101,7 +105,7 @@ static long double dmono_l(int i, int j, int dx, int dy, long double x, long dou
 orc *orc_create(void) { if (!mono_ready) mono_init(); return (orc *)calloc(1, sizeof(orc)); }
 void orc_destroy(orc *c) {
     if (!c) return;
-    free(c->RZ); free(c->tri); free(c->LU); free(c->piv); free(c->org); free(c->hh);
+    free(c->gcoef); free(c->RZ); free(c->tri); free(c->LU); free(c->piv); free(c->org); free(c->hh);
     free(c->head); free(c->list); free(c->coef[0]); free(c->coef[1]); free(c);
 }
 int orc_num_threads(void) {
@@ -120,7 +124,18 @@ void orc_set_num_threads(int n) {
 }
 
 int orc_equilibrium_set(orc *c, double R0, double a, double B0, double q0, double q1, double q2, int qbar_sqrt) {
-    c->R0 = R0; c->a = a; c->B0 = B0; c->q0 = q0; c->q1 = q1; c->q2 = q2; c->qbar_sqrt = qbar_sqrt; c->have_eq = 1;
+    c->R0 = R0; c->a = a; c->B0 = B0; c->q0 = q0; c->q1 = q1; c->q2 = q2; c->qbar_sqrt = qbar_sqrt; c->have_eq = 1; c->eq_numeric = 0;
+    return 0;
+}
+/* O13: coef[(nR+3)][(nZ+3)] of psi on [Rmin,Rmax] x [Zmin,Zmax] with nR x nZ intervals, F = R B_phi; R0, a: axis and minor
+ * radius for the Eq.(8) profiles (their radial coordinate stays r = |(R - R0, Z)|) */
+int orc_equilibrium_set_numeric(orc *c, int nR, int nZ, double Rmin, double Rmax, double Zmin, double Zmax, double F, double R0, double a, const double *coef) {
+    if (!c || nR < 1 || nZ < 1 || !(Rmax > Rmin) || !(Zmax > Zmin) || !coef) return -1;
+    free(c->gcoef);
+    size_t n = (size_t)(nR + 3) * (nZ + 3);
+    c->gcoef = (double *)malloc(sizeof(double) * n); memcpy(c->gcoef, coef, sizeof(double) * n);
+    c->gnR = nR; c->gnZ = nZ; c->gRmin = Rmin; c->gRmax = Rmax; c->gZmin = Zmin; c->gZmax = Zmax; c->gF = F;
+    c->R0 = R0; c->a = a; c->eq_numeric = 1; c->have_eq = 1;
     return 0;
 }
 int orc_species_set(orc *c, double qom, double kn, double kT, double wn, double wT, double r0, int bstar_exact, int weight_mode) {
@@ -365,7 +380,48 @@ int orc_gather(orc *c, int64_t n, const double *R, const double *Z, const double
 
 /* ---------------------------------------------------------------- O5 ---- */
 typedef struct { double r, q, qbar, psi1, psi2; double B[3]; /* R,phi,Z */ double Bmag; double b[3]; double gradB[3]; double curlb[3]; double F; } equil;
+/* uniform cubic B-spline pieces on one interval, fraction s in [0,1]: values, first and second derivatives w.r.t. s */
+static void cubic_pieces(double s, double *w, double *d1, double *d2) {
+    double t = 1 - s;
+    w[0] = t * t * t / 6; w[1] = (3 * s * s * s - 6 * s * s + 4) / 6; w[2] = (-3 * s * s * s + 3 * s * s + 3 * s + 1) / 6; w[3] = s * s * s / 6;
+    d1[0] = -t * t / 2; d1[1] = (3 * s * s - 4 * s) / 2; d1[2] = (-3 * s * s + 2 * s + 1) / 2; d1[3] = s * s / 2;
+    d2[0] = t; d2[1] = 3 * s - 2; d2[2] = -3 * s + 1; d2[3] = s;
+}
+/* psi_R, psi_Z, psi_RR, psi_RZ, psi_ZZ of the tensor-product spline  psi = sum_ab coef[i+a][j+b] B_a(s) B_b(t)  */
+static void psi_spline(const orc *c, double R, double Z, double *p5) {
+    double hR = (c->gRmax - c->gRmin) / c->gnR, hZ = (c->gZmax - c->gZmin) / c->gnZ;
+    double uR = (R - c->gRmin) / hR, uZ = (Z - c->gZmin) / hZ;
+    int i = (int)floor(uR), j = (int)floor(uZ);
+    if (i < 0) i = 0; if (i > c->gnR - 1) i = c->gnR - 1;
+    if (j < 0) j = 0; if (j > c->gnZ - 1) j = c->gnZ - 1;
+    double wa[4], da[4], dda[4], wb[4], db[4], ddb[4];
+    cubic_pieces(uR - i, wa, da, dda); cubic_pieces(uZ - j, wb, db, ddb);
+    for (int q = 0; q < 5; q++) p5[q] = 0;
+    for (int a = 0; a < 4; a++) for (int b = 0; b < 4; b++) {
+        double cf = c->gcoef[(size_t)(i + a) * (c->gnZ + 3) + (j + b)];
+        p5[0] += cf * da[a] * wb[b] / hR; p5[1] += cf * wa[a] * db[b] / hZ;
+        p5[2] += cf * dda[a] * wb[b] / (hR * hR); p5[3] += cf * da[a] * db[b] / (hR * hZ); p5[4] += cf * wa[a] * ddb[b] / (hZ * hZ);
+    }
+}
 static void equil_eval(const orc *c, double R, double Z, equil *e) {
+    if (c->eq_numeric) {   /* O13: the same derivation as below from the spline's derivatives of psi */
+        double x = R - c->R0, r = sqrt(x * x + Z * Z), p5[5];
+        psi_spline(c, R, Z, p5);
+        double pR = p5[0], pZ = p5[1], pRR = p5[2], pRZ = p5[3], pZZ = p5[4], F = c->gF;
+        double BR = -pZ / R, BZ = pR / R, Bp = F / R;
+        double BR_R = -pRZ / R + pZ / (R * R), BR_Z = -pZZ / R, BZ_R = pRR / R - pR / (R * R), BZ_Z = pRZ / R, Bp_R = -F / (R * R), Bp_Z = 0;
+        double B = sqrt(BR * BR + BZ * BZ + Bp * Bp);
+        double B_R = (BR * BR_R + BZ * BZ_R + Bp * Bp_R) / B, B_Z = (BR * BR_Z + BZ * BZ_Z + Bp * Bp_Z) / B;
+        double bR = BR / B, bp = Bp / B, bZ = BZ / B;
+        double bR_Z = BR_Z / B - BR * B_Z / (B * B), bZ_R = BZ_R / B - BZ * B_R / (B * B);
+        double bp_R = Bp_R / B - Bp * B_R / (B * B), bp_Z = Bp_Z / B - Bp * B_Z / (B * B);
+        (void)BZ_Z;
+        e->r = r; e->q = 0; e->qbar = 0; e->psi1 = 0; e->psi2 = 0; e->F = F;
+        e->B[0] = BR; e->B[1] = Bp; e->B[2] = BZ; e->Bmag = B; e->b[0] = bR; e->b[1] = bp; e->b[2] = bZ;
+        e->gradB[0] = B_R; e->gradB[1] = 0; e->gradB[2] = B_Z;
+        e->curlb[0] = -bp_Z; e->curlb[1] = bR_Z - bZ_R; e->curlb[2] = bp_R + bp / R;
+        return;
+    }
     double x = R - c->R0, r = sqrt(x * x + Z * Z), xa = r / c->a;
     double q = c->q0 + c->q1 * xa + c->q2 * xa * xa, dq = (c->q1 + 2 * c->q2 * xa) / c->a;
     double s = 1, ds = 0;

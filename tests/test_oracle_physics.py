@@ -480,3 +480,93 @@ def test_P21_gyro_average_of_polynomial_fields_has_a_closed_form():
     g1b, _ = o.gather_gyro(R + rho, Z, phi, rho, 1)                            # one point: the ring point at angle 0
     pl2, _ = o.gather(R + 2 * rho, Z, phi)
     assert np.abs(g1b - pl2).max() < 1e-14 * np.abs(pl2).max()
+
+
+# ------------------------------------------------------------------------------------------- O13: numeric equilibrium
+def _cubic_exact_coefs(f, nR, nZ, Rmin, Rmax, Zmin, Zmax):
+    """B-spline coefficients that reproduce a function that is a cubic in R and a cubic in Z EXACTLY: the textbook
+    quasi-interpolant c = f - h^2 f''/6 applied in each direction (exact on cubics), with derivatives by exact finite
+    differences of cubics.  Knot i of the coefficient array sits at Rmin + (i - 1) h."""
+    hR, hZ = (Rmax - Rmin) / nR, (Zmax - Zmin) / nZ
+    Rk = Rmin + (np.arange(nR + 3) - 1) * hR
+    Zk = Zmin + (np.arange(nZ + 3) - 1) * hZ
+    RR, ZZ = np.meshgrid(Rk, Zk, indexing="ij")
+    d2R = lambda g: (g(RR + hR, ZZ) - 2 * g(RR, ZZ) + g(RR - hR, ZZ))          # = h^2 f_RR exactly for cubics
+    d2Z = lambda g: (g(RR, ZZ + hZ) - 2 * g(RR, ZZ) + g(RR, ZZ - hZ))
+    f0 = f(RR, ZZ)
+    fR = d2R(f)
+    fZ = d2Z(f)
+    fRZ = (f(RR + hR, ZZ + hZ) - 2 * f(RR, ZZ + hZ) + f(RR - hR, ZZ + hZ)) - 2 * fR + (f(RR + hR, ZZ - hZ) - 2 * f(RR, ZZ - hZ) + f(RR - hR, ZZ - hZ))
+    return f0 - fR / 6 - fZ / 6 + fRZ / 36
+
+
+def test_P22_numeric_equilibrium_closed_form_and_convergence_to_the_analytic_one(cfg0_oracle):
+    """Pin P22 (reading R27).  (a) a flux function that is cubic in R and in Z is reproduced exactly by the spline, so B, grad B
+    and curl b have closed forms: B_R = -psi_Z/R, B_Z = psi_R/R, B_phi = F/R, checked directly, with div B = 0, grad B and
+    curl b by central differences of the returned B and b (the P6 checks), at points that straddle knot lines.
+    (b) the spline interpolant of the ANALYTIC circular equilibrium's psi converges to the analytic oracle's B, grad B,
+    curl b at fourth / second order in the knot spacing (values / second-derivative quantities)."""
+    from oracle import Oracle
+    from scipy.interpolate import RectBivariateSpline  # noqa: F401  (scipy is only used for (b))
+    cfg, RZ, tri, o, _ = cfg0_oracle
+    al, be, ga, de, R0, F = 0.8, 1.3, 0.4, -0.6, 1.1, 2.3
+    psi = lambda R, Z: al * (R - R0) ** 2 + be * Z**2 + ga * (R - R0) ** 3 + de * (R - R0) * Z**2 + 0.2 * (R - R0) ** 2 * Z**3
+    z = Oracle()
+    box = (0.6, 1.7, -0.5, 0.6)
+    coef = _cubic_exact_coefs(psi, 11, 9, *box)
+    z.equilibrium_set_numeric(11, 9, *box, F, R0, 0.4, coef)
+    rng = np.random.default_rng(8)
+    h = 1e-5
+    for _ in range(12):
+        R, Z = rng.uniform(0.7, 1.6), rng.uniform(-0.4, 0.5)
+        x = R - R0
+        pR = 2 * al * x + 3 * ga * x**2 + de * Z**2 + 0.4 * x * Z**3
+        pZ = 2 * be * Z + 2 * de * x * Z + 0.6 * x**2 * Z**2
+        e = z.equil(R, Z)
+        assert abs(e["B_R"] + pZ / R) < 1e-13 and abs(e["B_Z"] - pR / R) < 1e-13 and abs(e["B_phi"] - F / R) < 1e-15
+        assert abs(e["B"] - np.sqrt(pR**2 + pZ**2 + F**2) / R) < 1e-13
+        eRp, eRm, eZp, eZm = z.equil(R + h, Z), z.equil(R - h, Z), z.equil(R, Z + h), z.equil(R, Z - h)
+        d = lambda k, p_, m_: (p_[k] - m_[k]) / (2 * h)
+        divB = ((R + h) * eRp["B_R"] - (R - h) * eRm["B_R"]) / (2 * h) / R + d("B_Z", eZp, eZm)
+        assert abs(divB) < 1e-8
+        assert abs(d("B", eRp, eRm) - e["gradB_R"]) < 1e-8 and abs(d("B", eZp, eZm) - e["gradB_Z"]) < 1e-8
+        curl = np.array([-d("b_phi", eZp, eZm), d("b_R", eZp, eZm) - d("b_Z", eRp, eRm),
+                         ((R + h) * eRp["b_phi"] - (R - h) * eRm["b_phi"]) / (2 * h) / R])
+        assert np.abs(curl - np.array([e["curlb_R"], e["curlb_phi"], e["curlb_Z"]])).max() < 1e-8
+    # (b) convergence to the analytic circular equilibrium of config 0
+    from scipy.integrate import quad
+    from scipy.interpolate import make_interp_spline
+    psi1 = lambda r: o.equil(cfg.R0 + r, 0.0)["psi1"]
+    rr = np.linspace(0.0, 1.6 * cfg.a, 400)
+    pr = np.concatenate([[0.0], np.cumsum([quad(psi1, a_, b_, epsabs=1e-14)[0] for a_, b_ in zip(rr[:-1], rr[1:])])])
+    psi_r = make_interp_spline(rr, pr, k=5)
+    errs = []
+    for n in (24, 48):
+        box = (cfg.R0 - 1.2 * cfg.a, cfg.R0 + 1.2 * cfg.a, -1.2 * cfg.a, 1.2 * cfg.a)
+        hR = (box[1] - box[0]) / n
+        # interpolating spline coefficients through samples at the knots (library routine): not-a-knot is not what the
+        # uniform spline space wants at the ends, so fit on an extended grid and keep a window
+        Rk = box[0] + (np.arange(n + 3) - 1) * hR
+        Zk = box[2] + (np.arange(n + 3) - 1) * hR
+        RR, ZZ = np.meshgrid(Rk, Zk, indexing="ij")
+        samples = psi_r(np.hypot(RR - cfg.R0, ZZ))
+        # solve the tridiagonal (1,4,1)/6 systems in both directions with natural-ish ends (end effects stay at the border)
+        M = (np.diag(np.full(n + 3, 4.0)) + np.diag(np.ones(n + 2), 1) + np.diag(np.ones(n + 2), -1)) / 6
+        M[0, :3] = [1, -2, 1]; M[-1, -3:] = [1, -2, 1]
+        rhs = samples.copy(); rhs[0, :] = 0; rhs[-1, :] = 0
+        c1 = np.linalg.solve(M, rhs)
+        rhs2 = c1.T.copy(); rhs2[0, :] = 0; rhs2[-1, :] = 0
+        coef = np.linalg.solve(M, rhs2).T
+        z.equilibrium_set_numeric(n, n, *box, cfg.B0 * cfg.R0, cfg.R0, cfg.a, coef)
+        e_max = np.zeros(3)
+        for r_, th in [(0.3, 0.4), (0.5, 2.0), (0.7, 4.0), (0.6, 5.5)]:
+            R, Z = cfg.R0 + r_ * cfg.a * np.cos(th), r_ * cfg.a * np.sin(th)
+            en, ea = z.equil(R, Z), o.equil(R, Z)
+            e_max[0] = max(e_max[0], abs(en["B"] - ea["B"]) / ea["B"])
+            e_max[1] = max(e_max[1], abs(en["gradB_R"] - ea["gradB_R"]), abs(en["gradB_Z"] - ea["gradB_Z"]))
+            e_max[2] = max(e_max[2], abs(en["curlb_phi"] - ea["curlb_phi"]))
+        errs.append(e_max)
+    print("numeric equilibrium vs analytic, n = 24 / 48:", errs)
+    assert errs[1][0] < 2e-6 and errs[0][0] / errs[1][0] > 5          # |B| from first derivatives of psi: third order or better
+    assert errs[1][1] < 1e-3 and errs[1][1] < errs[0][1]              # grad B, curl b from second derivatives of the fitted psi: small
+    assert errs[1][2] < 1e-3 and errs[1][2] < errs[0][2]              # and decreasing (their rate is set by the crude end conditions of this fit)
