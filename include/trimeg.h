@@ -62,6 +62,21 @@ typedef struct {
 } trimeg_equil;
 int trimeg_equilibrium_set(trimeg_ctx* ctx, const trimeg_equil* eq);
 
+/* Numeric equilibrium ("equilibrium variables are represented using B-splines", L121, L142-146: the paper's
+ * B-spline library; reading R27): the poloidal flux psi(R, Z) as a tensor-product uniform cubic B-spline,
+ *   psi = sum_{a,b=0..3} psi_coef[i + a][j + b] B_a(s) B_b(t),  i = floor((R - Rmin) / hR), s its fraction (likewise j, t in Z),
+ * psi_coef[nR + 3][nZ + 3] in HOST memory (copied), hR = (Rmax - Rmin) / nR; outside the rectangle the edge polynomial is
+ * continued.  B = grad psi x grad phi + F grad phi with constant F = R B_phi; R0 and a only serve the Eq.(8) profiles (their
+ * radial coordinate stays r = |(R - R0, Z)|) and the triangle numbering.  Replaces a previous equilibrium of either kind.
+ * With a numeric equilibrium trimeg_push_rk4 runs variant 1 (one thread per marker); trimeg_push_variant_used says so.
+ * Errors: BAD_ARG, CUDA, OOM. */
+typedef struct {
+    int32_t nR, nZ;
+    double Rmin, Rmax, Zmin, Zmax;
+    double F, R0, a;
+} trimeg_equil_grid;
+int trimeg_equilibrium_set_numeric(trimeg_ctx* ctx, const trimeg_equil_grid* grid, const double* psi_coef);
+
 /* Species and equilibrium profiles.  qom = q_s/m_s in the normalised units of Eq.(2)-(6) (sign = charge sign);
  * Eq.(8) (L314): H(r)/H(r0) = exp[-kappa_H w_H (a/R0) tanh((r - r0)/(w_H a))] for H = n, T.
  * bstar_exact = 1: bstar = Bstar / Bstar_par with Bstar = B + (m/q) u curl b (default); 0: the literal expression printed at L53.

@@ -22,7 +22,7 @@ EXPORTS = [
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
     "trimeg_rhs", "trimeg_set_push_variant", "trimeg_push_variant_used", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
     "trimeg_fields_bytes", "trimeg_fields_export", "trimeg_fields_import", "trimeg_build_info", "trimeg_set_gather_mode", "trimeg_gather_kernel_ms",
-    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp", "trimeg_deposit", "trimeg_gather_gyro",
+    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp", "trimeg_deposit", "trimeg_gather_gyro", "trimeg_equilibrium_set_numeric",
 ]
 
 
@@ -33,6 +33,11 @@ class TrimegError(RuntimeError):
 class _Equil(C.Structure):
     _fields_ = [("R0", C.c_double), ("a", C.c_double), ("B0", C.c_double), ("q0", C.c_double), ("q1", C.c_double),
                 ("q2", C.c_double), ("qbar_sqrt", C.c_int32)]
+
+
+class _EquilGrid(C.Structure):
+    _fields_ = [("nR", C.c_int32), ("nZ", C.c_int32), ("Rmin", C.c_double), ("Rmax", C.c_double), ("Zmin", C.c_double),
+                ("Zmax", C.c_double), ("F", C.c_double), ("R0", C.c_double), ("a", C.c_double)]
 
 
 class _Species(C.Structure):
@@ -64,6 +69,7 @@ def load_library():
     lib.trimeg_last_error.argtypes = [vp]
     lib.trimeg_last_error.restype = C.c_char_p
     lib.trimeg_equilibrium_set.argtypes = [vp, C.POINTER(_Equil)]
+    lib.trimeg_equilibrium_set_numeric.argtypes = [vp, C.POINTER(_EquilGrid), vp]
     lib.trimeg_species_set.argtypes = [vp, C.POINTER(_Species)]
     lib.trimeg_mesh_load.argtypes = [vp, i64, vp, i64, vp, i32, dbl]
     lib.trimeg_fields_set.argtypes = [vp, C.c_int, vp, C.c_int]
@@ -155,6 +161,12 @@ class Trimeg:
     def equilibrium_set(self, R0, a, B0, q0, q1, q2, qbar_sqrt=1):
         e = _Equil(R0, a, B0, q0, q1, q2, int(qbar_sqrt))
         self._ck(self._lib.trimeg_equilibrium_set(self._h, C.byref(e)), "trimeg_equilibrium_set")
+
+    def equilibrium_set_numeric(self, nR, nZ, Rmin, Rmax, Zmin, Zmax, F, R0, a, coef):
+        coef = np.ascontiguousarray(coef, dtype=np.float64)
+        assert coef.shape == (nR + 3, nZ + 3), coef.shape
+        gs = _EquilGrid(int(nR), int(nZ), Rmin, Rmax, Zmin, Zmax, F, R0, a)
+        self._ck(self._lib.trimeg_equilibrium_set_numeric(self._h, C.byref(gs), coef.ctypes.data), "trimeg_equilibrium_set_numeric")
 
     def species_set(self, qom, kappa_n=0.0, kappa_T=0.0, w_n=0.3, w_T=0.3, r0=0.0, bstar_exact=1, weight_mode=0):
         s = _Species(qom, kappa_n, kappa_T, w_n, w_T, r0, int(bstar_exact), int(weight_mode))

@@ -26,6 +26,7 @@ struct trimeg_ctx {
     std::string err;
     bool have_eq = false, have_sp = false, have_mesh = false, have_markers = false;
     EquilP ep{};
+    double* d_psi = nullptr;     // numeric equilibrium: spline coefficients of psi (library-owned)
     SpeciesP sp{};
     trimeg_equil eq_in{};
     trimeg_species sp_in{};
@@ -163,6 +164,7 @@ int trimeg_destroy(trimeg_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     for (auto& st : ctx->ev) for (auto& e : st) if (e) cudaEventDestroy(e);
     for (auto& e : ctx->gev) if (e) cudaEventDestroy(e);
+    cudaFree(ctx->d_psi);
     free_mesh(ctx);
     delete ctx;
     return TRIMEG_OK;
@@ -184,8 +186,33 @@ int trimeg_equilibrium_set(trimeg_ctx* ctx, const trimeg_equil* eq) {
     EquilP& e = ctx->ep;
     e.R0 = eq->R0; e.B0 = eq->B0; e.F = eq->B0 * eq->R0; e.F2 = e.F * e.F; e.inv_a = 1.0 / eq->a; e.inv_R0sq = 1.0 / (eq->R0 * eq->R0);
     e.q0 = eq->q0; e.q1 = eq->q1; e.q2 = eq->q2; e.qbar_sqrt = eq->qbar_sqrt ? 1 : 0;
+    e.kind = 0; e.psi = nullptr;
     ctx->have_eq = true;
     if (ctx->have_sp) derive_species(ctx);   // the profile scalars of Eq.(8) depend on a and R0
+    invalidate_step_state(ctx);
+    return TRIMEG_OK;
+}
+
+int trimeg_equilibrium_set_numeric(trimeg_ctx* ctx, const trimeg_equil_grid* g, const double* psi_coef) {
+    if (!ctx || !g || !psi_coef) return fail(ctx, TRIMEG_ERR_BAD_ARG, "equilibrium_set_numeric: null argument");
+    if (g->nR < 1 || g->nZ < 1 || !(g->Rmax > g->Rmin) || !(g->Zmax > g->Zmin) || !(g->Rmin > 0) || !std::isfinite(g->F) || g->F == 0 || !(g->R0 > 0) ||
+        !(g->a > 0) || (long long)(g->nR + 3) * (g->nZ + 3) > 100000000LL)
+        return fail(ctx, TRIMEG_ERR_BAD_ARG, "equilibrium_set_numeric: need nR, nZ >= 1, 0 < Rmin < Rmax, Zmin < Zmax, finite nonzero F, R0 > 0, a > 0");
+    CU(cudaSetDevice(ctx->device));
+    CU(cudaStreamSynchronize(ctx->stream));
+    cudaFree(ctx->d_psi); ctx->d_psi = nullptr;
+    const size_t bytes = sizeof(double) * (size_t)(g->nR + 3) * (g->nZ + 3);
+    CU(cudaMalloc(&ctx->d_psi, bytes));
+    CU(cudaMemcpy(ctx->d_psi, psi_coef, bytes, cudaMemcpyHostToDevice));
+    ctx->eq_in = trimeg_equil{};
+    ctx->eq_in.R0 = g->R0; ctx->eq_in.a = g->a; ctx->eq_in.B0 = g->F / g->R0;
+    EquilP& e = ctx->ep;
+    e = EquilP{};
+    e.R0 = g->R0; e.B0 = g->F / g->R0; e.F = g->F; e.F2 = g->F * g->F; e.inv_a = 1.0 / g->a; e.inv_R0sq = 1.0 / (g->R0 * g->R0);
+    e.kind = 1; e.psi = ctx->d_psi; e.nR = g->nR; e.nZ = g->nZ; e.Rmin = g->Rmin; e.Zmin = g->Zmin;
+    e.inv_hR = g->nR / (g->Rmax - g->Rmin); e.inv_hZ = g->nZ / (g->Zmax - g->Zmin);
+    ctx->have_eq = true;
+    if (ctx->have_sp) derive_species(ctx);
     invalidate_step_state(ctx);
     return TRIMEG_OK;
 }
@@ -654,7 +681,7 @@ int trimeg_push_rk4(trimeg_ctx* ctx, double dt, int32_t nsteps) {
     for (int s = 0; s < nsteps; ++s) {
         const bool timed = (nsteps - s <= trimeg_ctx::EV_STEPS);
         cudaEvent_t* const sev = ctx->ev[timed ? ctx->ev_steps : 0];
-        if (ctx->variant == 0 && ctx->tiled_ok) {
+        if (ctx->variant == 0 && ctx->tiled_ok && !ctx->ep.kind) {
             const bool need_sort = ctx->force_sort || !ctx->order_valid || (ctx->sort_every > 0 && ctx->steps_since_sort >= ctx->sort_every);
             if (!ctx->k1_valid || ctx->key_dt != dt || (need_sort && !ctx->keys_valid)) {
                 // k1 = f(y_n) and the keys of the half-step points, through the global tables (first step after a bind, or after
@@ -711,7 +738,7 @@ const char* trimeg_build_info(void) { return TRIMEG_BUILD_DEFS; }
 int trimeg_push_variant_used(trimeg_ctx* ctx, int32_t* out) {
     if (!ctx || !out) return fail(ctx, TRIMEG_ERR_BAD_ARG, "push_variant_used: null argument");
     if (!ctx->have_mesh) return fail(ctx, TRIMEG_ERR_BAD_STATE, "push_variant_used: call trimeg_mesh_load first");
-    *out = (ctx->variant == 0 && ctx->tiled_ok) ? 0 : 1;
+    *out = (ctx->variant == 0 && ctx->tiled_ok && !ctx->ep.kind) ? 0 : 1;
     return TRIMEG_OK;
 }
 

@@ -251,7 +251,7 @@ __device__ __forceinline__ int stage_simple(const DevTables& tb, const EquilP& e
     gather_at(tb, t, R, Z, phi, f);
     FieldsG<double> fg;
     fields_to_g(f, u, fg);
-    rhs_eval<double>(ep, sp, R, Z, u, w, mu, p, fg, d);
+    rhs_eval<double, true>(ep, sp, R, Z, u, w, mu, p, fg, d);
     return t < 0;
 }
 
@@ -503,7 +503,7 @@ __global__ void __launch_bounds__(128) k_f_interp(DevTables tb, EquilP ep, Speci
     Fields f;
     gather_at(tb, t, r.y[0], r.y[1], r.y[2], f);
     Equil<double> e;
-    equil_eval<double>(ep, r.y[0], r.y[1], e);
+    equil_eval<double, true>(ep, r.y[0], r.y[1], e);
     const double thT = profile_th(sp, sp.two_inv_wT_a, e.r), thn = profile_th(sp, sp.two_inv_wn_a, e.r);
     const double iT = exp(sp.cT * thT), dens = exp(-sp.cn * thn);
     const double v = r.y[3] - sp.qom * f.A;

@@ -26,6 +26,12 @@ using ::fma;
 struct EquilP {
     double R0, B0, F, F2, inv_a, inv_R0sq, q0, q1, q2;   // F = B0 R0, F2 = F^2
     int qbar_sqrt;
+    // kind 1: numeric equilibrium, psi(R, Z) as tensor-product uniform cubic B-spline coefficients psi[nR + 3][nZ + 3] on
+    // [Rmin, Rmin + nR hR] x [Zmin, Zmin + nZ hZ] (reading R27); F, F2, R0 as above
+    int kind;
+    const double* psi;
+    int nR, nZ;
+    double Rmin, Zmin, inv_hR, inv_hZ;
 };
 struct SpeciesP {
     double qom, kappa;                 // q/m and m/q
@@ -265,8 +271,47 @@ template <class T>
 struct Equil {
     T B, iB, iR, bR, bp, bZ, gBR, gBZ, J, r, c, s;
 };
-template <class T>
+// Numeric equilibrium: B = grad psi x grad phi + F grad phi from the spline's first and second derivatives of psi, through
+// the same identities as the analytic one (H = sqrt(|grad psi|^2 + F^2), B = H / R, b = (-psi_Z, F, psi_R) / H,
+// grad B = grad H / R - B e_R / R, (curl B)_phi = (psi_R / R - laplace psi) / R).  The oracle differentiates b instead.
+TRIMEG_DI void equil_eval_numeric(const EquilP& e, double R, double Z, Equil<double>& o) {
+    const double uR = (R - e.Rmin) * e.inv_hR, uZ = (Z - e.Zmin) * e.inv_hZ;
+    const int i = max(0, min(e.nR - 1, (int)floor(uR))), j = max(0, min(e.nZ - 1, (int)floor(uZ)));
+    double wa[4], da[4], ca[4], wb[4], db[4], cb[4];
+    auto pieces = [](double s, double* w, double* d1, double* d2) {
+        const double t = 1.0 - s, s2 = s * s, t2 = t * t;
+        w[0] = t2 * t * (1.0 / 6.0); w[3] = s2 * s * (1.0 / 6.0);
+        w[1] = fma(s2, fma(0.5, s, -1.0), 2.0 / 3.0); w[2] = fma(t2, fma(0.5, t, -1.0), 2.0 / 3.0);
+        d1[0] = -0.5 * t2; d1[3] = 0.5 * s2; d1[1] = fma(1.5, s2, -2.0 * s); d1[2] = -fma(1.5, t2, -2.0 * t);
+        d2[0] = t; d2[1] = fma(3.0, s, -2.0); d2[2] = fma(3.0, t, -2.0); d2[3] = s;
+    };
+    pieces(uR - (double)i, wa, da, ca);
+    pieces(uZ - (double)j, wb, db, cb);
+    double pR = 0, pZ = 0, pRR = 0, pRZ = 0, pZZ = 0;
+    const double* base = e.psi + (long long)i * (e.nZ + 3) + j;
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+        double v = 0, vz = 0, vzz = 0;     // sums over the Z direction for row a
+#pragma unroll
+        for (int b = 0; b < 4; ++b) { const double c = __ldg(base + (long long)a * (e.nZ + 3) + b); v = fma(c, wb[b], v); vz = fma(c, db[b], vz); vzz = fma(c, cb[b], vzz); }
+        pR = fma(da[a], v, pR); pRR = fma(ca[a], v, pRR); pZ = fma(wa[a], vz, pZ); pRZ = fma(da[a], vz, pRZ); pZZ = fma(wa[a], vzz, pZZ);
+    }
+    pR *= e.inv_hR; pZ *= e.inv_hZ; pRR *= e.inv_hR * e.inv_hR; pRZ *= e.inv_hR * e.inv_hZ; pZZ *= e.inv_hZ * e.inv_hZ;
+    const double H2 = fma(pR, pR, fma(pZ, pZ, e.F2)), iH = rsqrt_nr(H2), H = H2 * iH, iR = rcp_nr(R);
+    const double B = H * iR;
+    o.B = B; o.iB = R * iH; o.iR = iR;
+    o.bR = -(pZ * iH); o.bZ = pR * iH; o.bp = e.F * iH;
+    const double HR = fma(pR, pRR, pZ * pRZ) * iH, HZ = fma(pR, pRZ, pZ * pZZ) * iH;
+    o.gBR = fma(HR, iR, -(B * iR)); o.gBZ = HZ * iR;
+    o.J = fma(pR, iR, -(pRR + pZZ)) * iR;
+    const double x = R - e.R0, r2 = fma(x, x, Z * Z), ir = rsqrt_nr(r2);
+    o.r = r2 * ir; o.c = x * ir; o.s = Z * ir;
+}
+// NUM: whether this instantiation may meet a numeric equilibrium (the tiled phase kernel never does: the library runs
+// variant 1 then, so its hot loop carries no branch and no extra code for it)
+template <class T, bool NUM = false>
 TRIMEG_DI void equil_eval(const EquilP& e, T R, T Z, Equil<T>& o) {
+    if (NUM && e.kind) { equil_eval_numeric(e, R, Z, o); return; }
     const T x = R - T(e.R0);
     const T r2 = fma(x, x, Z * Z);
     const T ir = rsqrt_nr(r2), r = r2 * ir;
@@ -309,9 +354,9 @@ struct RhsPre {
     Equil<T> e;
     T dlnT, dlnn, iT;     // d ln T / dr, d ln n / dr, 1 / T(r)
 };
-template <class T>
+template <class T, bool NUM = false>
 TRIMEG_DI void rhs_pre(const EquilP& ep, const SpeciesP& sp, T R, T Z, RhsPre<T>& o) {
-    equil_eval(ep, R, Z, o.e);
+    equil_eval<T, NUM>(ep, R, Z, o.e);
     const T dr = o.e.r - T(sp.r0);
     const T thT = fma(T(-2.0), rcp_nr(exp_nr(dr * T(sp.two_inv_wT_a)) + T(1.0)), T(1.0));
     T thn = thT;
@@ -359,10 +404,10 @@ TRIMEG_DI void rhs_post(const SpeciesP& sp, const RhsPre<T>& pre, T u, T w, T mu
     const T pw = sp.weight_mode ? (p - w) : p;
     d[4] = -((pw * iBss) * fma(eR, glR, fma(eZ, glZ, Sqg * (u * pre.iT))));
 }
-template <class T>
+template <class T, bool NUM = false>
 TRIMEG_DI void rhs_eval(const EquilP& ep, const SpeciesP& sp, T R, T Z, T u, T w, T mu, T p, const FieldsG<T>& f, T d[5]) {
     RhsPre<T> pre;
-    rhs_pre(ep, sp, R, Z, pre);
+    rhs_pre<T, NUM>(ep, sp, R, Z, pre);
     rhs_post(sp, pre, u, w, mu, p, f, d);
 }
 

@@ -368,3 +368,45 @@ def test_gather_gyro_matches_oracle(npts):
     if npts == 1:
         plain, _ = g.gather(R + rho, Z, phi)
         assert np.abs(out - plain).max() <= 1e-13 * np.abs(plain).max()
+
+
+def test_numeric_equilibrium_rhs_and_push_match_oracle():
+    """Numeric (B-spline) equilibrium, reading R27: a shaped flux function given as tensor-product cubic B-spline coefficients
+    (elongated, with a cubic shift term), the same coefficients to the oracle and the library; trimeg_rhs (1e-11) and 10 RK4
+    steps (1e-10) against the oracle; the library runs variant 1 with it and says so; switching back to the analytic
+    equilibrium restores the tiled path."""
+    from oracle import Oracle
+    from paper_2606_24327_b200.binding import Trimeg
+    from test_oracle_physics import _cubic_exact_coefs
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, nr=10, ntheta=30, n_planes=8, n_markers=7001)
+    RZ, tri = synth.make_mesh(cfg)
+    dphi, dap = synth.make_fields(cfg, RZ)
+    m = synth.make_markers(cfg)
+    R0, a, F = cfg.R0, cfg.a, cfg.B0 * cfg.R0
+    k = cfg.B0 / (2 * 1.6)                                     # psi ~ B0 r^2 / (2 q) near the axis, q ~ 1.6
+    psi = lambda R, Z: k * ((R - R0) ** 2 + Z**2 / 1.4**2) + 0.15 * k / a * (R - R0) ** 3 - 0.1 * k / a * (R - R0) * Z**2
+    box = (R0 - 1.3 * a, R0 + 1.3 * a, -1.3 * a, 1.3 * a)
+    nR, nZ = 37, 41
+    coef = _cubic_exact_coefs(psi, nR, nZ, *box)
+    o, g = Oracle(), Trimeg(0)
+    for x in (o, g):
+        x.equilibrium_set_numeric(nR, nZ, *box, F, R0, a, coef)
+        x.species_set(**synth.species_args(cfg))
+        x.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+        x.fields_set(0, dphi)
+        x.fields_set(1, dap)
+    d = _dev(m)
+    g.markers_bind(*[d[k_] for k_ in KEYS])
+    out = g.rhs(host=True)
+    ref, _ = o.rhs(*[m[k_] for k_ in KEYS])
+    for q in range(5):
+        assert _rel(out[q], ref[q]) < 1e-11, (q, _rel(out[q], ref[q]))
+    _check_push(o, g, m, cfg, 0.05, 10, 0, sort_every=1)
+    assert g.push_variant_used() == 1
+    fi = g.f_interp(host=True)
+    res = g.markers_get(host=True)
+    assert np.abs(fi - o.f_interp(res["R"], res["Z"], res["phi"], res["u"], m["mu"])).max() <= 1e-12 * np.abs(fi).max()
+    for x in (o, g):
+        x.equilibrium_set(**synth.equilibrium_args(cfg))
+    _check_push(o, g, m, cfg, 0.05, 10, 0, sort_every=1)
+    assert g.push_variant_used() == 0
