@@ -451,23 +451,8 @@ k_phase_ws(DevTables tb, TileTables tt, EquilP ep, SpeciesP sp, const Rec* src, 
                     slot = sl;
                     double w[4], dw[4], g8[8];
                     bspline_from_s<double>(tb.tor, sf, w, dw);
-#ifdef TRIMEG_GATHER_ROLL2   // tuning: the four planes as a rolled loop over two pairs (fewer live registers, half the code)
-                    {
-                        const unsigned gb = smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE);
-#pragma unroll
-                        for (int q = 0; q < 8; ++q) g8[q] = 0.0;
-#pragma unroll 1
-                        for (int h = 0; h < 2; ++h) {
-                            const double wa = h ? w[2] : w[0], wb = h ? w[3] : w[1], da = h ? dw[2] : dw[0], db = h ? dw[3] : dw[1];
-                            LdShared l0{gb + (unsigned)(2 * h * PLANE_STRIDE * sizeof(double))}, l1{gb + (unsigned)((2 * h + 1) * PLANE_STRIDE * sizeof(double))};
-                            quintic_pair_accum<false>(l0, xi, eta, wa, da, g8);
-                            quintic_pair_accum<false>(l1, xi, eta, wb, db, g8);
-                        }
-                    }
-#else
                     LdShared ld{smem_u32(coef + (size_t)sl * C::SLOT_DOUBLES + (size_t)lk * PLANE_STRIDE)};
                     gather_cell<false, double>(ld, xi, eta, w, dw, g8);
-#endif
                     FieldsG<double> f;
                     to_fields_g<double>(jj[0], jj[1], jj[2], jj[3], g8, y[3], f);
                     double mu, pw;
