@@ -410,3 +410,27 @@ def test_numeric_equilibrium_rhs_and_push_match_oracle():
         x.equilibrium_set(**synth.equilibrium_args(cfg))
     _check_push(o, g, m, cfg, 0.05, 10, 0, sort_every=1)
     assert g.push_variant_used() == 0
+
+
+def test_fields_export_import_round_trip():
+    """trimeg_fields_export / trimeg_fields_import (the payload of the one multi-GPU collective): a second context
+    that never ran fields_set gathers bit-identical values after importing the first one's table; wrong sizes are refused."""
+    import torch
+    from paper_2606_24327_b200.binding import Trimeg, TrimegError
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, nr=8, ntheta=24, n_planes=8, n_markers=3001)
+    RZ, tri, o, g, m = _make(cfg)
+    d = _dev({k: m[k] for k in ("R", "Z", "phi")})
+    ref, _ = g.gather(d["R"], d["Z"], d["phi"])
+    buf = g.fields_export()
+    assert buf.numel() == g.fields_bytes() > 0
+    g2 = Trimeg(0)
+    g2.equilibrium_set(**synth.equilibrium_args(cfg))
+    g2.species_set(**synth.species_args(cfg))
+    g2.mesh_load(RZ, tri, cfg.n_planes, cfg.phi_period)
+    zero, _ = g2.gather(d["R"], d["Z"], d["phi"])
+    assert float(zero.abs().max()) == 0.0
+    g2.fields_import(buf)
+    out, _ = g2.gather(d["R"], d["Z"], d["phi"])
+    assert torch.equal(out, ref)
+    with pytest.raises(TrimegError, match="rc=-1"):
+        g2.fields_import(buf[:-8])
