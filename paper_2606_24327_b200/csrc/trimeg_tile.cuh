@@ -20,11 +20,8 @@ struct TileTables {
     int npatch, nwin, nsc;   // super-cells = npatch * nwin
 };
 
-template <int TP_, int SMAX_, int WK_, int NBUF_, int K_>
-struct TileCfg {
-    static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD;
-    // 16 warps: one light warp-group (stager, two publishers, one spare) and three compute warp-groups
-    #ifndef TRIMEG_NCOMP
+// tuning switches of the phase kernel (the shipped build uses the defaults; python -m paper_2606_24327_b200.build --defs ...)
+#ifndef TRIMEG_NCOMP
 #define TRIMEG_NCOMP 12
 #endif
 #ifndef TRIMEG_REG_COMP
@@ -33,11 +30,16 @@ struct TileCfg {
 #ifndef TRIMEG_NPUB
 #define TRIMEG_NPUB 2
 #endif
-    static constexpr int NLIGHT = 4, NPUB = TRIMEG_NPUB, NCOMP = TRIMEG_NCOMP;   // light warps: stager, NPUB publishers, (prefetcher if NPUB = 2)
+template <int TP_, int SMAX_, int WK_, int NBUF_, int K_>
+struct TileCfg {
+    static constexpr int TP = TP_, SMAX = SMAX_, WK = WK_, HK = PLANE_PAD;
+    // 16 warps: one light warp-group (stager, NPUB publishers, prefetcher if NPUB = 2) and NCOMP / 4 compute warp-groups
+    static constexpr int NLIGHT = 4, NPUB = TRIMEG_NPUB, NCOMP = TRIMEG_NCOMP;
     static constexpr int NWARPS = NLIGHT + NCOMP, NTHREADS = 32 * NWARPS;
-    // register hand-over (setmaxnreg): 16 warps launch with 128 registers; the light warps drop to 40, the compute warps
-    // take 24 more each (12 x 24 <= 4 x 88)
+    // register hand-over (setmaxnreg): 16 warps launch with 128 registers; the light warps drop to 56, the compute warps
+    // take 24 more each (4 x 56 + 12 x 152 = 2048 = 16 x 128)
     static constexpr int REG_LIGHT = 56, REG_COMP = TRIMEG_REG_COMP;
+    static_assert(NLIGHT * REG_LIGHT + NCOMP * REG_COMP <= NWARPS * (65536 / (32 * NWARPS) / 8 * 8), "setmaxnreg: the roles' registers must fit the launch allocation (else the kernel hangs)");
     static constexpr int NPL = WK + 2 * HK + 3;      // staged planes per slot
     static constexpr int NW = WK + 2 * HK;           // toroidal intervals covered
     static constexpr int CPS = TP * WK;              // cells per super-cell
