@@ -425,7 +425,7 @@ static int gather_device(trimeg_ctx* ctx, long long n, const double* R, const do
     k_gather_decide<<<1, 1, 0, ctx->stream>>>(ctx->gather_mode, ctx->d_gwork + 2, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[0], ctx->stream));
-    k_gather_keys<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, ctx->gm, n, R, Z, phi, (int)ctx->g_ncell, keys, tris, ctx->d_ghist, flag);
+    k_gather_keys<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, ctx->gm, n, R, Z, phi, (int)ctx->g_ncell, keys, tris, inv, ctx->d_ghist, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[1], ctx->stream));
     k_scan_reduce<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums);
@@ -433,7 +433,7 @@ static int gather_device(trimeg_ctx* ctx, long long n, const double* R, const do
     k_scan_apply<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums, ctx->d_goffs, ctx->d_gfill);   // also clears histogram and fill
     KCHECK();
     CU(cudaEventRecord(ctx->gev[2], ctx->stream));
-    k_gather_scatter<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(n, R, Z, phi, keys, tris, ctx->d_goffs, ctx->d_gfill, pts, inv, flag);
+    k_gather_scatter<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(n, R, Z, phi, keys, tris, ctx->d_goffs, pts, inv, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[3], ctx->stream));
     k_gather_staged<<<ctx->num_sms * 2, GTHREADS, GatherSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->g_nunits, ctx->NPP, ctx->d_goffs, pts, res, ctx->d_gwork, flag);

@@ -67,7 +67,7 @@ __global__ void k_gather_decide(int mode, const int* __restrict__ cnt, int* __re
 
 __global__ void __launch_bounds__(256) k_gather_keys(DevTables tb, GatherMap gm, long long n, const double* __restrict__ R, const double* __restrict__ Z,
                                                      const double* __restrict__ phi, int ncell, int* __restrict__ keys, int* __restrict__ tris,
-                                                     int* __restrict__ hist, const int* __restrict__ flag) {
+                                                     int* __restrict__ ranks, int* __restrict__ hist, const int* __restrict__ flag) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n || *flag != 2) return;
     const int t = locate_box(tb.bg, tb.geom, R[i], Z[i]);
@@ -76,16 +76,16 @@ __global__ void __launch_bounds__(256) k_gather_keys(DevTables tb, GatherMap gm,
     const int key = t < 0 ? ncell : gm.cell(t, k);
     keys[i] = key;
     tris[i] = t;
-    atomicAdd(hist + key, 1);
+    ranks[i] = atomicAdd(hist + key, 1);      // the old count is this point's rank within its cell: the scatter needs no second atomic
 }
 
 __global__ void __launch_bounds__(256) k_gather_scatter(long long n, const double* __restrict__ R, const double* __restrict__ Z, const double* __restrict__ phi,
                                                         const int* __restrict__ keys, const int* __restrict__ tris, const int* __restrict__ offs,
-                                                        int* __restrict__ fill, GPoint* __restrict__ pts, int* __restrict__ inv, const int* __restrict__ flag) {
+                                                        GPoint* __restrict__ pts, int* __restrict__ inv, const int* __restrict__ flag) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n || *flag != 2) return;
     const int key = keys[i];
-    const int pos = offs[key] + atomicAdd(fill + key, 1);
+    const int pos = offs[key] + inv[i];      // inv[] comes in holding the rank within the cell and leaves holding the position
     st256(pts + pos, R[i], Z[i], phi[i], __hiloint2double(tris[i], (int)i));     // (id, tri) in the low and high word
     inv[i] = pos;
 }
