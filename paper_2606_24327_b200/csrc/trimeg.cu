@@ -414,6 +414,7 @@ static int gather_device(trimeg_ctx* ctx, long long n, const double* R, const do
     double* res = (double*)ptr;
     const long long gcnt = ctx->g_ncell + 2;
     const int nb = (int)((gcnt + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    const unsigned sgrid = (unsigned)std::min<long long>(blocks_for(n, 256), (long long)ctx->num_sms * 32);   // grid-stride kernels of the staged path
     // d_gwork: [0] work counter of the staged kernel, [1] path flag (1 direct, 2 staged), [2..3] probe counters
     int* flag = ctx->d_gwork + 1;
     CU(cudaMemsetAsync(ctx->d_gwork, 0, sizeof(int) * 4, ctx->stream));
@@ -425,21 +426,21 @@ static int gather_device(trimeg_ctx* ctx, long long n, const double* R, const do
     k_gather_decide<<<1, 1, 0, ctx->stream>>>(ctx->gather_mode, ctx->d_gwork + 2, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[0], ctx->stream));
-    k_gather_keys<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, ctx->gm, n, R, Z, phi, (int)ctx->g_ncell, keys, tris, inv, ctx->d_ghist, flag);
+    k_gather_keys<<<sgrid, 256, 0, ctx->stream>>>(ctx->tb, ctx->gm, n, R, Z, phi, (int)ctx->g_ncell, keys, tris, inv, ctx->d_ghist, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[1], ctx->stream));
-    k_scan_reduce<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums);
-    k_scan_sums<<<1, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_gsums, nb);
-    k_scan_apply<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums, ctx->d_goffs, ctx->d_gfill);   // also clears histogram and fill
+    k_scan_reduce<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums, flag);
+    k_scan_sums<<<1, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_gsums, nb, flag);
+    k_scan_apply<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums, ctx->d_goffs, ctx->d_gfill, flag);   // also clears histogram and fill
     KCHECK();
     CU(cudaEventRecord(ctx->gev[2], ctx->stream));
-    k_gather_scatter<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(n, R, Z, phi, keys, tris, ctx->d_goffs, pts, inv, flag);
+    k_gather_scatter<<<sgrid, 256, 0, ctx->stream>>>(n, R, Z, phi, keys, tris, ctx->d_goffs, pts, inv, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[3], ctx->stream));
     k_gather_staged<<<ctx->num_sms * 2, GTHREADS, GatherSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->g_nunits, ctx->NPP, ctx->d_goffs, pts, res, ctx->d_gwork, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[4], ctx->stream));
-    k_gather_unsort<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(n, tris, inv, res, ctx->d_orig, out, tri_out, flag);
+    k_gather_unsort<<<sgrid, 256, 0, ctx->stream>>>(n, tris, inv, res, ctx->d_orig, out, tri_out, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[5], ctx->stream));
     k_gather<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, n, R, Z, phi, out, tri_out, flag);

@@ -68,26 +68,28 @@ __global__ void k_gather_decide(int mode, const int* __restrict__ cnt, int* __re
 __global__ void __launch_bounds__(256) k_gather_keys(DevTables tb, GatherMap gm, long long n, const double* __restrict__ R, const double* __restrict__ Z,
                                                      const double* __restrict__ phi, int ncell, int* __restrict__ keys, int* __restrict__ tris,
                                                      int* __restrict__ ranks, int* __restrict__ hist, const int* __restrict__ flag) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n || *flag != 2) return;
-    const int t = locate_box(tb.bg, tb.geom, R[i], Z[i]);
-    double s;
-    const int k = toroidal_interval(tb.tor, phi[i], s);
-    const int key = t < 0 ? ncell : gm.cell(t, k);
-    keys[i] = key;
-    tris[i] = t;
-    ranks[i] = atomicAdd(hist + key, 1);      // the old count is this point's rank within its cell: the scatter needs no second atomic
+    if (*flag != 2) return;      // fixed grid + grid-stride loop: the path not taken costs microseconds, not a 5e7-thread launch
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int t = locate_box(tb.bg, tb.geom, R[i], Z[i]);
+        double s;
+        const int k = toroidal_interval(tb.tor, phi[i], s);
+        const int key = t < 0 ? ncell : gm.cell(t, k);
+        keys[i] = key;
+        tris[i] = t;
+        ranks[i] = atomicAdd(hist + key, 1);      // the old count is this point's rank within its cell: the scatter needs no second atomic
+    }
 }
 
 __global__ void __launch_bounds__(256) k_gather_scatter(long long n, const double* __restrict__ R, const double* __restrict__ Z, const double* __restrict__ phi,
                                                         const int* __restrict__ keys, const int* __restrict__ tris, const int* __restrict__ offs,
                                                         GPoint* __restrict__ pts, int* __restrict__ inv, const int* __restrict__ flag) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n || *flag != 2) return;
-    const int key = keys[i];
-    const int pos = offs[key] + inv[i];      // inv[] comes in holding the rank within the cell and leaves holding the position
-    st256(pts + pos, R[i], Z[i], phi[i], __hiloint2double(tris[i], (int)i));     // (id, tri) in the low and high word
-    inv[i] = pos;
+    if (*flag != 2) return;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int key = keys[i];
+        const int pos = offs[key] + inv[i];      // inv[] comes in holding the rank within the cell and leaves holding the position
+        st256(pts + pos, R[i], Z[i], phi[i], __hiloint2double(tris[i], (int)i));     // (id, tri) in the low and high word
+        inv[i] = pos;
+    }
 }
 
 // shared memory of one CTA: GNST stages of { coefficients [GT][GSLOT], geometry [GT] }, then control.  Two CTAs per SM, one
@@ -179,18 +181,19 @@ k_gather_staged(DevTables tb, GatherMap gm, int nunits, int NPP, const int* __re
 __global__ void __launch_bounds__(256) k_gather_unsort(long long n, const int* __restrict__ tris, const int* __restrict__ inv, const double* __restrict__ res,
                                                        const int* __restrict__ orig, double* __restrict__ out, int* __restrict__ tri_out,
                                                        const int* __restrict__ flag) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n || *flag != 2) return;
-    const int t = tris[i];
-    double2 a = make_double2(0, 0), b = a, c = a, d = a;
-    if (t >= 0) {
-        const double* r = res + 8ll * inv[i];
-        ld256(r, a.x, a.y, b.x, b.y);
-        ld256(r + 4, c.x, c.y, d.x, d.y);
+    if (*flag != 2) return;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const int t = tris[i];
+        double2 a = make_double2(0, 0), b = a, c = a, d = a;
+        if (t >= 0) {
+            const double* r = res + 8ll * inv[i];
+            ld256(r, a.x, a.y, b.x, b.y);
+            ld256(r + 4, c.x, c.y, d.x, d.y);
+        }
+        out[i] = a.x; out[n + i] = a.y; out[2 * n + i] = b.x; out[3 * n + i] = b.y;
+        out[4 * n + i] = c.x; out[5 * n + i] = c.y; out[6 * n + i] = d.x; out[7 * n + i] = d.y;
+        if (tri_out) tri_out[i] = t < 0 ? -1 : orig[t];
     }
-    out[i] = a.x; out[n + i] = a.y; out[2 * n + i] = b.x; out[3 * n + i] = b.y;
-    out[4 * n + i] = c.x; out[5 * n + i] = c.y; out[6 * n + i] = d.x; out[7 * n + i] = d.y;
-    if (tri_out) tri_out[i] = t < 0 ? -1 : orig[t];
 }
 
 }  // namespace trimeg

@@ -202,7 +202,10 @@ __device__ __forceinline__ void gather_at(const DevTables& tb, int t, double R, 
     to_fields(g, acc, f);
 }
 
-__global__ void __launch_bounds__(256, 4) k_gather(DevTables tb, long long n, const double* __restrict__ R, const double* __restrict__ Z,
+#ifndef TRIMEG_GATHER_OCC
+#define TRIMEG_GATHER_OCC 4
+#endif
+__global__ void __launch_bounds__(256, TRIMEG_GATHER_OCC) k_gather(DevTables tb, long long n, const double* __restrict__ R, const double* __restrict__ Z,
                                                 const double* __restrict__ phi, double* __restrict__ out, int* __restrict__ tri_out,
                                                 const int* __restrict__ flag) {   // flag: null, or the path chosen on the device (1 = this kernel)
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -665,7 +668,9 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int* total) {   // SC
     __syncthreads();
     return base + x - v;
 }
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(const int* __restrict__ in, long long n, int* __restrict__ sums) {
+// `skip`: null, or a device flag: the scan is skipped unless *skip == 2 (trimeg_gather's path choice on the device)
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(const int* __restrict__ in, long long n, int* __restrict__ sums, const int* __restrict__ skip = nullptr) {
+    if (skip && *skip != 2) return;
     long long base = (long long)blockIdx.x * SCAN_CHUNK + (long long)threadIdx.x * SCAN_ITEMS;
     int s = 0;
 #pragma unroll
@@ -674,8 +679,9 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(const int* __restr
     block_exclusive_scan(s, &tot);
     if (threadIdx.x == 0) sums[blockIdx.x] = tot;
 }
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(int* __restrict__ sums, int nb) {   // single block
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(int* __restrict__ sums, int nb, const int* __restrict__ skip = nullptr) {   // single block
     __shared__ int carry;
+    if (skip && *skip != 2) return;
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
     for (int b0 = 0; b0 < nb; b0 += SCAN_THREADS) {
@@ -690,7 +696,8 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(int* __restrict__ su
 }
 // writes the exclusive offsets and clears the histogram and the fill counters for the next pass
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(int* __restrict__ in, long long n, const int* __restrict__ sums,
-                                                             int* __restrict__ out, int* __restrict__ fill) {
+                                                             int* __restrict__ out, int* __restrict__ fill, const int* __restrict__ skip = nullptr) {
+    if (skip && *skip != 2) return;
     long long base = (long long)blockIdx.x * SCAN_CHUNK + (long long)threadIdx.x * SCAN_ITEMS;
     int v[SCAN_ITEMS], s = 0;
 #pragma unroll
