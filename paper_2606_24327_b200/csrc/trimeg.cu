@@ -437,7 +437,7 @@ static int gather_device(trimeg_ctx* ctx, long long n, const double* R, const do
     k_gather_scatter<<<sgrid, 256, 0, ctx->stream>>>(n, R, Z, phi, keys, tris, ctx->d_goffs, pts, inv, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[3], ctx->stream));
-    k_gather_staged<<<ctx->num_sms * 2, GTHREADS, GatherSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->g_nunits, ctx->NPP, ctx->d_goffs, pts, res, ctx->d_gwork, flag);
+    k_gather_staged<<<ctx->num_sms * TRIMEG_GOCC, GTHREADS, GatherSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->g_nunits, ctx->NPP, ctx->d_goffs, pts, res, ctx->d_gwork, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[4], ctx->stream));
     k_gather_unsort<<<sgrid, 256, 0, ctx->stream>>>(n, tris, inv, res, ctx->d_orig, out, tri_out, flag);

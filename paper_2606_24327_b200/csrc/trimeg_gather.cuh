@@ -15,11 +15,25 @@
 
 namespace trimeg {
 
-constexpr int GT = 8, GW = 8;                       // triangles x toroidal intervals per gather super-cell
+// tuning knobs of the staged kernel (python -m paper_2606_24327_b200.build --defs "-DTRIMEG_GT=8 ..."): triangles per
+// super-cell, threads per CTA, CTAs per SM, TMA stages
+#ifndef TRIMEG_GT
+#define TRIMEG_GT 4
+#endif
+#ifndef TRIMEG_GTHREADS
+#define TRIMEG_GTHREADS 96
+#endif
+#ifndef TRIMEG_GOCC
+#define TRIMEG_GOCC 6
+#endif
+#ifndef TRIMEG_GNST
+#define TRIMEG_GNST 2
+#endif
+constexpr int GT = TRIMEG_GT, GW = 8;                       // triangles x toroidal intervals per gather super-cell
 constexpr int GNPL = GW + 3;                        // staged planes per triangle
 constexpr int GSLOT = GNPL * PLANE_STRIDE;          // doubles per staged triangle
 constexpr int GCELLS = GT * GW;                     // cells per super-cell
-constexpr int GTHREADS = 256;
+constexpr int GTHREADS = TRIMEG_GTHREADS;
 
 struct GatherMap {   // cell numbering of the gather: super-cell (patch, window) major, then triangle, then interval
     int nwin;
@@ -92,10 +106,11 @@ __global__ void __launch_bounds__(256) k_gather_scatter(long long n, const doubl
     }
 }
 
-// shared memory of one CTA: GNST stages of { coefficients [GT][GSLOT], geometry [GT] }, then control.  Two CTAs per SM, one
-// stage being evaluated and two in flight each: ~120 KB of coefficient copies in flight per SM (HBM latency x bandwidth / SM
-// is ~90 KB)
-constexpr int GNST = 3;
+// shared memory of one CTA: GNST stages of { coefficients [GT][GSLOT], geometry [GT] }, then control.  The kernel is bound by
+// the latency of one super-cell's round (wait, evaluate, barrier), not by bytes, so many small CTAs beat few large ones:
+// measured on config 4 (profiles/r02_gather_cfg4.md), 8 triangles x 256 threads x 2 CTAs/SM x 3 stages 3.70 ms,
+// 4 triangles x 96 threads x 6 CTAs/SM x 2 stages 3.01 ms (the default; ~83 points per super-cell there fill 96 lanes to 87 %).
+constexpr int GNST = TRIMEG_GNST;
 struct GatherSmem {
     static constexpr size_t COEF = sizeof(double) * GT * GSLOT;
     static constexpr size_t STAGE = COEF + sizeof(TriGeom) * GT;
@@ -103,7 +118,7 @@ struct GatherSmem {
     static constexpr size_t BYTES = OFF_CTRL + GNST * 32;
 };
 
-__global__ void __launch_bounds__(GTHREADS, 2)
+__global__ void __launch_bounds__(GTHREADS, TRIMEG_GOCC)
 k_gather_staged(DevTables tb, GatherMap gm, int nunits, int NPP, const int* __restrict__ offs, const GPoint* __restrict__ pts,
                 double* __restrict__ res, int* __restrict__ work_counter, const int* __restrict__ flag) {
     extern __shared__ __align__(128) unsigned char smem[];
