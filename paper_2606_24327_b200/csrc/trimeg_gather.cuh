@@ -32,14 +32,19 @@ namespace trimeg {
 constexpr int GT = TRIMEG_GT, GW = 8;                       // triangles x toroidal intervals per gather super-cell
 constexpr int GNPL = GW + 3;                        // staged planes per triangle
 constexpr int GSLOT = GNPL * PLANE_STRIDE;          // doubles per staged triangle
-constexpr int GCELLS = GT * GW;                     // cells per super-cell
+#ifndef TRIMEG_GKEY_CELL
+#define TRIMEG_GKEY_CELL 0
+#endif
+// bins per super-cell: one per (triangle, window) - the order of a triangle's points within the window does not matter to the
+// staged kernel, and 8x fewer counters keep the histogram L2-resident - or, as a tuning build, one per cell
+constexpr int GCELLS = TRIMEG_GKEY_CELL ? GT * GW : GT;
 constexpr int GTHREADS = TRIMEG_GTHREADS;
 
-struct GatherMap {   // cell numbering of the gather: super-cell (patch, window) major, then triangle, then interval
+struct GatherMap {   // bin numbering of the gather: super-cell (patch, window) major, then triangle (then interval)
     int nwin;
     __host__ __device__ __forceinline__ int cell(int t, int k) const {
         const int patch = t / GT, tl = t - patch * GT, w = k / GW, kl = k - w * GW;
-        return ((patch * nwin + w) * GT + tl) * GW + kl;
+        return TRIMEG_GKEY_CELL ? ((patch * nwin + w) * GT + tl) * GW + kl : (patch * nwin + w) * GT + tl;
     }
 };
 struct __align__(32) GPoint { double R, Z, phi; int id, tri; };   // one point in cell order (32 B = one sector)

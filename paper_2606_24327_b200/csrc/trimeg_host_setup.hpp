@@ -10,6 +10,9 @@
 #include <unordered_map>
 #include <vector>
 
+#ifndef TRIMEG_BOX_REFINE
+#define TRIMEG_BOX_REFINE 3.0
+#endif
 namespace trimeg_host {
 
 // coefficient index of xi^i eta^j in the j-major layout the kernels use
@@ -189,7 +192,11 @@ inline int build_mesh(int64_t n_nodes, const double* RZ, int64_t T, const int32_
         }
     }
     // box grid
-    int nx = (int)std::ceil(std::sqrt((double)T * wx / wy)), ny = (int)std::ceil(std::sqrt((double)T * wy / wx));
+    // TRIMEG_BOX_REFINE^2 boxes per triangle of the bounding rectangle; a triangle is listed in the boxes it overlaps (separating-
+    // axis test against its three edges, conservative by a small margin), not in all boxes of its bounding box: the candidate
+    // lists are what a locate reads (k_gather_keys is bound by those loads, profiles/r02_gather_cfg4.md)
+    const double refine = TRIMEG_BOX_REFINE;
+    int nx = (int)std::ceil(refine * std::sqrt((double)T * wx / wy)), ny = (int)std::ceil(refine * std::sqrt((double)T * wy / wx));
     nx = std::max(nx, 1); ny = std::max(ny, 1);
     hm.nx = nx; hm.ny = ny; hm.xmin = xmin; hm.ymin = ymin; hm.dx = wx / nx; hm.dy = wy / ny;
     size_t nb = (size_t)nx * ny;
@@ -203,7 +210,23 @@ inline int build_mesh(int64_t n_nodes, const double* RZ, int64_t T, const int32_
             const double eps = 1e-6;   // in box units: a point on a box boundary may round into either box
             int i0 = std::max(0, (int)std::floor((bx0 - xmin) / hm.dx - eps)), i1 = std::min(nx - 1, (int)std::floor((bx1 - xmin) / hm.dx + eps));
             int j0 = std::max(0, (int)std::floor((by0 - ymin) / hm.dy - eps)), j1 = std::min(ny - 1, (int)std::floor((by1 - ymin) / hm.dy + eps));
+            // edge e from vertex e to e+1: outward normal (oriented by the sign of the area) and its offset
+            double vx[3], vy[3], enx[3], eny[3], eoff[3];
+            for (int v = 0; v < 3; v++) { vx[v] = RZ[2 * hm.tri[3 * t + v]]; vy[v] = RZ[2 * hm.tri[3 * t + v] + 1]; }
+            const double area2 = (vx[1] - vx[0]) * (vy[2] - vy[0]) - (vx[2] - vx[0]) * (vy[1] - vy[0]), sg = area2 >= 0.0 ? 1.0 : -1.0;
+            for (int e = 0; e < 3; e++) {
+                const double ex = vx[(e + 1) % 3] - vx[e], ey = vy[(e + 1) % 3] - vy[e];
+                enx[e] = sg * ey; eny[e] = -sg * ex; eoff[e] = enx[e] * vx[e] + eny[e] * vy[e];
+            }
             for (int j = j0; j <= j1; j++) for (int i = i0; i <= i1; i++) {
+                // the box (grown by eps on every side) lies outside edge e if even its corner nearest to the triangle does
+                const double cx0 = xmin + (i - eps) * hm.dx, cx1 = xmin + (i + 1 + eps) * hm.dx, cy0 = ymin + (j - eps) * hm.dy, cy1 = ymin + (j + 1 + eps) * hm.dy;
+                bool apart = false;
+                for (int e = 0; e < 3 && !apart; e++) {
+                    const double dmin = enx[e] * (enx[e] > 0.0 ? cx0 : cx1) + eny[e] * (eny[e] > 0.0 ? cy0 : cy1) - eoff[e];
+                    apart = dmin > 1e-9 * (std::fabs(enx[e]) * hm.dx + std::fabs(eny[e]) * hm.dy);
+                }
+                if (apart) continue;
                 size_t b = (size_t)j * nx + i;
                 if (!pass) hm.head[b + 1]++; else hm.list[hm.head[b] + fill[b]++] = (int32_t)t;
             }
