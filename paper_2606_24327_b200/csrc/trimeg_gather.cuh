@@ -116,10 +116,12 @@ __global__ void __launch_bounds__(256) k_gather_scatter(long long n, const doubl
 // measured on config 4 (profiles/r02_gather_cfg4.md), 8 triangles x 256 threads x 2 CTAs/SM x 3 stages 3.70 ms,
 // 4 triangles x 96 threads x 6 CTAs/SM x 2 stages 3.01 ms (the default; ~83 points per super-cell there fill 96 lanes to 87 %).
 constexpr int GNST = TRIMEG_GNST;
+constexpr int GPCAP = GTHREADS;                     // point records staged with a super-cell (the first pass of its evaluation)
 struct GatherSmem {
     static constexpr size_t COEF = sizeof(double) * GT * GSLOT;
-    static constexpr size_t STAGE = COEF + sizeof(TriGeom) * GT;
-    static constexpr size_t OFF_CTRL = GNST * STAGE;      // per stage: mbarrier (8 B), unit, begin, end (ints)
+    static constexpr size_t OFF_PTS = COEF + sizeof(TriGeom) * GT;
+    static constexpr size_t STAGE = OFF_PTS + sizeof(GPoint) * GPCAP;
+    static constexpr size_t OFF_CTRL = GNST * STAGE;      // per stage: 'landed' mbarrier (8 B), unit, begin, end (ints), pad, 'consumed' mbarrier (8 B)
     static constexpr size_t BYTES = OFF_CTRL + GNST * 32;
 };
 
@@ -131,43 +133,56 @@ k_gather_staged(DevTables tb, GatherMap gm, int nunits, int NPP, const int* __re
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     auto bar_of = [&](int s) { return reinterpret_cast<unsigned long long*>(smem + GatherSmem::OFF_CTRL + 32 * s); };
     auto ctl_of = [&](int s) { return reinterpret_cast<int*>(smem + GatherSmem::OFF_CTRL + 32 * s + 8); };
+    auto done_of = [&](int s) { return reinterpret_cast<unsigned long long*>(smem + GatherSmem::OFF_CTRL + 32 * s + 24); };
+    constexpr int NW = GTHREADS / 32;
     if (tid == 0) {
-        for (int q = 0; q < GNST; ++q) mbar_init(bar_of(q), 1);
+        for (int q = 0; q < GNST; ++q) { mbar_init(bar_of(q), 1); mbar_init(done_of(q), NW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    // warp 0 stages: next non-empty super-cell off the work list -> stage s (its previous contents have been consumed)
-    auto stage = [&](int s) {
-        int u = 0, begin = 0, end = 0;
-        for (;;) {
-            if (lane == 0) u = atomicAdd(work_counter, 1);
-            u = __shfl_sync(0xffffffffu, u, 0);
-            if (u >= nunits) { u = -1; break; }
-            begin = offs[(long long)u * GCELLS]; end = offs[(long long)(u + 1) * GCELLS];
-            if (begin != end) break;
-        }
+    // warp 0 stages.  Super-cells are dealt out round-robin (CTA b takes b, b + grid, ...: ~700 per CTA on config 4, so the load
+    // evens out) and the point range of the NEXT one is loaded while the current one is being issued, so that staging is
+    // issue-only: no global round trip sits between the end of a round and the next round's copies.  (With a work counter
+    // and the geometry copied by the warp itself, warp 0 came 2-3 us late to every round's barrier: 38 % of the kernel's
+    // stall samples were the other warps waiting there, profiles/r02_gather_cfg4.md.)
+    static_assert(sizeof(TriGeom) == 64, "geometry records are copied in bulk");
+    int nu = blockIdx.x, nbeg = 0, nend = 0;               // warp 0: the next super-cell and its point range
+    auto fetch = [&]() { if (nu < nunits) { nbeg = offs[(long long)nu * GCELLS]; nend = offs[(long long)(nu + 1) * GCELLS]; } };
+    if (wid == 0) fetch();
+    auto stage = [&](int s, unsigned use) {                  // use: how often stage s has been filled before
+        if (use > 0) mbar_wait(done_of(s), (use - 1) & 1);    // every warp is done with its previous contents
+        while (nu < nunits && nbeg == nend) { nu += gridDim.x; fetch(); }        // empty super-cells are skipped
+        const int u = nu < nunits ? nu : -1, begin = nbeg, end = nend;
+        nu += gridDim.x; fetch();
         int* ctl = ctl_of(s);
         if (lane == 0) { ctl[0] = u; ctl[1] = begin; ctl[2] = end; }
         if (u < 0) { __syncwarp(); if (lane == 0) mbar_arrive(bar_of(s)); return; }
         const int patch = u / gm.nwin, w = u - patch * gm.nwin;
         const int pp0 = w * GW + PLANE_PAD, npl = min(GNPL, NPP - pp0);
         const int t = patch * GT + lane;
-        const bool has = lane < GT && t < tb.T;
-        double* coef = reinterpret_cast<double*>(smem + GatherSmem::STAGE * s);
-        TriGeom* geom = reinterpret_cast<TriGeom*>(smem + GatherSmem::STAGE * s + GatherSmem::COEF);
-        if (has) geom[lane] = tb.geom[t];
+        const int cnt = min(GT, tb.T - patch * GT);
+        const bool has = lane < cnt;
+        unsigned char* st = smem + GatherSmem::STAGE * s;
         const unsigned bytes = (unsigned)(npl * PLANE_STRIDE * sizeof(double));
-        const int cnt = __popc(__ballot_sync(0xffffffffu, has));
-        fence_async_smem();
+        // the super-cell's first GPCAP point records come with it: the evaluation starts from shared memory
+        const unsigned pbytes = (unsigned)(min(end - begin, GPCAP) * (int)sizeof(GPoint));
+        const unsigned gbytes = (unsigned)(cnt * (int)sizeof(TriGeom));
+        if (lane == 0) mbar_expect_tx(bar_of(s), cnt * bytes + pbytes + gbytes);
         __syncwarp();
-        if (lane == 0) mbar_expect_tx(bar_of(s), cnt * bytes);
-        __syncwarp();
-        if (has) tma_bulk_g2s(coef + (size_t)lane * GSLOT, tb.coef + (long long)t * tb.tri_stride + (long long)pp0 * PLANE_STRIDE, bytes, bar_of(s));
+        if (has) tma_bulk_g2s(reinterpret_cast<double*>(st) + (size_t)lane * GSLOT, tb.coef + (long long)t * tb.tri_stride + (long long)pp0 * PLANE_STRIDE, bytes, bar_of(s));
+        if (lane == 0) {
+            tma_bulk_g2s(st + GatherSmem::COEF, tb.geom + (long long)patch * GT, gbytes, bar_of(s));
+            tma_bulk_g2s(st + GatherSmem::OFF_PTS, pts + begin, pbytes, bar_of(s));
+        }
     };
-    if (wid == 0) { for (int q = 0; q < GNST - 1; ++q) stage(q); }
+    // No CTA-wide barrier per round: a warp that is done with a stage says so on the stage's 'consumed' barrier and goes on to
+    // the next stage, so the warps may drift apart by up to GNST - 1 rounds.  A super-cell with more points than threads
+    // gives some warp a second pass; with a barrier per round the other warps stood idle for it (28 % of all stall samples),
+    // now they work ahead, and the lane numbering rotates by one warp per round so that the extra pass is not always warp 0's.
+    if (wid == 0) { for (int q = 0; q < GNST - 1; ++q) stage(q, 0); }
     for (unsigned it = 0;; ++it) {
         const int s = it % GNST;
-        if (wid == 0) stage((it + GNST - 1) % GNST);      // that stage was released by the barrier at the end of the last round
+        if (wid == 0) stage((it + GNST - 1) % GNST, (it + GNST - 1) / GNST);
         mbar_wait(bar_of(s), (it / GNST) & 1);
         const int* ctl = ctl_of(s);
         const int u = ctl[0], begin = ctl[1], end = ctl[2];
@@ -175,11 +190,18 @@ k_gather_staged(DevTables tb, GatherMap gm, int nunits, int NPP, const int* __re
         const int patch = u / gm.nwin, w = u - patch * gm.nwin;
         const double* coef = reinterpret_cast<const double*>(smem + GatherSmem::STAGE * s);
         const TriGeom* geom = reinterpret_cast<const TriGeom*>(smem + GatherSmem::STAGE * s + GatherSmem::COEF);
-        for (int pos = begin + tid; pos < end; pos += GTHREADS) {
+        const int rot = tid + 32 * (int)(it % NW), vt = rot >= GTHREADS ? rot - GTHREADS : rot;
+        for (int pos = begin + vt; pos < end; pos += GTHREADS) {
             GPoint p;
             {
                 double it;
-                ld256(pts + pos, p.R, p.Z, p.phi, it);
+                if (pos - begin < GPCAP) {
+                    const double2* sp = reinterpret_cast<const double2*>(smem + GatherSmem::STAGE * s + GatherSmem::OFF_PTS) + 2 * (pos - begin);
+                    const double2 a = sp[0], b = sp[1];
+                    p.R = a.x; p.Z = a.y; p.phi = b.x; it = b.y;
+                } else {
+                    ld256(pts + pos, p.R, p.Z, p.phi, it);
+                }
                 p.id = __double2loint(it); p.tri = __double2hiint(it);
             }
             const int tl = p.tri - patch * GT;
@@ -194,7 +216,8 @@ k_gather_staged(DevTables tb, GatherMap gm, int nunits, int NPP, const int* __re
             st256(res + 8ll * pos, f.P, f.PR, f.PZ, f.Pp);
             st256(res + 8ll * pos + 4, f.A, f.AR, f.AZ, f.Ap);
         }
-        __syncthreads();                                  // everybody is done with stage s
+        __syncwarp();
+        if (lane == 0) mbar_arrive(done_of(s));            // this warp is done with stage s
     }
 }
 
@@ -202,17 +225,29 @@ __global__ void __launch_bounds__(256) k_gather_unsort(long long n, const int* _
                                                        const int* __restrict__ orig, double* __restrict__ out, int* __restrict__ tri_out,
                                                        const int* __restrict__ flag) {
     if (*flag != 2) return;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const int t = tris[i];
-        double2 a = make_double2(0, 0), b = a, c = a, d = a;
-        if (t >= 0) {
-            const double* r = res + 8ll * inv[i];
-            ld256(r, a.x, a.y, b.x, b.y);
-            ld256(r + 4, c.x, c.y, d.x, d.y);
+    // A warp takes 32 consecutive caller indices.  Each 64-byte result record is fetched by a PAIR of lanes (one 32-byte
+    // half each, so the pair's two accesses are one 64-byte request), 16 records per load instruction; the halves are then
+    // handed to the lane that writes the point (coalesced stores into the caller's eight arrays).
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, half = lane & 1, pl = lane >> 1;
+    const long long nround = (n + 31) / 32 * 32;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nround; i += (long long)gridDim.x * blockDim.x) {
+        int t = -1, pos = 0;
+        if (i < n) { t = tris[i]; pos = inv[i]; }
+        double q[2][4];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int ts = __shfl_sync(FULL, t, 16 * h + pl), ps = __shfl_sync(FULL, pos, 16 * h + pl);
+            q[h][0] = q[h][1] = q[h][2] = q[h][3] = 0.0;
+            if (ts >= 0) ld256(res + 8ll * ps + 4 * half, q[h][0], q[h][1], q[h][2], q[h][3]);
         }
-        out[i] = a.x; out[n + i] = a.y; out[2 * n + i] = b.x; out[3 * n + i] = b.y;
-        out[4 * n + i] = c.x; out[5 * n + i] = c.y; out[6 * n + i] = d.x; out[7 * n + i] = d.y;
-        if (tri_out) tri_out[i] = t < 0 ? -1 : orig[t];
+        const int src = 2 * (lane & 15);
+#pragma unroll
+        for (int f = 0; f < 8; ++f) {
+            const double v0 = __shfl_sync(FULL, q[0][f & 3], src + (f >> 2)), v1 = __shfl_sync(FULL, q[1][f & 3], src + (f >> 2));
+            if (i < n) out[(long long)f * n + i] = lane < 16 ? v0 : v1;
+        }
+        if (tri_out && i < n) tri_out[i] = t < 0 ? -1 : orig[t];
     }
 }
 
