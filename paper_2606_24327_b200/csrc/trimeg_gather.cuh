@@ -2,15 +2,22 @@
 //
 // One field evaluation reads 8 x 168 B of coefficients per point; through L1/L2 with the points in caller order that is
 // 7x the algorithmic HBM traffic on config 4 (profiles/r01c_gather_cfg4.md).  Here the library bins the points itself:
-//   1. k_gather_keys     caller order: box-grid locate (L89, L125-140), toroidal interval -> cell key, histogram;
-//   2. scan              (the push's counting-sort kernels) -> cell offsets;
-//   3. k_gather_scatter  caller order: position in the cell order; 32-byte point record written there (a full sector),
+//   1. k_gather_keys     caller order: box-grid locate (L89, L125-140), toroidal interval -> bin key, histogram (the atomic's
+//                        return value is the point's rank within its bin).  A bin is a (triangle, window of GW intervals):
+//                        the staged kernel does not care about the order within it, and 8x fewer counters than cells stay
+//                        in L2;
+//   2. scan              (the push's counting-sort kernels) -> bin offsets;
+//   3. k_gather_scatter  caller order: position = offset + rank; 32-byte point record written there (a full sector),
 //                        position kept per caller index;
-//   4. k_gather_staged   persistent CTAs, one super-cell (GT triangles x GW toroidal intervals) at a time: its coefficient
-//                        block arrives by TMA bulk copies (double-buffered, mbarrier), warps evaluate its points from
-//                        shared memory and write 64-byte result records in cell order (coalesced);
-//   5. k_gather_unsort   caller order: result record -> the caller's eight arrays (coalesced writes), triangle id.
-// HBM bytes per point: 32 + 68 + (96 + coefficients) + 140, against 92 + coefficients algorithmic; DESIGN.md section 6.
+//   4. k_gather_staged   persistent CTAs, one super-cell (GT triangles x GW toroidal intervals) at a time, dealt out
+//                        round-robin: its coefficient block, geometry and point records arrive by TMA bulk copies (two
+//                        stages, 'landed' / 'consumed' mbarriers, no CTA-wide barrier), warps evaluate its points from
+//                        shared memory and write 64-byte result records in bin order (coalesced).  Bound by shared-memory
+//                        bandwidth (1 344 B of coefficients per point, ~4 wavefronts per LDS.128);
+//   5. k_gather_unsort   caller order: result record (fetched by a lane pair as one 64-byte request) -> the caller's eight
+//                        arrays (coalesced writes), triangle id.
+// HBM bytes per point: 36 + 68 + (96 + coefficients) + 140, against 92 + coefficients algorithmic; DESIGN.md section 6,
+// profiles/r02_gather_cfg4.md.
 #pragma once
 
 namespace trimeg {
