@@ -624,7 +624,7 @@ static int build_order(trimeg_ctx* ctx) {
     KCHECK();
     k_scan_apply<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_hist, ncnt, ctx->d_sums, ctx->d_offs, ctx->d_fill);
     KCHECK();
-    k_sort_perm<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(n, ctx->d_keys, ctx->d_offs, ctx->d_fill, ctx->d_perm);
+    k_sort_perm<<<blocks_for((n + SORT_PER_THREAD - 1) / SORT_PER_THREAD, 256), 256, 0, ctx->stream>>>(n, ctx->d_keys, ctx->d_offs, ctx->d_fill, ctx->d_perm);
     KCHECK();
     ctx->order_valid = true;
     ctx->stats[0] += 4;

@@ -709,14 +709,34 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(int* __restrict__ i
         ex += v[i];
     }
 }
+#ifndef TRIMEG_SORT_PER_THREAD
+#define TRIMEG_SORT_PER_THREAD 4
+#endif
+constexpr int SORT_PER_THREAD = TRIMEG_SORT_PER_THREAD;
 // permutation: perm[position in cell order] = record index (4-byte scattered writes)
 __global__ void __launch_bounds__(256) k_sort_perm(long long n, const int* __restrict__ keys, const int* __restrict__ offs, int* __restrict__ fill,
                                                    int* __restrict__ perm) {
-    long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (m >= n) return;
-    int key = keys[m];
-    long long pos = (long long)offs[key] + atomicAdd(fill + key, 1);
-    perm[pos] = (int)m;
+    // SORT_PER_THREAD records per thread: the chain key -> (offset, fill counter) -> store is three dependent memory round trips,
+    // so the kernel's time is set by how many of them a thread keeps in flight (per 1e8 records: 1 per thread 0.85 ms, 4: 0.57, 8: 0.60, 16: 0.75)
+    constexpr int W = SORT_PER_THREAD;
+    const long long m0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * W;
+    if (m0 >= n) return;
+    int key[W];
+    if (m0 + W <= n) {
+#pragma unroll
+        for (int q = 0; q < W; q += 4) {
+            const int4 k4 = *reinterpret_cast<const int4*>(keys + m0 + q);
+            key[q] = k4.x; key[q + 1] = k4.y; key[q + 2] = k4.z; key[q + 3] = k4.w;
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < W; ++q) key[q] = m0 + q < n ? keys[m0 + q] : -1;
+    }
+    int off[W], rank[W];
+#pragma unroll
+    for (int q = 0; q < W; ++q) if (key[q] >= 0) { off[q] = offs[key[q]]; rank[q] = atomicAdd(fill + key[q], 1); }
+#pragma unroll
+    for (int q = 0; q < W; ++q) if (key[q] >= 0) perm[(long long)off[q] + rank[q]] = (int)(m0 + q);
 }
 // per phase: acc[0] += markers left to the follow-up kernel
 __global__ void k_accumulate_stat(const int* __restrict__ v, unsigned long long* __restrict__ acc) { atomicAdd(acc, (unsigned long long)*v); }
