@@ -307,6 +307,10 @@ int trimeg_mesh_load(trimeg_ctx* ctx, int64_t n_nodes, const double* RZ, int64_t
         CU(cudaMemsetAsync(ctx->d_ghist, 0, sizeof(int) * gcnt, ctx->stream));
         CU(cudaMemsetAsync(ctx->d_gfill, 0, sizeof(int) * gcnt, ctx->stream));
         CU(cudaFuncSetAttribute(k_gather_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GatherSmem::BYTES));
+        CU(cudaFuncSetAttribute(k_gather_runs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GatherRunsSmem::BYTES));
+        // all of the SM's L1/shared array as shared memory for the kernels whose CTAs per SM are set by it
+        CU(cudaFuncSetAttribute(k_gather_runs, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        CU(cudaFuncSetAttribute(k_gather_staged, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     }
     CU(cudaMemcpyAsync(ctx->d_pslots, hp.slots.data(), sizeof(int) * hp.slots.size(), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(ctx->d_pnslots, hp.nslots.data(), sizeof(int) * hp.nslots.size(), cudaMemcpyHostToDevice, ctx->stream));
@@ -443,7 +447,7 @@ static int gather_device(trimeg_ctx* ctx, long long n, const double* R, const do
     k_gather_unsort<<<sgrid, 256, 0, ctx->stream>>>(n, tris, inv, res, ctx->d_orig, out, tri_out, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[5], ctx->stream));
-    k_gather<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(ctx->tb, n, R, Z, phi, out, tri_out, flag);
+    k_gather_runs<<<ctx->num_sms * TRIMEG_RW_OCC, 32 * RW_WARPS, GatherRunsSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->NPP, n, R, Z, phi, out, tri_out, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[6], ctx->stream));
     ctx->gather_ms[0] = -1.0;   // events recorded: trimeg_gather_kernel_ms reads them

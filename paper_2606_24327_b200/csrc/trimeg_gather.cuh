@@ -258,4 +258,151 @@ __global__ void __launch_bounds__(256) k_gather_unsort(long long n, const int* _
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// Points the caller has already clustered by cell (BASELINE configs[4], second run): no binning, no un-sorting, results written
+// straight into the caller's arrays.  The direct kernel (k_gather) reads every coefficient pair with one LDG.128 whose 32
+// lanes sit in ~12 different cells: 12 L1 tag look-ups per instruction, 84 instructions per point - it is bound by the L1
+// tag stage (profiles/r02_gather_cfg4.md).  Here every WARP works on its own: it takes 32 consecutive points, locates them,
+// finds the runs of equal (triangle, window) among its lanes, has the coefficient block of each of the first RW_SLOTS runs
+// copied into its private shared-memory slots by TMA (3.7 KB per run, its own mbarrier), and evaluates from shared memory;
+// lanes of further runs read through L1/L2.  No CTA-wide synchronisation: ~20 warps per SM, each at its own point of the
+// load -> locate -> copy -> evaluate -> store sequence, cover one another's latencies.
+#ifdef TRIMEG_WAITSTATS
+#define RW_CLK(c) const long long c = clock64()
+#define RW_ACC(c0, c1, c2, c3, c4) do { if (lane == 0) { unsigned long long* gw = g_wait[blockIdx.x % 160]; atomicAdd(gw + 30, (unsigned long long)(c1 - c0)); \
+    atomicAdd(gw + 31, (unsigned long long)(c2 - c1)); atomicAdd(gw + 32, (unsigned long long)(c3 - c2)); atomicAdd(gw + 33, (unsigned long long)(c4 - c3)); atomicAdd(gw + 34, 1ull); } } while (0)
+#else
+#define RW_CLK(c) do {} while (0)
+#define RW_ACC(c0, c1, c2, c3, c4) do {} while (0)
+#endif
+#ifndef TRIMEG_RW_SLOTS
+#define TRIMEG_RW_SLOTS 3
+#endif
+#ifndef TRIMEG_RW_WARPS
+#define TRIMEG_RW_WARPS 4
+#endif
+#ifndef TRIMEG_RW_OCC
+#define TRIMEG_RW_OCC 4
+#endif
+constexpr int RW_SLOTS = TRIMEG_RW_SLOTS, RW_WARPS = TRIMEG_RW_WARPS;
+struct GatherRunsSmem {
+    static constexpr size_t WARP = sizeof(double) * RW_SLOTS * GSLOT;      // coefficient slots of one warp
+    static constexpr size_t OFF_BAR = RW_WARPS * WARP;
+    static constexpr size_t BYTES = OFF_BAR + 8 * RW_WARPS;
+};
+__global__ void __launch_bounds__(32 * RW_WARPS, TRIMEG_RW_OCC)
+k_gather_runs(DevTables tb, GatherMap gm, int NPP, long long n, const double* __restrict__ R, const double* __restrict__ Z, const double* __restrict__ phi,
+              double* __restrict__ out, int* __restrict__ tri_out, const int* __restrict__ flag) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    if (flag && *flag != 1) return;
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double* slots = reinterpret_cast<double*>(smem + GatherRunsSmem::WARP * wid);
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + GatherRunsSmem::OFF_BAR) + wid;
+    if (lane == 0) { mbar_init(bar, 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+    __syncwarp();
+    const long long ngroups = (n + 31) / 32, nwarps = (long long)gridDim.x * RW_WARPS;
+    // software pipeline: while the copies of group g are in flight the warp locates the points of its next group (loaded one
+    // iteration earlier) and loads those of the one after, so a group costs max(copy, locate) + evaluation instead of
+    // load + locate + copy + evaluation (measured per group before: 1 200 + 7 000 + 500 + 4 300 cycles, the 7 000 being the
+    // dependent chain point -> box -> list -> geometry)
+    // a warp takes a contiguous range of groups: in clustered input its next group lies in the same or a neighbouring triangle,
+    // so the locate's head / list / geometry loads hit L1 instead of going to L2 three times in a row
+    const long long per = (ngroups + nwarps - 1) / nwarps;
+    long long grp = ((long long)blockIdx.x * RW_WARPS + wid) * per;
+    const long long gend = min(ngroups, grp + per);
+    auto load = [&](long long grp, double& r, double& z, double& ph) {
+        const long long i = grp * 32 + lane;
+        r = 0; z = 0; ph = 0;
+        if (grp < gend && i < n) { r = R[i]; z = Z[i]; ph = phi[i]; }
+    };
+    // the previous group of this warp ended in triangle `hint`; in clustered input most of the next points lie in it too, so one
+    // test against it (one address for the whole warp, an L1 hit) replaces the box lookup's chain of dependent loads
+    // (measured: 5 900 of a group's 10 300 cycles) for them
+    auto locate = [&](long long grp, double r, double z, int hint) {
+        if (!(grp < gend && grp * 32 + lane < n)) return -1;
+#ifdef TRIMEG_RW_NOLOCATE
+        if (hint >= 0) return hint;
+#endif
+        if (hint >= 0) {                            // one test (the caller's triangle numbering need not be spatial: no walk)
+            double xi, eta;
+            ref_coords(tb.geom[hint], r, z, xi, eta);
+            if (fmin(fmin(xi, eta), 1.0 - xi - eta) >= 0.0) return hint;
+        }
+        return locate_box(tb.bg, tb.geom, r, z);
+    };
+    auto last_of = [&](int t) {                      // triangle of the warp's last located lane, -1 if none
+        const unsigned m = __ballot_sync(FULL, t >= 0);
+        return m ? __shfl_sync(FULL, t, 31 - __clz(m)) : -1;
+    };
+    double r, z, ph, rn, zn, phn;
+    load(grp, r, z, ph);
+    load(grp + 1, rn, zn, phn);
+    int t = locate(grp, r, z, -1);
+    for (unsigned round = 0; grp < gend; ++grp, ++round) {
+        const long long i = grp * 32 + lane;
+        double s;
+        RW_CLK(c0);
+        const int k = toroidal_interval(tb.tor, ph, s);
+        const int w = k / GW, pp0 = w * GW + PLANE_PAD;
+        const int bid = t >= 0 ? t * gm.nwin + w : -1;
+        const int prev = __shfl_up_sync(FULL, bid, 1);
+        const bool head = bid >= 0 && (lane == 0 || prev != bid);
+        const unsigned hm = __ballot_sync(FULL, head);
+        const int run = __popc(hm & (0xffffffffu >> (31 - lane))) - 1;     // heads at or before this lane; -1: leading points outside the mesh
+        const unsigned bytes = (unsigned)(min(GNPL, NPP - pp0) * PLANE_STRIDE * (int)sizeof(double));
+        const bool issue = head && run < RW_SLOTS;
+        unsigned tot = issue ? bytes : 0u;
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) tot += __shfl_xor_sync(FULL, tot, o);
+        fence_async_smem();                    // this warp's reads of its slots (previous group) come before the copies that overwrite them
+        if (lane == 0) mbar_expect_tx(bar, tot);
+        __syncwarp();
+        if (issue) tma_bulk_g2s(slots + (size_t)run * GSLOT, tb.coef + (long long)t * tb.tri_stride + (long long)pp0 * PLANE_STRIDE, bytes, bar);
+        double rf, zf, phf;
+        RW_CLK(c1);
+        load(grp + 2, rf, zf, phf);
+        RW_CLK(c1a);
+        const int tn = locate(grp + 1, rn, zn, last_of(t));
+        RW_CLK(c2);
+#ifdef TRIMEG_WAITSTATS
+        if (lane == 0) atomicAdd(g_wait[blockIdx.x % 160] + 35, (unsigned long long)(c1a - c1));
+#endif
+        Fields f = Fields{0, 0, 0, 0, 0, 0, 0, 0};
+        int orig = -1;
+        mbar_wait(bar, round & 1);
+        RW_CLK(c3);
+        if (t >= 0) {
+            const TriGeom g = tb.geom[t];
+            double xi, eta, acc[8], bw[4], dw[4];
+            ref_coords(g, r, z, xi, eta);
+            bspline_from_s<double>(tb.tor, s, bw, dw);
+            if (run < RW_SLOTS) {
+#ifdef TRIMEG_RW_NOEVAL
+                const double2 v = *reinterpret_cast<const double2*>(slots + (size_t)run * GSLOT + (size_t)(k - w * GW) * PLANE_STRIDE);
+                for (int q = 0; q < 8; ++q) acc[q] = v.x * xi + v.y * eta + bw[q & 3] + dw[q & 3];
+#else
+                LdShared ld{smem_u32(slots + (size_t)run * GSLOT + (size_t)(k - w * GW) * PLANE_STRIDE)};
+                gather_cell<true, double>(ld, xi, eta, bw, dw, acc);
+#endif
+            } else {
+                LdGlobal ld{reinterpret_cast<const double2*>(tb.coef + (long long)t * tb.tri_stride + (long long)(k + PLANE_PAD) * PLANE_STRIDE)};
+                gather_cell<true, double>(ld, xi, eta, bw, dw, acc);
+            }
+            to_fields(g, acc, f);
+            orig = g.orig;
+        }
+        if (i < n) {
+            out[i] = f.P; out[n + i] = f.PR; out[2 * n + i] = f.PZ; out[3 * n + i] = f.Pp;
+            out[4 * n + i] = f.A; out[5 * n + i] = f.AR; out[6 * n + i] = f.AZ; out[7 * n + i] = f.Ap;
+            if (tri_out) tri_out[i] = orig;
+        }
+        RW_CLK(c4);
+        RW_ACC(c0, c1, c2, c3, c4);
+        r = rn; z = zn; ph = phn; t = tn;
+        rn = rf; zn = zf; phn = phf;
+        __syncwarp();
+    }
+}
+
 }  // namespace trimeg
