@@ -447,7 +447,7 @@ static int gather_device(trimeg_ctx* ctx, long long n, const double* R, const do
     k_gather_unsort<<<sgrid, 256, 0, ctx->stream>>>(n, tris, inv, res, ctx->d_orig, out, tri_out, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[5], ctx->stream));
-    k_gather_runs<<<ctx->num_sms * TRIMEG_RW_OCC, 32 * RW_WARPS, GatherRunsSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->NPP, n, R, Z, phi, out, tri_out, flag);
+    k_gather_runs<<<ctx->num_sms * TRIMEG_RW_OCC, 32 * RW_WARPS, GatherRunsSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->NPP, n, R, Z, phi, out, tri_out, ctx->d_gwork, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[6], ctx->stream));
     ctx->gather_ms[0] = -1.0;   // events recorded: trimeg_gather_kernel_ms reads them

@@ -290,9 +290,11 @@ struct GatherRunsSmem {
     static constexpr size_t OFF_BAR = RW_WARPS * WARP;
     static constexpr size_t BYTES = OFF_BAR + 8 * RW_WARPS;
 };
+// (The same kernel fed with the library's own bin-ordered records, as the evaluation step of the staged path, was measured too:
+// 3.2 ms against k_gather_staged's 2.9 ms on config 4 - the super-cell kernel stays.)
 __global__ void __launch_bounds__(32 * RW_WARPS, TRIMEG_RW_OCC)
 k_gather_runs(DevTables tb, GatherMap gm, int NPP, long long n, const double* __restrict__ R, const double* __restrict__ Z, const double* __restrict__ phi,
-              double* __restrict__ out, int* __restrict__ tri_out, const int* __restrict__ flag) {
+              double* __restrict__ out, int* __restrict__ tri_out, int* __restrict__ work_counter, const int* __restrict__ flag) {
     extern __shared__ __align__(128) unsigned char smem[];
     if (flag && *flag != 1) return;
     const unsigned FULL = 0xffffffffu;
@@ -301,26 +303,35 @@ k_gather_runs(DevTables tb, GatherMap gm, int NPP, long long n, const double* __
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + GatherRunsSmem::OFF_BAR) + wid;
     if (lane == 0) { mbar_init(bar, 1); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
     __syncwarp();
-    const long long ngroups = (n + 31) / 32, nwarps = (long long)gridDim.x * RW_WARPS;
+    const long long ngroups = (n + 31) / 32;
     // software pipeline: while the copies of group g are in flight the warp locates the points of its next group (loaded one
     // iteration earlier) and loads those of the one after, so a group costs max(copy, locate) + evaluation instead of
     // load + locate + copy + evaluation (measured per group before: 1 200 + 7 000 + 500 + 4 300 cycles, the 7 000 being the
     // dependent chain point -> box -> list -> geometry)
-    // a warp takes a contiguous range of groups: in clustered input its next group lies in the same or a neighbouring triangle,
-    // so the locate's head / list / geometry loads hit L1 instead of going to L2 three times in a row
-    const long long per = (ngroups + nwarps - 1) / nwarps;
-    long long grp = ((long long)blockIdx.x * RW_WARPS + wid) * per;
-    const long long gend = min(ngroups, grp + per);
+    // groups are handed out in chunks of RW_CHUNK consecutive ones off a work counter (the next chunk is claimed while the
+    // current one is worked on): consecutive groups keep the same-triangle hint useful and the locate's loads in L1, the
+    // counter evens out the warps (with a static split the slowest warp set the kernel's time: SMs 60 % busy on average)
+    constexpr int RW_CHUNK = 32;
+    auto claim = [&]() { int c = 0; if (lane == 0) c = atomicAdd(work_counter, 1); return (long long)__shfl_sync(FULL, c, 0) * RW_CHUNK; };
+    long long gpos = claim(), gnext = claim(), gstop = min(ngroups, gpos + RW_CHUNK);
+    auto next_group = [&]() -> long long {
+        if (gpos >= gstop) {
+            if (gpos >= ngroups) return ngroups;
+            gpos = gnext; gstop = min(ngroups, gpos + RW_CHUNK); gnext = claim();
+            if (gpos >= ngroups) return ngroups;
+        }
+        return gpos++;
+    };
     auto load = [&](long long grp, double& r, double& z, double& ph) {
         const long long i = grp * 32 + lane;
         r = 0; z = 0; ph = 0;
-        if (grp < gend && i < n) { r = R[i]; z = Z[i]; ph = phi[i]; }
+        if (grp < ngroups && i < n) { r = R[i]; z = Z[i]; ph = phi[i]; }
     };
     // the previous group of this warp ended in triangle `hint`; in clustered input most of the next points lie in it too, so one
     // test against it (one address for the whole warp, an L1 hit) replaces the box lookup's chain of dependent loads
     // (measured: 5 900 of a group's 10 300 cycles) for them
     auto locate = [&](long long grp, double r, double z, int hint) {
-        if (!(grp < gend && grp * 32 + lane < n)) return -1;
+        if (!(grp < ngroups && grp * 32 + lane < n)) return -1;
 #ifdef TRIMEG_RW_NOLOCATE
         if (hint >= 0) return hint;
 #endif
@@ -336,10 +347,11 @@ k_gather_runs(DevTables tb, GatherMap gm, int NPP, long long n, const double* __
         return m ? __shfl_sync(FULL, t, 31 - __clz(m)) : -1;
     };
     double r, z, ph, rn, zn, phn;
+    long long grp = next_group(), grp1 = next_group();
     load(grp, r, z, ph);
-    load(grp + 1, rn, zn, phn);
+    load(grp1, rn, zn, phn);
     int t = locate(grp, r, z, -1);
-    for (unsigned round = 0; grp < gend; ++grp, ++round) {
+    for (unsigned round = 0; grp < ngroups; ++round) {
         const long long i = grp * 32 + lane;
         double s;
         RW_CLK(c0);
@@ -361,9 +373,10 @@ k_gather_runs(DevTables tb, GatherMap gm, int NPP, long long n, const double* __
         if (issue) tma_bulk_g2s(slots + (size_t)run * GSLOT, tb.coef + (long long)t * tb.tri_stride + (long long)pp0 * PLANE_STRIDE, bytes, bar);
         double rf, zf, phf;
         RW_CLK(c1);
-        load(grp + 2, rf, zf, phf);
+        const long long grp2 = next_group();
+        load(grp2, rf, zf, phf);
         RW_CLK(c1a);
-        const int tn = locate(grp + 1, rn, zn, last_of(t));
+        const int tn = locate(grp1, rn, zn, last_of(t));
         RW_CLK(c2);
 #ifdef TRIMEG_WAITSTATS
         if (lane == 0) atomicAdd(g_wait[blockIdx.x % 160] + 35, (unsigned long long)(c1a - c1));
@@ -401,6 +414,7 @@ k_gather_runs(DevTables tb, GatherMap gm, int NPP, long long n, const double* __
         RW_ACC(c0, c1, c2, c3, c4);
         r = rn; z = zn; ph = phn; t = tn;
         rn = rf; zn = zf; phn = phf;
+        grp = grp1; grp1 = grp2;
         __syncwarp();
     }
 }
