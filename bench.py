@@ -234,7 +234,7 @@ def run_gather(args, cfg, n=None, steps=None, warmup=None):
             "roofline": {"bound": "hbm", "achieved": algo / t_rand_auto / 1e9, "achieved_sorted_input": algo / t_sort_auto / 1e9, "peak": peak, "unit": "GB/s",
                          "frac": algo / t_rand_auto / 1e9 / peak, "frac_sorted_input": algo / t_sort_auto / 1e9 / peak,
                          "frac_direct_unsorted_input": algo / t_rand_direct / 1e9 / peak, "traffic": None,
-                         "kernel": "trimeg_gather, whole call in automatic mode (unsorted input: probe + k_gather_keys + scan + k_gather_scatter + k_gather_staged + k_gather_unsort; cell-sorted input: probe + k_gather)",
+                         "kernel": "trimeg_gather, whole call in automatic mode (unsorted input: probe + k_gather_keys + scan + k_gather_scatter + k_gather_staged + k_gather_unsort; cell-sorted input: probe + k_gather_runs)",
                          "algorithmic_bytes": algo, "peak_kind": "MEASURED_PEAKS.json hbm_gbs" if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else "fallback"}}
     g.close()
     del pts, spts, out, tri
