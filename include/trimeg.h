@@ -120,6 +120,20 @@ size_t trimeg_fields_bytes(const trimeg_ctx* ctx);
 int trimeg_fields_export(trimeg_ctx* ctx, void* dst_device, size_t bytes);
 int trimeg_fields_import(trimeg_ctx* ctx, const void* src_device, size_t bytes);
 
+/* trimeg_gather for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): same operation, same arguments and results as trimeg_gather with DEVICE buffers, always through the staged
+ * path (library-side binning, TMA-staged coefficient blocks), but every per-call buffer lives in ONE
+ * static device array inside the library (13.5 MiB, held by every GPU that loads the library until the process exits), so the
+ * call issues kernels and one cudaMemsetAsync on the context's stream and nothing else: no cudaMalloc / cudaFree, no events,
+ * no synchronisation.  n <= TRIMEG_GATHER_NOALLOC_MAX points per call; more is refused with BAD_ARG and a message naming
+ * the limit (split the points, or use trimeg_gather).  R, Z, phi, out [8][n], tri_out (nullable) are DEVICE pointers owned by
+ * the caller.  All contexts on a device share the array and it keeps the last call's contents: calls are safe one after the
+ * other on one stream (or otherwise ordered on the GPU); two calls that OVERLAP on the GPU (different streams or contexts
+ * of the same device without ordering) race and give wrong results.  Errors: BAD_ARG, BAD_STATE (no mesh), CUDA. */
+#define TRIMEG_GATHER_NOALLOC_MAX 131072
+int trimeg_gather_noalloc(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi, double* out,
+                          int32_t* tri_out);
+
 /* N-point gyro-average of the gather (the <...> of Eq.(4)-(6); off in the paper's runs, L320; DESIGN.md
  * reading R26): out[q][i] = mean over j = 0 .. npts-1 of the gathered quantity q at (R_i + rho_i cos(2 pi j / npts),
  * Z_i + rho_i sin(2 pi j / npts), phi_i); ring points outside the mesh contribute zero; rho_i >= 0 is the gyro-radius of

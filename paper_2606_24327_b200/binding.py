@@ -22,7 +22,7 @@ EXPORTS = [
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
     "trimeg_rhs", "trimeg_set_push_variant", "trimeg_push_variant_used", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
     "trimeg_fields_bytes", "trimeg_fields_export", "trimeg_fields_import", "trimeg_build_info", "trimeg_set_gather_mode", "trimeg_gather_kernel_ms",
-    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp", "trimeg_deposit", "trimeg_gather_gyro", "trimeg_equilibrium_set_numeric",
+    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp", "trimeg_deposit", "trimeg_gather_gyro", "trimeg_equilibrium_set_numeric", "trimeg_gather_noalloc",
 ]
 
 
@@ -74,6 +74,7 @@ def load_library():
     lib.trimeg_mesh_load.argtypes = [vp, i64, vp, i64, vp, i32, dbl]
     lib.trimeg_fields_set.argtypes = [vp, C.c_int, vp, C.c_int]
     lib.trimeg_gather.argtypes = [vp, i64, vp, vp, vp, vp, vp, C.c_int]
+    lib.trimeg_gather_noalloc.argtypes = [vp, i64, vp, vp, vp, vp, vp]
     lib.trimeg_set_gather_mode.argtypes = [vp, i32]
     lib.trimeg_gather_kernel_ms.argtypes = [vp, C.POINTER(dbl)]
     lib.trimeg_pullback.argtypes = [vp]
@@ -237,6 +238,17 @@ class Trimeg:
         po, _ = _ptr(out)
         pt, _ = _ptr(tri_out)
         self._ck(self._lib.trimeg_gather(self._h, n, pR, pZ, pP, po, pt, ms), "trimeg_gather")
+        return out, tri_out
+
+    GATHER_NOALLOC_MAX = 131072
+
+    def gather_noalloc(self, R, Z, phi, out, tri_out=None):
+        """trimeg_gather_noalloc: CUDA tensors only, caller-provided out [8, n] (and tri_out [n] or None); the library allocates
+        nothing (static scratch array, at most GATHER_NOALLOC_MAX points per call)."""
+        ptrs = [_ptr(a) for a in (R, Z, phi, out)]
+        assert all(q[1] == DEVICE for q in ptrs), "gather_noalloc takes DEVICE buffers"
+        pt = _ptr(tri_out)[0] if tri_out is not None else None
+        self._ck(self._lib.trimeg_gather_noalloc(self._h, int(R.shape[0]), *[q[0] for q in ptrs], pt), "trimeg_gather_noalloc")
         return out, tri_out
 
     def gather_gyro(self, R, Z, phi, rho, npts):

@@ -9,6 +9,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -74,6 +75,7 @@ struct trimeg_ctx {
     int *d_orig = nullptr, *d_ghist = nullptr, *d_goffs = nullptr, *d_gfill = nullptr, *d_gsums = nullptr, *d_gwork = nullptr;
     void* d_gws = nullptr;
     size_t gws_bytes = 0;
+    unsigned char* noalloc_ws = nullptr;   // device address of g_noalloc_scratch on this context's device (trimeg_create)
     int gather_mode = 0;        // 0 automatic (staged for n >= GATHER_STAGED_MIN), 1 always direct, 2 always staged
     double gather_ms[5] = {0, 0, 0, 0, 0};   // device time of the last staged gather: keys, scan, scatter, staged, unsort
     cudaEvent_t gev[7] = {};
@@ -103,6 +105,34 @@ static int fail(trimeg_ctx* c, int code, const char* fmt, ...) {
 
 static inline unsigned blocks_for(long long n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 static inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// ---- trimeg_gather_noalloc: the staged gather with its per-call scratch in a static device array instead of the grow-only
+// cudaMalloc'ed workspace, for callers that must not allocate (CUDA graph capture, serving loops).  Layout: a 256-byte header
+// (work counter, path flag, two spare words) followed by the five arrays gather_device carves from its workspace, sized for
+// TRIMEG_GATHER_NOALLOC_MAX points.  Every GPU that loads the library holds these 13.5 MiB until the process exits; every
+// call on a device shares them (calls that overlap on the GPU race).
+constexpr size_t noalloc_align256(size_t x) { return (x + 255) & ~(size_t)255; }
+constexpr size_t NOALLOC_N = TRIMEG_GATHER_NOALLOC_MAX;
+constexpr size_t NOALLOC_HEADER = 256;
+constexpr size_t NOALLOC_BYTES = NOALLOC_HEADER + 3 * noalloc_align256(sizeof(int) * NOALLOC_N) + noalloc_align256(sizeof(GPoint) * NOALLOC_N) +
+                                 noalloc_align256(sizeof(double) * 8 * NOALLOC_N);
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_BYTES];
+// In host code the name g_noalloc_scratch is only a stand-in for the symbol: its device address is looked up once per device
+// (with that device current) and kept here.
+static std::mutex g_noalloc_mutex;
+static void* g_noalloc_addr[64] = {};
+static cudaError_t noalloc_scratch_address(int device, void** out) {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+    if (!g_noalloc_addr[device]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch);     // the device of the calling thread: trimeg_create has set it
+        if (e != cudaSuccess) return e;
+        g_noalloc_addr[device] = p;
+    }
+    *out = g_noalloc_addr[device];
+    return cudaSuccess;
+}
 
 static void free_mesh(trimeg_ctx* c) {
     cudaFree(c->d_geom); cudaFree(c->d_tri); cudaFree(c->d_head); cudaFree(c->d_list);
@@ -152,6 +182,7 @@ int trimeg_create(trimeg_ctx** out, int device, void* cuda_stream) {
         delete c;
         return TRIMEG_ERR_CUDA;
     }
+    if (noalloc_scratch_address(device, (void**)&c->noalloc_ws) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
     for (auto& st : c->ev) for (auto& e : st) if (cudaEventCreate(&e) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
     for (auto& e : c->gev) if (cudaEventCreate(&e) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
     *out = c;
@@ -480,6 +511,49 @@ int trimeg_gather(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, 
     cudaFree(d); cudaFree(dt);
     if (rc != TRIMEG_OK) return rc;
     if (e != cudaSuccess) return fail(ctx, TRIMEG_ERR_CUDA, "gather: %s", cudaGetErrorString(e));
+    return TRIMEG_OK;
+}
+
+// The staged path of gather_device with every per-call buffer inside the static array: no cudaMalloc, no cudaFree, no event, no
+// synchronisation; kernels, one cudaMemsetAsync.  (The histogram / offset tables it also uses belong to the mesh and were
+// allocated by trimeg_mesh_load.)
+int trimeg_gather_noalloc(trimeg_ctx* ctx, int64_t n, const double* R, const double* Z, const double* phi, double* out, int32_t* tri_out) {
+    if (!ctx || n < 0 || (n > 0 && (!R || !Z || !phi || !out))) return fail(ctx, TRIMEG_ERR_BAD_ARG, "gather_noalloc: bad argument");
+    if (n > (int64_t)NOALLOC_N)
+        return fail(ctx, TRIMEG_ERR_BAD_ARG, "gather_noalloc: n = %lld exceeds TRIMEG_GATHER_NOALLOC_MAX = %lld points (the size of the static scratch array); use trimeg_gather",
+                    (long long)n, (long long)NOALLOC_N);
+    if (!ctx->have_mesh) return fail(ctx, TRIMEG_ERR_BAD_STATE, "gather_noalloc: call trimeg_mesh_load first");
+    if (!ctx->noalloc_ws) return fail(ctx, TRIMEG_ERR_BAD_STATE, "gather_noalloc: static scratch address unknown");
+    if (n == 0) return TRIMEG_OK;
+    CU(cudaSetDevice(ctx->device));
+    unsigned char* ptr = ctx->noalloc_ws;
+    int* work = (int*)ptr; ptr += NOALLOC_HEADER;          // [0] work counter of the staged kernel, [1] path flag
+    int* keys = (int*)ptr; ptr += noalloc_align256(sizeof(int) * NOALLOC_N);
+    int* tris = (int*)ptr; ptr += noalloc_align256(sizeof(int) * NOALLOC_N);
+    int* inv = (int*)ptr; ptr += noalloc_align256(sizeof(int) * NOALLOC_N);
+    GPoint* pts = (GPoint*)ptr; ptr += noalloc_align256(sizeof(GPoint) * NOALLOC_N);
+    double* res = (double*)ptr;
+    const long long gcnt = ctx->g_ncell + 2;
+    const int nb = (int)((gcnt + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    const unsigned sgrid = (unsigned)std::min<long long>(blocks_for(n, 256), (long long)ctx->num_sms * 32);
+    int* flag = work + 1;
+    // the array keeps the last call's contents: the header must start at zero (work counter); keys, triangles, ranks, point and
+    // result records are written for every index below n before they are read
+    CU(cudaMemsetAsync(work, 0, NOALLOC_HEADER, ctx->stream));
+    k_gather_decide<<<1, 1, 0, ctx->stream>>>(2, work + 2, flag);
+    KCHECK();
+    k_gather_keys<<<sgrid, 256, 0, ctx->stream>>>(ctx->tb, ctx->gm, n, R, Z, phi, (int)ctx->g_ncell, keys, tris, inv, ctx->d_ghist, flag);
+    KCHECK();
+    k_scan_reduce<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums, flag);
+    k_scan_sums<<<1, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_gsums, nb, flag);
+    k_scan_apply<<<nb, SCAN_THREADS, 0, ctx->stream>>>(ctx->d_ghist, gcnt, ctx->d_gsums, ctx->d_goffs, ctx->d_gfill, flag);   // also clears histogram and fill
+    KCHECK();
+    k_gather_scatter<<<sgrid, 256, 0, ctx->stream>>>(n, R, Z, phi, keys, tris, ctx->d_goffs, pts, inv, flag);
+    KCHECK();
+    k_gather_staged<<<ctx->num_sms * TRIMEG_GOCC, GTHREADS, GatherSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->g_nunits, ctx->NPP, ctx->d_goffs, pts, res, work, flag);
+    KCHECK();
+    k_gather_unsort<<<sgrid, 256, 0, ctx->stream>>>(n, tris, inv, res, ctx->d_orig, out, tri_out, flag);
+    KCHECK();
     return TRIMEG_OK;
 }
 
