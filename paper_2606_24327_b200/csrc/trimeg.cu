@@ -906,7 +906,7 @@ int trimeg_deposit(trimeg_ctx* ctx, int quantity, double* dof_out, int memspace)
     if (memspace == TRIMEG_HOST) CU(cudaMalloc(&d, bytes));
     cudaError_t e = cudaMemsetAsync(d, 0, bytes, ctx->stream);
     if (e == cudaSuccess) {
-        k_deposit<<<blocks_for(ctx->n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->P, quantity, ctx->recs[ctx->cur], ctx->n, ctx->d_tri, ctx->d_RZ, ctx->d_K, ctx->n_nodes, d);
+        k_deposit<<<(unsigned)std::min<long long>(blocks_for(ctx->n, 32 * DEP_WARPS), (long long)ctx->num_sms * 16), 32 * DEP_WARPS, 0, ctx->stream>>>(ctx->tb, ctx->P, quantity, ctx->recs[ctx->cur], ctx->n, ctx->d_tri, ctx->d_RZ, ctx->d_K, ctx->n_nodes, d);
         e = cudaGetLastError();
     }
     if (memspace == TRIMEG_HOST) {

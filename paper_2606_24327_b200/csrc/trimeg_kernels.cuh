@@ -227,6 +227,7 @@ __global__ void __launch_bounds__(256, 3) k_gather_gyro(DevTables tb, long long 
                                                         const double* __restrict__ phi, const double* __restrict__ rho, int npts, double* __restrict__ out,
                                                         int* __restrict__ tri_out) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned lanes = __ballot_sync(0xffffffffu, m < n);
     if (m >= n) return;
     const double r0 = R[m], z0 = Z[m], ph = phi[m], rh = rho[m];
     double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -236,6 +237,7 @@ __global__ void __launch_bounds__(256, 3) k_gather_gyro(DevTables tb, long long 
         sincospi(2.0 * (double)j / (double)npts, &sn, &cs);
         const double rj = fma(rh, cs, r0), zj = fma(rh, sn, z0);
         t = t >= 0 ? locate_walk(tb.bg, tb.geom, t, rj, zj) : locate_box(tb.bg, tb.geom, rj, zj);
+        __syncwarp(lanes);
         Fields f;
         gather_at(tb, t, rj, zj, ph, f);
         acc[0] += f.P; acc[1] += f.PR; acc[2] += f.PZ; acc[3] += f.Pp; acc[4] += f.A; acc[5] += f.AR; acc[6] += f.AZ; acc[7] += f.Ap;
@@ -247,9 +249,13 @@ __global__ void __launch_bounds__(256, 3) k_gather_gyro(DevTables tb, long long 
 }
 
 // one right-hand-side evaluation for one marker, fields through L1/L2; updates the triangle hint; returns 1 if outside
+// `lanes`: the lanes of the warp that make this call together.  They leave the edge walk after different numbers of hops and
+// would otherwise stay diverged through the gather and the right-hand side (the warp then runs that arithmetic once per
+// group of lanes: measured 3.0 times per warp in k_deposit before its own reconvergence point was added).
 __device__ __forceinline__ int stage_simple(const DevTables& tb, const EquilP& ep, const SpeciesP& sp, int& t, double R, double Z,
-                                            double phi, double u, double w, double mu, double p, double d[5]) {
+                                            double phi, double u, double w, double mu, double p, double d[5], unsigned lanes) {
     t = locate_walk(tb.bg, tb.geom, t, R, Z);
+    __syncwarp(lanes);
     Fields f;
     gather_at(tb, t, R, Z, phi, f);
     FieldsG<double> fg;
@@ -335,7 +341,7 @@ __device__ __forceinline__ void store_rec(const DevTables& tb, const CellMap& cm
 // left their staged block, markers outside the mesh), the initial k1, and un-sorted operation
 template <int PHASE>
 __device__ __forceinline__ void phase_global(const DevTables& tb, const EquilP& ep, const SpeciesP& sp, const CellMap& cm, const KeyOut& ko,
-                                             const Rec* src, Rec* dst, long long ri, long long m, double dt) {
+                                             const Rec* src, Rec* dst, long long ri, long long m, double dt, unsigned lanes) {
     Rec r;
     rec_load(src, ri, r);
     int t = r.tri, st = r.st;
@@ -347,7 +353,7 @@ __device__ __forceinline__ void phase_global(const DevTables& tb, const EquilP& 
     if (PHASE == PHASE_INIT) st &= ~2;
     int ev = 0;
     auto eval = [&](const double y[5], double d[5]) {
-        const int out = stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, d);
+        const int out = stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, d, lanes);
         st |= (PHASE == PHASE_A || (PHASE == PHASE_B && ev == 0)) ? out : 2 * out;
         ++ev;
         return true;
@@ -365,9 +371,16 @@ __global__ void __launch_bounds__(128) k_phase_global(DevTables tb, EquilP ep, S
                                                       Rec* dst, const int* __restrict__ perm, const int* __restrict__ index,
                                                       const int* __restrict__ first, const int* __restrict__ count, long long n, double dt) {
     const long long lo = first ? (long long)*first : 0, hi = count ? (long long)*count : n;
-    for (long long i = lo + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < hi; i += (long long)gridDim.x * blockDim.x) {
-        const long long m = index ? (long long)index[i] : i;
-        phase_global<PHASE>(tb, ep, sp, cm, ko, src, dst, perm ? (long long)perm[m] : m, m, dt);
+    // whole warps go round the loop together (the lanes of the last round that have no record sit it out), so that the lanes
+    // with a record can be named for the reconvergence points inside
+    const int lane = threadIdx.x & 31;
+    for (long long base = lo + (long long)blockIdx.x * blockDim.x + (threadIdx.x - lane); base < hi; base += (long long)gridDim.x * blockDim.x) {
+        const long long i = base + lane;
+        const unsigned lanes = __ballot_sync(0xffffffffu, i < hi);
+        if (i < hi) {
+            const long long m = index ? (long long)index[i] : i;
+            phase_global<PHASE>(tb, ep, sp, cm, ko, src, dst, perm ? (long long)perm[m] : m, m, dt, lanes);
+        }
     }
 }
 
@@ -419,6 +432,7 @@ __global__ void __launch_bounds__(128) k_fix_keys(DevTables tb, CellMap cm, KeyO
 // two-phase path; leaves the records' k stale)
 __global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, SpeciesP sp, Rec* __restrict__ recs, long long n, double dt) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned lanes = __ballot_sync(0xffffffffu, m < n);
     if (m >= n) return;
     Rec r;
     rec_load(recs, m, r);
@@ -427,16 +441,16 @@ __global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, Sp
     for (int q = 0; q < 5; ++q) y0[q] = r.y[q];
     const double mu = r.mu, p = r.p;
     int t = r.tri, st = r.st & ~2;   // variant 1 keeps no cached k1
-    st |= stage_simple(tb, ep, sp, t, y0[0], y0[1], y0[2], y0[3], y0[4], mu, p, k);
+    st |= stage_simple(tb, ep, sp, t, y0[0], y0[1], y0[2], y0[3], y0[4], mu, p, k, lanes);
 #pragma unroll
     for (int q = 0; q < 5; ++q) { acc[q] = k[q]; y[q] = fma(0.5 * dt, k[q], y0[q]); }
-    st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k);
+    st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k, lanes);
 #pragma unroll
     for (int q = 0; q < 5; ++q) { acc[q] = fma(2.0, k[q], acc[q]); y[q] = fma(0.5 * dt, k[q], y0[q]); }
-    st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k);
+    st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k, lanes);
 #pragma unroll
     for (int q = 0; q < 5; ++q) { acc[q] = fma(2.0, k[q], acc[q]); y[q] = fma(dt, k[q], y0[q]); }
-    st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k);
+    st |= stage_simple(tb, ep, sp, t, y[0], y[1], y[2], y[3], y[4], mu, p, k, lanes);
     const double h6 = dt / 6.0;
 #pragma unroll
     for (int q = 0; q < 5; ++q) r.y[q] = fma(h6, acc[q] + k[q], y0[q]);
@@ -448,12 +462,13 @@ __global__ void __launch_bounds__(128) k_push_simple(DevTables tb, EquilP ep, Sp
 // the paper's own kernel boundary (L89): the five time derivatives at the current state, caller order
 __global__ void __launch_bounds__(128) k_rhs(DevTables tb, EquilP ep, SpeciesP sp, const Rec* __restrict__ recs, long long n, double* __restrict__ out) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned lanes = __ballot_sync(0xffffffffu, m < n);
     if (m >= n) return;
     Rec r;
     rec_load(recs, m, r);
     int t = r.tri;
     double d[5];
-    stage_simple(tb, ep, sp, t, r.y[0], r.y[1], r.y[2], r.y[3], r.y[4], r.mu, r.p, d);
+    stage_simple(tb, ep, sp, t, r.y[0], r.y[1], r.y[2], r.y[3], r.y[4], r.mu, r.p, d, lanes);
 #pragma unroll
     for (int q = 0; q < 5; ++q) out[(long long)q * n + r.id] = d[q];
 }
@@ -469,10 +484,12 @@ __device__ __forceinline__ double profile_th(const SpeciesP& sp, double two_inv_
 // pullback (L99, Eq.(1), (6)): u <- u - (q/m) A_par,  w <- w + p (q/m) A_par d ln f0/du at the old u,  d ln f0/du = -u / T(r)
 __global__ void __launch_bounds__(128) k_pullback(DevTables tb, EquilP ep, SpeciesP sp, Rec* __restrict__ recs, long long n) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned lanes = __ballot_sync(0xffffffffu, m < n);
     if (m >= n) return;
     Rec r;
     rec_load(recs, m, r);
     const int t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
+    __syncwarp(lanes);                       // reconverge after the walk (see stage_simple)
     if (t < 0) { r.st |= 1; }
     else {
         Fields f;
@@ -488,10 +505,12 @@ __global__ void __launch_bounds__(128) k_pullback(DevTables tb, EquilP ep, Speci
 // density (L100): value of grid field `which` at every marker, caller order
 __global__ void __launch_bounds__(128) k_density_g2p(DevTables tb, int which, const Rec* __restrict__ recs, long long n, double* __restrict__ out) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned lanes = __ballot_sync(0xffffffffu, m < n);
     if (m >= n) return;
     Rec r;
     rec_load(recs, m, r);
     const int t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
+    __syncwarp(lanes);                       // reconverge after the walk (see stage_simple)
     Fields f;
     gather_at(tb, t, r.y[0], r.y[1], r.y[2], f);
     out[r.id] = which ? f.A : f.P;
@@ -499,10 +518,12 @@ __global__ void __launch_bounds__(128) k_density_g2p(DevTables tb, int which, co
 // distribution-function interpolation (L101): f0 = n T^-3/2 exp(-(v^2/2 + mu B)/T) at the marker's position and v = u - (q/m) A_par
 __global__ void __launch_bounds__(128) k_f_interp(DevTables tb, EquilP ep, SpeciesP sp, const Rec* __restrict__ recs, long long n, double* __restrict__ out) {
     long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned lanes = __ballot_sync(0xffffffffu, m < n);
     if (m >= n) return;
     Rec r;
     rec_load(recs, m, r);
     const int t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
+    __syncwarp(lanes);                       // reconverge after the walk (see stage_simple)
     Fields f;
     gather_at(tb, t, r.y[0], r.y[1], r.y[2], f);
     Equil<double> e;
@@ -519,114 +540,121 @@ __global__ void __launch_bounds__(128) k_f_interp(DevTables tb, EquilP ep, Speci
 //   b[k][v][c] += q_p B_k(phi_p) N_{v,c}(R_p, Z_p),
 // N_{v,c} = the element's nodal basis functions.  With F = m . c (m = the 21 monomials at the point), c = c0 - Nul (K c0_5),
 // c0 = Aplus d_ref, d_ref = T_J d (k_fields_set), the 18 basis values are N = T_J^T Aplus^T (m - S^T K^T Nul^T m).
-// One thread per marker record.  The 72 contributions of a marker (3 nodes x 6 components x 4 planes) go to addresses that
-// depend on its cell (triangle, toroidal interval) only, and the store is in cell order after a push: a warp then holds a
-// few runs of markers of the same cell, each run is summed with warp shuffles and added with ONE atomic per address
-// (a per-cell segmented reduction); a warp with many different cells (unsorted store) falls back to per-marker atomics.
-__global__ void __launch_bounds__(128) k_deposit(DevTables tb, int P, int quantity, const Rec* __restrict__ recs, long long n, const int* __restrict__ tri,
+// One thread per marker record: its 18 basis values (times the charge) and 4 toroidal weights go into the warp's rows in
+// shared memory.  The 72 contributions of a marker (3 nodes x 6 components x 4 planes) go to addresses that depend on its
+// cell (triangle, toroidal interval) only, and the store is in cell order after a push: a warp then holds a few runs of
+// markers of the same cell; per run the lanes share the 72 sums (lane l takes outputs l, l + 32, l + 64 and walks over the
+// run's rows), ONE atomic per address.  An unsorted store degenerates to runs of one marker, i.e. per-marker atomics.
+// (History, per 1e8 markers on config 3: five-step segmented shuffle sums of all 72 values 27.8 ms; sums through shared memory
+// 14.7 ms; the moments summed per run and mapped once per run instead of per marker 20.4 ms - fewer instructions, but a
+// chain of five dependent warp-wide stages per run; this form, with the per-marker map written out: DESIGN.md section 6.)
+constexpr int DEP_STRIDE = 23, DEP_WARPS = 4;      // row: 18 basis values x charge, 4 toroidal weights, pad (odd stride: conflict-free)
+__global__ void __launch_bounds__(32 * DEP_WARPS) k_deposit(DevTables tb, int P, int quantity, const Rec* __restrict__ recs, long long n, const int* __restrict__ tri,
                                                  const double* __restrict__ RZ, const double* __restrict__ Kmat, long long n_nodes, double* __restrict__ out) {
     constexpr unsigned FULL = 0xffffffffu;
-    const long long mi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int lane = threadIdx.x & 31;
-    int t = -1, k = 0, key = -1;
-    int nd[3] = {0, 0, 0};
-    double N[18], w[4] = {0.0, 0.0, 0.0, 0.0}, charge = 0.0;
-#pragma unroll
-    for (int q = 0; q < 18; ++q) N[q] = 0.0;
-    if (mi < n) {
+    __shared__ double s_rows[DEP_WARPS][32][DEP_STRIDE];
+    __shared__ int s_meta[DEP_WARPS][32][4];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double (*rows)[DEP_STRIDE] = s_rows[wid];
+    int (*meta)[4] = s_meta[wid];
+    const long long ngroups = (n + 31) / 32;
+    for (long long grp = (long long)blockIdx.x * DEP_WARPS + wid; grp < ngroups; grp += (long long)gridDim.x * DEP_WARPS) {
+        const long long mi = grp * 32 + lane;
+        int t = -1, k = 0, key = -1;
+        double w[4] = {0.0, 0.0, 0.0, 0.0};
         Rec r;
-        rec_load(recs, mi, r);
-        t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
-        if (t >= 0) {
-            const TriGeom g = tb.geom[t];
-            double xi, eta, dw[4];
-            ref_coords(g, r.y[0], r.y[1], xi, eta);
-            k = bspline_weights(tb.tor, r.y[2], w, dw);
-            key = t * P + k;
-            charge = quantity == 0 ? r.y[4] : r.y[4] * r.y[3];
-            // monomials xi^i eta^j at j-major index off_j + i
-            double m[21];
-            {
-                double xp[6], ep[6];
-                xp[0] = ep[0] = 1.0;
-#pragma unroll
-                for (int i = 1; i < 6; ++i) { xp[i] = xp[i - 1] * xi; ep[i] = ep[i - 1] * eta; }
-                int idx = 0;
-#pragma unroll
-                for (int j = 0; j < 6; ++j)
-#pragma unroll
-                    for (int i = 0; i < 6 - j; ++i) m[idx++] = xp[i] * ep[j];
-            }
-            double y[3] = {0.0, 0.0, 0.0};
-#pragma unroll
-            for (int i = 0; i < 21; ++i) { y[0] = fma(c_Nul[i * 3], m[i], y[0]); y[1] = fma(c_Nul[i * 3 + 1], m[i], y[1]); y[2] = fma(c_Nul[i * 3 + 2], m[i], y[2]); }
-            const int qi[6] = {5, 6 + 4, 11 + 3, 15 + 2, 18 + 1, 20};
-            const double* K = Kmat + (long long)t * 18;
-#pragma unroll
-            for (int mm = 0; mm < 6; ++mm) m[qi[mm]] -= fma(y[0], K[mm], fma(y[1], K[6 + mm], y[2] * K[12 + mm]));
-            double a[18];
-#pragma unroll
-            for (int q = 0; q < 18; ++q) {
-                double s = 0.0;
-#pragma unroll
-                for (int i = 0; i < 21; ++i) s = fma(c_Aplus[i * 18 + q], m[i], s);
-                a[q] = s;
-            }
-            nd[0] = tri[3 * t]; nd[1] = tri[3 * t + 1]; nd[2] = tri[3 * t + 2];
-            const double x0 = RZ[2 * nd[0]], y0 = RZ[2 * nd[0] + 1];
-            const double j11 = RZ[2 * nd[1]] - x0, j21 = RZ[2 * nd[1] + 1] - y0, j12 = RZ[2 * nd[2]] - x0, j22 = RZ[2 * nd[2] + 1] - y0;
-#pragma unroll
-            for (int v = 0; v < 3; ++v) {
-                const double* av = a + 6 * v;
-                N[6 * v + 0] = av[0];
-                N[6 * v + 1] = fma(j11, av[1], j12 * av[2]);
-                N[6 * v + 2] = fma(j21, av[1], j22 * av[2]);
-                N[6 * v + 3] = fma(j11 * j11, av[3], fma(j11 * j12, av[4], j12 * j12 * av[5]));
-                N[6 * v + 4] = fma(2.0 * j11 * j21, av[3], fma(j11 * j22 + j21 * j12, av[4], 2.0 * j12 * j22 * av[5]));
-                N[6 * v + 5] = fma(j21 * j21, av[3], fma(j21 * j22, av[4], j22 * j22 * av[5]));
-            }
+        if (mi < n) {
+            rec_load(recs, mi, r);
+            t = locate_walk(tb.bg, tb.geom, r.tri, r.y[0], r.y[1]);
         }
-    }
-    auto addr = [&](int v, int pa, int kk, const int* nodes) {
-        int pl = kk - 1 + pa;
-        if (pl < 0) pl += P; else if (pl >= P) pl -= P;
-        return out + ((long long)pl * n_nodes + nodes[v]) * 6;
-    };
-    const int prevk = __shfl_up_sync(FULL, key, 1);
-    const unsigned starts = __ballot_sync(FULL, lane == 0 || prevk != key);
-    if (__popc(starts) <= 16) {
-        // segmented reduction over the runs of equal cells (contiguous lane ranges), all runs at once: after the five steps
-        // the first lane of every run holds the run's sum
-        const unsigned above = lane == 31 ? 0u : (starts & ~((2u << lane) - 1u));
-        const int run_end = above ? __ffs(above) - 1 : 32;
-        const bool leader = ((starts >> lane) & 1u) && key >= 0;
+        // the lanes leave the walk after different numbers of hops: without this they stay diverged and the warp runs the
+        // arithmetic below once per group of lanes (measured: 3.0 times per warp)
+        __syncwarp();
+        {
+            if (t >= 0) {
+                const TriGeom g = tb.geom[t];
+                double xi, eta, dw[4];
+                ref_coords(g, r.y[0], r.y[1], xi, eta);
+                k = bspline_weights(tb.tor, r.y[2], w, dw);
+                key = t * P + k;
+                const double charge = quantity == 0 ? r.y[4] : r.y[4] * r.y[3];
+                // charge x monomials xi^i eta^j at j-major index off_j + i
+                double m[21];
+                {
+                    double xp[6], ep[6];
+                    xp[0] = 1.0; ep[0] = charge;
 #pragma unroll
-        for (int v = 0; v < 3; ++v)
+                    for (int i = 1; i < 6; ++i) { xp[i] = xp[i - 1] * xi; ep[i] = ep[i - 1] * eta; }
+                    int idx = 0;
 #pragma unroll
-            for (int pa = 0; pa < 4; ++pa) {
-                const double qw = charge * w[pa];
-                double* base = addr(v, pa, k, nd);
+                    for (int j = 0; j < 6; ++j)
 #pragma unroll
-                for (int c = 0; c < 6; ++c) {
-                    double sum = qw * N[6 * v + c];
+                        for (int i = 0; i < 6 - j; ++i) m[idx++] = xp[i] * ep[j];
+                }
+                double y0 = 0.0, y1 = 0.0, y2 = 0.0;
 #pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const double up = __shfl_down_sync(FULL, sum, o);
-                        if (lane + o < run_end) sum += up;
+                for (int i = 0; i < 21; ++i) { y0 = fma(c_Nul[i * 3], m[i], y0); y1 = fma(c_Nul[i * 3 + 1], m[i], y1); y2 = fma(c_Nul[i * 3 + 2], m[i], y2); }
+                const double* K = Kmat + (long long)t * 18;
+                // the six degree-5 monomials sit at 5, 10, 14, 17, 19, 20
+                m[5] -= fma(y0, K[0], fma(y1, K[6], y2 * K[12]));
+                m[10] -= fma(y0, K[1], fma(y1, K[7], y2 * K[13]));
+                m[14] -= fma(y0, K[2], fma(y1, K[8], y2 * K[14]));
+                m[17] -= fma(y0, K[3], fma(y1, K[9], y2 * K[15]));
+                m[19] -= fma(y0, K[4], fma(y1, K[10], y2 * K[16]));
+                m[20] -= fma(y0, K[5], fma(y1, K[11], y2 * K[17]));
+                const int n0 = tri[3 * t], n1 = tri[3 * t + 1], n2 = tri[3 * t + 2];
+                meta[lane][0] = n0; meta[lane][1] = n1; meta[lane][2] = n2;
+                const double x0 = RZ[2 * n0], yy0 = RZ[2 * n0 + 1];
+                const double j11 = RZ[2 * n1] - x0, j21 = RZ[2 * n1 + 1] - yy0, j12 = RZ[2 * n2] - x0, j22 = RZ[2 * n2 + 1] - yy0;
+                const double t11 = j11 * j11, t12 = j11 * j12, t22 = j12 * j12, u11 = 2.0 * j11 * j21, u12 = fma(j11, j22, j21 * j12), u22 = 2.0 * j12 * j22,
+                             v11 = j21 * j21, v12 = j21 * j22, v22 = j22 * j22;
+#pragma unroll
+                for (int v = 0; v < 3; ++v) {
+                    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0, a4 = 0.0, a5 = 0.0;      // six independent chains
+#pragma unroll
+                    for (int i = 0; i < 21; ++i) {
+                        a0 = fma(c_Aplus[i * 18 + 6 * v + 0], m[i], a0); a1 = fma(c_Aplus[i * 18 + 6 * v + 1], m[i], a1);
+                        a2 = fma(c_Aplus[i * 18 + 6 * v + 2], m[i], a2); a3 = fma(c_Aplus[i * 18 + 6 * v + 3], m[i], a3);
+                        a4 = fma(c_Aplus[i * 18 + 6 * v + 4], m[i], a4); a5 = fma(c_Aplus[i * 18 + 6 * v + 5], m[i], a5);
                     }
-                    if (leader) atomicAdd(base + c, sum);
+                    rows[lane][6 * v + 0] = a0;
+                    rows[lane][6 * v + 1] = fma(j11, a1, j12 * a2);
+                    rows[lane][6 * v + 2] = fma(j21, a1, j22 * a2);
+                    rows[lane][6 * v + 3] = fma(t11, a3, fma(t12, a4, t22 * a5));
+                    rows[lane][6 * v + 4] = fma(u11, a3, fma(u12, a4, u22 * a5));
+                    rows[lane][6 * v + 5] = fma(v11, a3, fma(v12, a4, v22 * a5));
                 }
             }
-    } else if (t >= 0) {
+        }
 #pragma unroll
-        for (int v = 0; v < 3; ++v)
+        for (int pa = 0; pa < 4; ++pa) rows[lane][18 + pa] = w[pa];
+        meta[lane][3] = k;
+        const int prevk = __shfl_up_sync(FULL, key, 1);
+        unsigned starts = __ballot_sync(FULL, lane == 0 || prevk != key);
+        const unsigned inside = __ballot_sync(FULL, key >= 0);
+        __syncwarp();
+        while (starts) {
+            const int b = __ffs(starts) - 1;
+            starts &= starts - 1;
+            const int e = starts ? __ffs(starts) - 1 : 32;
+            if (!((inside >> b) & 1u)) continue;
+            const int kk = meta[b][3];
 #pragma unroll
-            for (int pa = 0; pa < 4; ++pa) {
-                double* base = addr(v, pa, k, nd);
-                const double qw = charge * w[pa];
-#pragma unroll
-                for (int c = 0; c < 6; ++c) atomicAdd(base + c, qw * N[6 * v + c]);
+            for (int pass = 0; pass < 3; ++pass) {
+                const int o = lane + 32 * pass;           // output pa * 18 + (6 v + c)
+                if (o < 72) {
+                    const int pa = o / 18, q = o - 18 * pa, v = q / 6, c = q - 6 * v;
+                    double s0 = 0.0, s1 = 0.0;
+                    int pp = b;
+                    for (; pp + 1 < e; pp += 2) { s0 = fma(rows[pp][q], rows[pp][18 + pa], s0); s1 = fma(rows[pp + 1][q], rows[pp + 1][18 + pa], s1); }
+                    if (pp < e) s0 = fma(rows[pp][q], rows[pp][18 + pa], s0);
+                    int pl = kk - 1 + pa;
+                    if (pl < 0) pl += P; else if (pl >= P) pl -= P;
+                    atomicAdd(out + ((long long)pl * n_nodes + meta[b][v]) * 6 + c, s0 + s1);
+                }
             }
+        }
+        __syncwarp();
     }
 }
 
