@@ -242,6 +242,36 @@ def run_gather(args, cfg, n=None, steps=None, warmup=None):
     return line
 
 
+def run_other_kernels(g, cfg, n, reps=3):
+    """The per-marker calls beside the push (SURVEY.md 8(f) rows N2 / N3 and the paper's own kernel boundary, L89, L97-103) on the
+    markers as the push left them (cell-ordered store), device buffers: milliseconds per call and the share of the HBM
+    roofline for the bytes each must move (record in, result out).  Pullback last: it changes u and w."""
+    import torch
+    peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"] if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else 6650.0
+
+    def timed(f):
+        f()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            f()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    grid = 8 * 6 * cfg.n_planes * (cfg.nr + 1) * cfg.ntheta       # deposit: the DOF array written once
+    calls = [("trimeg_rhs", lambda: g.rhs(), 128 + 40, 0), ("trimeg_density_g2p", lambda: g.density_g2p(0), 128 + 8, 0),
+             ("trimeg_f_interp", lambda: g.f_interp(), 128 + 8, 0), ("trimeg_deposit", lambda: g.deposit(0), 128, grid),
+             ("trimeg_pullback", lambda: g.pullback(), 256, 0)]
+    rec = {"markers": n, "reps": reps, "hbm_peak_GBps": peak}
+    for name, f, bytes_per_marker, extra in calls:
+        ms = timed(f)
+        algo = bytes_per_marker * n + extra
+        rec[name] = {"ms": ms, "markers_per_s": n / (ms * 1e-3), "algorithmic_bytes": algo, "frac_hbm": algo / (ms * 1e-3) / 1e9 / peak}
+    return rec
+
+
 def run_push_extra(cfg, sort_every, steps=10, warmup=3, parity_n=2000):
     """One more BASELINE config through the same library on cuda:0 (device-resident, both phases' kernels, sort inside the
     timed region), with a small oracle sample; for the `other_configs` record of the bench line."""
@@ -493,7 +523,14 @@ def main():
                 "slow_path_evals": slow, "retired_markers": retired, "parity": parity, "fields_bcast": fields_bcast}
         if not args.no_extras and world == 1 and args.config == 3 and n == cfg.n_markers:
             # the other BASELINE configs, same library, same run (not the headline)
-            del dev, pinned_out, host, views
+            del pinned_out, host, views
+            try:
+                g.markers_bind(*[dev[k] for k in KEYS])
+                g.push_rk4(cfg.dt, 2)
+                line["other_kernels"] = run_other_kernels(g, cfg, n)
+            except Exception as ex:
+                line["other_kernels"] = {"error": repr(ex)}
+            del dev
             g.close()
             torch.cuda.empty_cache()
             extras = {}

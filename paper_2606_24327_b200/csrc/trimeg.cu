@@ -849,8 +849,11 @@ int trimeg_rhs(trimeg_ctx* ctx, double* out, int memspace) {
     const long long n = ctx->n;
     double* d = out;
     if (memspace == TRIMEG_HOST) CU(cudaMalloc(&d, sizeof(double) * 5 * (size_t)n));
-    k_rhs<<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->recs[ctx->cur], n, d);
+    // staged through the inactive record buffer (free between steps; 64 of its 128 bytes per marker)
+    double* stage = (double*)ctx->recs[ctx->cur ^ 1];
+    k_rhs<<<blocks_for(n, 128), 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->recs[ctx->cur], n, d, stage);
     cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) { k_rhs_unpack<<<blocks_for(n, 256), 256, 0, ctx->stream>>>(stage, n, d); e = cudaGetLastError(); }
     if (memspace == TRIMEG_HOST) {
         if (e == cudaSuccess) e = cudaMemcpyAsync(out, d, sizeof(double) * 5 * n, cudaMemcpyDeviceToHost, ctx->stream);
         cudaError_t e2 = cudaStreamSynchronize(ctx->stream);

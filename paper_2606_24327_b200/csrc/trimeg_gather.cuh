@@ -56,14 +56,6 @@ struct GatherMap {   // bin numbering of the gather: super-cell (patch, window) 
 };
 struct __align__(32) GPoint { double R, Z, phi; int id, tri; };   // one point in cell order (32 B = one sector)
 static_assert(sizeof(GPoint) == 32, "GPoint");
-// 256-bit global accesses (sm_100: LDG/STG.256): a 32-byte record is one request and one full sector
-TRIMEG_DI void ld256(const void* p, double& a, double& b, double& c, double& d) {
-    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
-}
-TRIMEG_DI void st256(void* p, double a, double b, double c, double d) {
-    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
-}
-
 // Which path?  A strided sample of runs of 32 consecutive points: if most neighbours share a cell the caller's order is
 // already clustered and the direct kernel (coefficients through L1/L2) is the faster one; otherwise the points are binned.
 // flag[0] = 1 direct, 2 staged; every kernel of either path returns at once if the flag names the other path, so the choice

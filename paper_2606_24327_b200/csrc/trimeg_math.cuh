@@ -411,4 +411,12 @@ TRIMEG_DI void rhs_eval(const EquilP& ep, const SpeciesP& sp, T R, T Z, T u, T w
     rhs_post(sp, pre, u, w, mu, p, f, d);
 }
 
+// 256-bit global accesses (sm_100: LDG/STG.256): a 32-byte record is one request and one full sector
+TRIMEG_DI void ld256(const void* p, double& a, double& b, double& c, double& d) {
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
+TRIMEG_DI void st256(void* p, double a, double b, double c, double d) {
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
 }  // namespace trimeg
