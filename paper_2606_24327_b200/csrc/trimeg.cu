@@ -475,7 +475,7 @@ static int gather_device(trimeg_ctx* ctx, long long n, const double* R, const do
     k_gather_staged<<<ctx->num_sms * TRIMEG_GOCC, GTHREADS, GatherSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->g_nunits, ctx->NPP, ctx->d_goffs, pts, res, ctx->d_gwork, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[4], ctx->stream));
-    k_gather_unsort<<<sgrid, 256, 0, ctx->stream>>>(n, tris, inv, res, ctx->d_orig, out, tri_out, flag);
+    k_gather_unsort<<<sgrid, 256, 0, ctx->stream>>>(n, tris, res, ctx->d_orig, out, tri_out, flag);
     KCHECK();
     CU(cudaEventRecord(ctx->gev[5], ctx->stream));
     k_gather_runs<<<ctx->num_sms * TRIMEG_RW_OCC, 32 * RW_WARPS, GatherRunsSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->NPP, n, R, Z, phi, out, tri_out, ctx->d_gwork, flag);
@@ -552,7 +552,7 @@ int trimeg_gather_noalloc(trimeg_ctx* ctx, int64_t n, const double* R, const dou
     KCHECK();
     k_gather_staged<<<ctx->num_sms * TRIMEG_GOCC, GTHREADS, GatherSmem::BYTES, ctx->stream>>>(ctx->tb, ctx->gm, ctx->g_nunits, ctx->NPP, ctx->d_goffs, pts, res, work, flag);
     KCHECK();
-    k_gather_unsort<<<sgrid, 256, 0, ctx->stream>>>(n, tris, inv, res, ctx->d_orig, out, tri_out, flag);
+    k_gather_unsort<<<sgrid, 256, 0, ctx->stream>>>(n, tris, res, ctx->d_orig, out, tri_out, flag);
     KCHECK();
     return TRIMEG_OK;
 }

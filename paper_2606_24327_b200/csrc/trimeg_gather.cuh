@@ -7,16 +7,16 @@
 //                        the staged kernel does not care about the order within it, and 8x fewer counters than cells stay
 //                        in L2;
 //   2. scan              (the push's counting-sort kernels) -> bin offsets;
-//   3. k_gather_scatter  caller order: position = offset + rank; 32-byte point record written there (a full sector),
-//                        position kept per caller index;
+//   3. k_gather_scatter  caller order: position = offset + rank; 32-byte point record (with the caller's index) written there
+//                        (a full sector);
 //   4. k_gather_staged   persistent CTAs, one super-cell (GT triangles x GW toroidal intervals) at a time, dealt out
 //                        round-robin: its coefficient block, geometry and point records arrive by TMA bulk copies (two
 //                        stages, 'landed' / 'consumed' mbarriers, no CTA-wide barrier), warps evaluate its points from
-//                        shared memory and write 64-byte result records in bin order (coalesced).  Bound by shared-memory
-//                        bandwidth (1 344 B of coefficients per point, ~4 wavefronts per LDS.128);
-//   5. k_gather_unsort   caller order: result record (fetched by a lane pair as one 64-byte request) -> the caller's eight
-//                        arrays (coalesced writes), triangle id.
-// HBM bytes per point: 36 + 68 + (96 + coefficients) + 140, against 92 + coefficients algorithmic; DESIGN.md section 6,
+//                        shared memory and write each 64-byte result record at the CALLER's index (two full sectors,
+//                        scattered).  Bound by shared-memory bandwidth (1 344 B of coefficients per point, ~4 wavefronts
+//                        per LDS.128);
+//   5. k_gather_unsort   caller order: result record (read in order) -> the caller's eight arrays, triangle id.
+// HBM bytes per point: 36 + 64 + (96 + coefficients) + 136, against 92 + coefficients algorithmic; DESIGN.md section 6,
 // profiles/r02_gather_cfg4.md.
 #pragma once
 
@@ -100,13 +100,12 @@ __global__ void __launch_bounds__(256) k_gather_keys(DevTables tb, GatherMap gm,
 
 __global__ void __launch_bounds__(256) k_gather_scatter(long long n, const double* __restrict__ R, const double* __restrict__ Z, const double* __restrict__ phi,
                                                         const int* __restrict__ keys, const int* __restrict__ tris, const int* __restrict__ offs,
-                                                        GPoint* __restrict__ pts, int* __restrict__ inv, const int* __restrict__ flag) {
+                                                        GPoint* __restrict__ pts, const int* __restrict__ ranks, const int* __restrict__ flag) {
     if (*flag != 2) return;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         const int key = keys[i];
-        const int pos = offs[key] + inv[i];      // inv[] comes in holding the rank within the cell and leaves holding the position
+        const int pos = offs[key] + ranks[i];    // rank within the bin: the value the histogram atomic of k_gather_keys returned
         st256(pts + pos, R[i], Z[i], phi[i], __hiloint2double(tris[i], (int)i));     // (id, tri) in the low and high word
-        inv[i] = pos;
     }
 }
 
@@ -212,15 +211,17 @@ k_gather_staged(DevTables tb, GatherMap gm, int nunits, int NPP, const int* __re
             gather_cell<true, double>(ld, xi, eta, bw, dw, acc);
             Fields f;
             to_fields(g, acc, f);
-            st256(res + 8ll * pos, f.P, f.PR, f.PZ, f.Pp);
-            st256(res + 8ll * pos + 4, f.A, f.AR, f.AZ, f.Ap);
+            // the result record goes to the CALLER's index (two full sectors, scattered), so that the last pass reads its input
+            // in order: 3.0 + 1.1 ms against 2.9 + 1.8 ms with records in bin order and a random-read un-sort (config 4)
+            st256(res + 8ll * p.id, f.P, f.PR, f.PZ, f.Pp);
+            st256(res + 8ll * p.id + 4, f.A, f.AR, f.AZ, f.Ap);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(done_of(s));            // this warp is done with stage s
     }
 }
 
-__global__ void __launch_bounds__(256) k_gather_unsort(long long n, const int* __restrict__ tris, const int* __restrict__ inv, const double* __restrict__ res,
+__global__ void __launch_bounds__(256) k_gather_unsort(long long n, const int* __restrict__ tris, const double* __restrict__ res,
                                                        const int* __restrict__ orig, double* __restrict__ out, int* __restrict__ tri_out,
                                                        const int* __restrict__ flag) {
     if (*flag != 2) return;
@@ -232,7 +233,7 @@ __global__ void __launch_bounds__(256) k_gather_unsort(long long n, const int* _
     const long long nround = (n + 31) / 32 * 32;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nround; i += (long long)gridDim.x * blockDim.x) {
         int t = -1, pos = 0;
-        if (i < n) { t = tris[i]; pos = inv[i]; }
+        if (i < n) { t = tris[i]; pos = (int)i; }
         double q[2][4];
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
