@@ -346,6 +346,33 @@ def test_deposit_matches_oracle_and_is_the_transpose_of_the_gather():
     assert abs(float((b * dof).sum()) - float((q * F[0]).sum())) < 1e-10 * np.abs(q * F[0]).sum()
 
 
+@pytest.mark.parametrize("sort_every", [1, 3])
+def test_read_only_calls_between_pushes_leave_the_push_unchanged(sort_every):
+    """trimeg_rhs stages its results in the inactive record buffer, trimeg_deposit / density / f-interpolation / markers_get read
+    the store: none of them may change what the next push computes.  5 steps, all of those calls, 5 more steps = the oracle's
+    10 steps (1e-10), for the re-sorting push and for stale-order steps in between."""
+    cfg = dataclasses.replace(synth.CONFIGS[1], em=True, nr=12, ntheta=36, n_planes=16, n_markers=30_011)
+    RZ, tri, o, g, m = _make(cfg)
+    d = _dev(m)
+    g.set_push_variant(0)
+    g.set_sort_interval(sort_every)
+    g.markers_bind(*[d[k] for k in KEYS])
+    g.push_rk4(cfg.dt, 5)
+    rhs_a = g.rhs(host=True)
+    g.density_g2p(1); g.f_interp(); g.deposit(0); g.deposit(1)
+    mid = g.markers_get()                                   # DEVICE arrays
+    rhs_b = g.rhs(host=True)
+    assert np.array_equal(rhs_a, rhs_b)
+    ref, _ = o.rhs(*[mid[k].cpu().numpy() if k in mid else m[k] for k in KEYS])
+    for q in range(5):
+        assert _rel(rhs_b[q], ref[q]) < 1e-11, (q, _rel(rhs_b[q], ref[q]))
+    g.push_rk4(cfg.dt, 5)
+    res = g.markers_get(host=True)
+    exp = o.push_rk4(*[m[k] for k in KEYS], cfg.dt, 10)
+    _compare_state(res, exp, np.arange(cfg.n_markers), cfg.phi_period, STATE_TOL, f"push / calls / push, sort_every={sort_every}")
+    assert g.push_variant_used() == 0
+
+
 @pytest.mark.parametrize("npts", [1, 4, 8])
 def test_gather_gyro_matches_oracle(npts):
     """trimeg_gather_gyro (N-point gyro-average of the gather, reading R26) against the oracle on the unstructured EM mesh:
