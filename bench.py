@@ -411,6 +411,7 @@ def main():
     g.set_sort_interval(args.sort_every)
     g.markers_bind(*[dev[k] for k in KEYS])
     dfma = g.bench_dfma()
+    dfma3 = g.bench_dfma_mix(1)     # DFMAs whose three operands are three different register pairs (2/3 of the pipe's rate: operand fetch)
 
     # ---- device-resident timing
     for _ in range(args.warmup):
@@ -517,6 +518,9 @@ def main():
                                             "source": "python -m paper_2606_24327_b200.flopcount"},
                              "peak_kind": "nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (derived, DESIGN.md)",
                              "measured_dfma_tflops": dfma, "frac_of_measured_dfma": achieved / dfma,
+                             "measured_dfma_three_register_operands_tflops": dfma3,
+                             "note_operands": "a DFMA with three different register-pair operands and no operand reuse issues every 3 cycles instead of 2 "
+                                              "(trimeg_bench_dfma_mix; 235 of the ~610 FP64 instructions of an evaluation are of that kind): DESIGN.md section 6",
                              "whole_step_frac": step_achieved / FP64_PEAK_TFLOPS,
                              "hbm_algorithmic_GBps": ALGO_BYTES_PER_LAUNCH * n / kern_s / 1e9},
                 "step_breakdown_ms": {"sort": sort_ms, "push": 1e3 * kern_s * launches_per_step, "finish": finish_ms},

@@ -209,6 +209,10 @@ int trimeg_push_variant_used(trimeg_ctx* ctx, int32_t* out);
 /* Diagnostics used by the benchmark: achieved FP64 FMA throughput of this device in TFLOP/s
  * (a register-only DFMA loop; the roofline's measured "alu" peak). */
 int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops);
+/* The same loop with the register operands of real arithmetic: kind 1 = accumulator, multiplier and addend are three
+ * different register pairs in every DFMA; kind 2 = Horner-like, one multiplier shared by eight chains with different addends.
+ * (trimeg_bench_dfma's loop takes multiplier and addend from two fixed registers.)  Errors: BAD_ARG, OOM, CUDA. */
+int trimeg_bench_dfma_mix(trimeg_ctx* ctx, int32_t kind, double* tflops);
 /* The three other grid-to-particle kernels of the paper ("pullback treatment", "density calculation",
  * "distribution-function interpolation"; "all these kernels rely on the same G2P function").  The paper gives each one
  * sentence; what they compute here is DESIGN.md readings R22-R24.  All work on the bound marker store.

@@ -22,7 +22,7 @@ EXPORTS = [
     "trimeg_markers_bind", "trimeg_markers_get", "trimeg_sort", "trimeg_set_sort_interval", "trimeg_push_rk4",
     "trimeg_rhs", "trimeg_set_push_variant", "trimeg_push_variant_used", "trimeg_bench_dfma", "trimeg_push_stats", "trimeg_push_kernel_ms",
     "trimeg_fields_bytes", "trimeg_fields_export", "trimeg_fields_import", "trimeg_build_info", "trimeg_set_gather_mode", "trimeg_gather_kernel_ms",
-    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp", "trimeg_deposit", "trimeg_gather_gyro", "trimeg_equilibrium_set_numeric", "trimeg_gather_noalloc",
+    "trimeg_pullback", "trimeg_density_g2p", "trimeg_f_interp", "trimeg_deposit", "trimeg_gather_gyro", "trimeg_equilibrium_set_numeric", "trimeg_gather_noalloc", "trimeg_bench_dfma_mix",
 ]
 
 
@@ -99,6 +99,7 @@ def load_library():
     lib.trimeg_set_push_variant.argtypes = [vp, i32]
     lib.trimeg_push_variant_used.argtypes = [vp, C.POINTER(i32)]
     lib.trimeg_bench_dfma.argtypes = [vp, C.POINTER(dbl)]
+    lib.trimeg_bench_dfma_mix.argtypes = [vp, i32, C.POINTER(dbl)]
     lib.trimeg_push_stats.argtypes = [vp, C.POINTER(i64)]
     lib.trimeg_push_kernel_ms.argtypes = [vp, C.POINTER(dbl)]
     _lib = lib
@@ -361,6 +362,11 @@ class Trimeg:
     def bench_dfma(self):
         v = C.c_double(0)
         self._ck(self._lib.trimeg_bench_dfma(self._h, C.byref(v)), "trimeg_bench_dfma")
+        return v.value
+
+    def bench_dfma_mix(self, kind):
+        v = C.c_double(0)
+        self._ck(self._lib.trimeg_bench_dfma_mix(self._h, int(kind), C.byref(v)), "trimeg_bench_dfma_mix")
         return v.value
 
     def push_stats(self):

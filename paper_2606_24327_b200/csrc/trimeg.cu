@@ -948,6 +948,36 @@ int trimeg_bench_dfma(trimeg_ctx* ctx, double* tflops) {
     return TRIMEG_OK;
 }
 
+int trimeg_bench_dfma_mix(trimeg_ctx* ctx, int32_t kind, double* tflops) {
+    if (!ctx || !tflops || kind < 1 || kind > 2) return fail(ctx, TRIMEG_ERR_BAD_ARG, "bench_dfma_mix: kind 1 (three register operands) or 2 (shared multiplier)");
+    CU(cudaSetDevice(ctx->device));
+    const int nb = ctx->num_sms * 2, th = 512, iters = 40000;
+    double *d = nullptr, *in = nullptr;
+    CU(cudaMalloc(&d, sizeof(double) * (size_t)nb * th));
+    if (cudaMalloc(&in, sizeof(double) * 24) != cudaSuccess) { cudaFree(d); return fail(ctx, TRIMEG_ERR_OOM, "bench_dfma_mix: out of device memory"); }
+    double h[24];
+    for (int q = 0; q < 8; ++q) { h[q] = 1.0 + q; h[8 + q] = 1.0000001 + 1e-9 * q; h[16 + q] = 1e-9 * (1 + q); }
+    cudaMemcpyAsync(in, h, sizeof h, cudaMemcpyHostToDevice, ctx->stream);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 6; ++rep) {     // the first is the warm-up
+        cudaEventRecord(e0, ctx->stream);
+        if (kind == 1) k_dfma_mix<1><<<nb, th, 0, ctx->stream>>>(in, d, iters);
+        else k_dfma_mix<2><<<nb, th, 0, ctx->stream>>>(in, d, iters);
+        cudaEventRecord(e1, ctx->stream);
+        cudaEventSynchronize(e1);
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaError_t e = cudaGetLastError();
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d); cudaFree(in);
+    if (e != cudaSuccess) return fail(ctx, TRIMEG_ERR_CUDA, "bench_dfma_mix: %s", cudaGetErrorString(e));
+    *tflops = 2.0 * 8 * (double)iters * nb * th / (best * 1e-3) * 1e-12;
+    return TRIMEG_OK;
+}
+
 int trimeg_push_stats(trimeg_ctx* ctx, int64_t out[4]) {
     if (!ctx || !out) return TRIMEG_ERR_BAD_ARG;
     for (int i = 0; i < 4; ++i) out[i] = ctx->stats[i];

@@ -797,4 +797,19 @@ __global__ void __launch_bounds__(512) k_dfma(double* out, int iters, double a, 
     out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
 }
 
+// the same loop with the operands a real evaluation has: KIND 1: three different register pairs per DFMA (accumulator,
+// multiplier, addend); KIND 2: Horner-like, one multiplier shared by the eight chains, addends different.  The values come
+// from memory so that nothing folds.
+template <int KIND>
+__global__ void __launch_bounds__(512) k_dfma_mix(const double* __restrict__ in, double* out, int iters) {
+    double x[8], y[8], z[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { x[q] = in[q] + threadIdx.x; y[q] = in[8 + q] + 1e-13 * threadIdx.x; z[q] = in[16 + q] * (1.0 + threadIdx.x); }   // per-thread values: vector registers
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) x[q] = fma(x[q], KIND == 1 ? y[q] : y[0], z[q]);
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x[0] + x[1]) + (x[2] + x[3])) + ((x[4] + x[5]) + (x[6] + x[7]));
+}
+
 }  // namespace trimeg
