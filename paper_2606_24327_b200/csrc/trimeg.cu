@@ -729,20 +729,17 @@ static int run_phase(trimeg_ctx* ctx, double dt, bool sort_now, bool keys_out, c
                                                                                            ctx->d_work);
     KCHECK();
     if (ev) CU(cudaEventRecord(ev[1], ctx->stream));
-    // markers that left their staged block, then markers outside the mesh (sorted behind the last cell): global tables
-    k_phase_global<PHASE><<<ctx->num_sms * 16, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->cm, ko, src, dst, perm, ctx->d_retired, nullptr,
-                                                                      ctx->d_work + 4, ctx->n, dt);
-    KCHECK();
-    k_phase_global<PHASE><<<ctx->num_sms * 2, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->cm, ko, src, dst, perm, nullptr, ctx->d_offs + ctx->ncell,
-                                                                      nullptr, ctx->n, dt);
-    KCHECK();
-    k_fix_keys<PHASE><<<ctx->num_sms * 16, 128, 0, ctx->stream>>>(ctx->tb, ctx->cm, ko, dst, ctx->d_retired, ctx->d_work + 5, ctx->n, dt);
-    KCHECK();
+    // follow-ups in one launch: markers that left their staged block and markers outside the mesh (sorted behind the last cell)
+    // through the global tables, sort keys of the markers whose next point left the staged geometry, statistics
+    {
+        const int nbA = ctx->num_sms * 12, nbB = ctx->num_sms * 2, nbC = ctx->num_sms * 12;
+        k_followups<PHASE><<<nbA + nbB + nbC, 128, 0, ctx->stream>>>(ctx->tb, ctx->ep, ctx->sp, ctx->cm, ko, src, dst, perm, ctx->d_retired, ctx->d_work,
+                                                                     ctx->d_offs + ctx->ncell, ctx->n, dt, ctx->d_stats + 1, nbA, nbB);
+        KCHECK();
+    }
     if (sort_now) ctx->cur ^= 1;
-    k_accumulate_stat<<<1, 1, 0, ctx->stream>>>(ctx->d_work + 4, ctx->d_stats + 1);
-    KCHECK();
     if (ev) CU(cudaEventRecord(ev[2], ctx->stream));
-    ctx->stats[0] += 5;
+    ctx->stats[0] += 2;
     return TRIMEG_OK;
 }
 

@@ -367,14 +367,13 @@ __device__ __forceinline__ void phase_global(const DevTables& tb, const EquilP& 
 // positions m = index[i] (or i if index is null) of the cell order for i in [*first (or 0), *count (or n)):
 // record src[perm[m]] (or src[m] if perm is null) -> dst[m]
 template <int PHASE>
-__global__ void __launch_bounds__(128) k_phase_global(DevTables tb, EquilP ep, SpeciesP sp, CellMap cm, KeyOut ko, const Rec* src,
-                                                      Rec* dst, const int* __restrict__ perm, const int* __restrict__ index,
-                                                      const int* __restrict__ first, const int* __restrict__ count, long long n, double dt) {
-    const long long lo = first ? (long long)*first : 0, hi = count ? (long long)*count : n;
+__device__ __forceinline__ void phase_global_range(const DevTables& tb, const EquilP& ep, const SpeciesP& sp, const CellMap& cm, const KeyOut& ko, const Rec* src,
+                                                   Rec* dst, const int* __restrict__ perm, const int* __restrict__ index, long long lo, long long hi,
+                                                   double dt, int bid, int nblocks) {
     // whole warps go round the loop together (the lanes of the last round that have no record sit it out), so that the lanes
     // with a record can be named for the reconvergence points inside
     const int lane = threadIdx.x & 31;
-    for (long long base = lo + (long long)blockIdx.x * blockDim.x + (threadIdx.x - lane); base < hi; base += (long long)gridDim.x * blockDim.x) {
+    for (long long base = lo + (long long)bid * blockDim.x + (threadIdx.x - lane); base < hi; base += (long long)nblocks * blockDim.x) {
         const long long i = base + lane;
         const unsigned lanes = __ballot_sync(0xffffffffu, i < hi);
         if (i < hi) {
@@ -382,6 +381,13 @@ __global__ void __launch_bounds__(128) k_phase_global(DevTables tb, EquilP ep, S
             phase_global<PHASE>(tb, ep, sp, cm, ko, src, dst, perm ? (long long)perm[m] : m, m, dt, lanes);
         }
     }
+}
+template <int PHASE>
+__global__ void __launch_bounds__(128) k_phase_global(DevTables tb, EquilP ep, SpeciesP sp, CellMap cm, KeyOut ko, const Rec* src,
+                                                      Rec* dst, const int* __restrict__ perm, const int* __restrict__ index,
+                                                      const int* __restrict__ first, const int* __restrict__ count, long long n, double dt) {
+    const long long lo = first ? (long long)*first : 0, hi = count ? (long long)*count : n;
+    phase_global_range<PHASE>(tb, ep, sp, cm, ko, src, dst, perm, index, lo, hi, dt, (int)blockIdx.x, (int)gridDim.x);
 }
 
 // first step after a bind: triangle and cell key of every marker's CURRENT position (box-grid locate), so that k1 = f(y_n)
@@ -405,10 +411,9 @@ __global__ void __launch_bounds__(256) k_locate_keys(DevTables tb, CellMap cm, K
 // the triangle of that point (the record holds a hint) and the sort key.  Next point: after phase A the stage-4 position held
 // in k, otherwise y + dt/2 k.
 template <int PHASE>
-__global__ void __launch_bounds__(128) k_fix_keys(DevTables tb, CellMap cm, KeyOut ko, Rec* recs, const int* __restrict__ list, const int* __restrict__ count,
-                                                  long long n, double dt) {
-    const int cnt = *count;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < cnt; i += gridDim.x * blockDim.x) {
+__device__ __forceinline__ void fix_keys_range(const DevTables& tb, const CellMap& cm, const KeyOut& ko, Rec* recs, const int* __restrict__ list, int cnt,
+                                               long long n, double dt, int bid, int nblocks) {
+    for (int i = bid * blockDim.x + threadIdx.x; i < cnt; i += nblocks * blockDim.x) {
         const long long m = list[n - 1 - i];
         Rec r;
         rec_load(recs, m, r);
@@ -425,6 +430,34 @@ __global__ void __launch_bounds__(128) k_fix_keys(DevTables tb, CellMap cm, KeyO
             ko.keys[m] = key;
             atomicAdd(ko.hist + key, 1);
         }
+    }
+}
+template <int PHASE>
+__global__ void __launch_bounds__(128) k_fix_keys(DevTables tb, CellMap cm, KeyOut ko, Rec* recs, const int* __restrict__ list, const int* __restrict__ count,
+                                                  long long n, double dt) {
+    fix_keys_range<PHASE>(tb, cm, ko, recs, list, *count, n, dt, (int)blockIdx.x, (int)gridDim.x);
+}
+#ifndef TRIMEG_FU_OCC
+#define TRIMEG_FU_OCC 4
+#endif
+// The three follow-ups of a phase in ONE launch (they touch disjoint markers, each alone is a short latency-bound kernel):
+// blocks [0, nbA): the markers the tiled kernel retired (list `retired`, *work[4] of them); [nbA, nbA + nbB): the markers
+// outside the mesh, sorted behind the last cell (positions from *outside_first); the rest: sort keys of the markers whose
+// next evaluation point left the staged geometry (the same list from its end, work[5] of them).  Thread 0 also adds the
+// retired count to the statistics.
+template <int PHASE>
+__global__ void __launch_bounds__(128, TRIMEG_FU_OCC) k_followups(DevTables tb, EquilP ep, SpeciesP sp, CellMap cm, KeyOut ko, const Rec* src, Rec* dst,
+                                                   const int* __restrict__ perm, const int* __restrict__ retired, const int* __restrict__ work,
+                                                   const int* __restrict__ outside_first, long long n, double dt, unsigned long long* __restrict__ stat,
+                                                   int nbA, int nbB) {
+    const int b = (int)blockIdx.x;
+    if (b == 0 && threadIdx.x == 0) atomicAdd(stat, (unsigned long long)work[4]);
+    if (b < nbA + nbB) {
+        const bool listed = b < nbA;
+        const long long lo = listed ? 0 : (long long)*outside_first, hi = listed ? (long long)work[4] : n;
+        phase_global_range<PHASE>(tb, ep, sp, cm, ko, src, dst, perm, listed ? retired : nullptr, lo, hi, dt, listed ? b : b - nbA, listed ? nbA : nbB);
+    } else {
+        fix_keys_range<PHASE>(tb, cm, ko, dst, retired, work[5], n, dt, b - nbA - nbB, (int)gridDim.x - nbA - nbB);
     }
 }
 
